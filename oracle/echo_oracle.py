@@ -1,0 +1,278 @@
+"""CPU ORACLE for the ECHO super-tree verify step -- TEST INFRASTRUCTURE ONLY.
+
+Plain, slow, obviously-correct numpy / pure-Python restatement of what the hot
+path computes.  It shares no code with the CUDA path (`paper_2604_09603_b200/csrc`)
+and imports nothing from the package.  Only `tests/`, `__graft_entry__.smoke()`
+and `bench.py`'s cpu_baseline / `--impl reference` legs may import it.
+
+Citations `P:<n>` are lines of /root/reference/PAPER.md; `S:<id>` are readings
+of SURVEY.md §8(c), restated in DESIGN.md §3.
+
+Pins (tests/test_oracle_pins.py, `-m "not gpu"`): worked example W1
+(tests/golden/w1.json), exactly-representable chain scores, Q=0 closed form,
+chain == dense causal attention, single node == decode attention, brute-force
+dense masked softmax, Python `sorted()` selection, exhaustive path enumeration.
+The paper prints no numeric example of this path, so parity with
+"the paper's values" is unpinned; every function below is pinned by the
+mathematics listed above.
+
+Precision: path scores fp32 sequential root->leaf (north_star); attention fp64.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+INT32_MAX = 2**31 - 1
+PAGE = 16
+D = 128
+
+
+# ---------------------------------------------------------------- O1 (S1)
+def path_scores(cand_offsets, parent, logq):
+    """Eq. 5: S[j] = S[pa(j)] + log q[j], fp32, strictly root->leaf
+    in node-index order (parent[j] < j); roots: S = 0.0f + logq (S:G-1, G-3, G-13)."""
+    N = int(cand_offsets[-1])
+    S = np.zeros(N, np.float32)
+    depth = np.zeros(N, np.uint8)
+    for i in range(len(cand_offsets) - 1):
+        b = int(cand_offsets[i])
+        for j in range(int(cand_offsets[i + 1]) - b):
+            p = int(parent[b + j])
+            if p < 0:
+                depth[b + j] = 0
+                S[b + j] = np.float32(0.0) + np.float32(logq[b + j])
+            else:
+                depth[b + j] = depth[b + p] + 1
+                S[b + j] = np.float32(S[b + p]) + np.float32(logq[b + j])
+    return S, depth
+
+
+# ---------------------------------------------------------------- O2 (S2)
+def gate_cut_depth(cand_offsets, S, depth, depth_mask, log_tau):
+    """Eq. 6-7; Alg. 1 l.8.  m[i][d] = max_j S over level d;
+    for gated depths ascending: pass iff m > log_tau[d] (log domain, strict; S:G-4);
+    an absent level is skipped (S:G-5); first failure = cut depth, else INT32_MAX."""
+    R = len(cand_offsets) - 1
+    cut = np.full(R, INT32_MAX, np.int32)
+    for i in range(R):
+        b, e = int(cand_offsets[i]), int(cand_offsets[i + 1])
+        for d in range(32):
+            if not (depth_mask >> d) & 1:
+                continue
+            lvl = [S[j] for j in range(b, e) if depth[j] == d]
+            if not lvl:
+                continue
+            m = max(lvl)
+            if not (np.float32(m) > np.float32(log_tau[d])):
+                cut[i] = d
+                break
+    return cut
+
+
+# ---------------------------------------------------------------- O3 (S3)
+def select(cand_offsets, S, depth, cut, budget, w_max, static_k=0):
+    """Eq. 4; Alg. 1; priority rule P:162-167 (S:G-7..G-12, G-15).
+    Returns the selected (request, node) pairs as a set-like sorted list."""
+    R = len(cand_offsets) - 1
+    if static_k > 0:
+        out = []
+        for i in range(R):
+            b, e = int(cand_offsets[i]), int(cand_offsets[i + 1])
+            order = sorted(range(e - b), key=lambda j: (-float(S[b + j]), j))
+            out += [(i, j) for j in order[:static_k]]
+        return sorted(out)
+    elig = []
+    for i in range(R):
+        b, e = int(cand_offsets[i]), int(cand_offsets[i + 1])
+        c = int(cut[i])
+        for j in range(e - b):
+            if depth[b + j] < c:
+                elig.append((0, -float(S[b + j]), i, j))           # tier 0: depth extension
+        lvl = sorted([j for j in range(e - b) if depth[b + j] == c], key=lambda j: (-float(S[b + j]), j))
+        for j in lvl[:max(0, w_max)]:
+            elig.append((1, -float(S[b + j]), i, j))               # tier 1: width expansion
+    elig.sort()
+    return sorted((i, j) for (_, _, i, j) in elig[:max(0, budget)])
+
+
+# ---------------------------------------------------------------- O4 + O5 (S4, S5)
+def pack(cand_offsets, parent, depth, selected, R):
+    """Flatten & Pack, Fig. 3(3): request asc, node asc (S:P-1); CSR offsets,
+    local parent remap, 128-bit ancestor-or-self masks as Python ints (S5)."""
+    sel_offsets = np.zeros(R + 1, np.int32)
+    sel_node, sel_req, parent_local, sel_depth, masks = [], [], [], [], []
+    by_req = [[] for _ in range(R)]
+    for (i, j) in selected:
+        by_req[i].append(j)
+    for i in range(R):
+        nodes = sorted(by_req[i])
+        loc = {j: l for l, j in enumerate(nodes)}
+        b = int(cand_offsets[i])
+        req_masks = []
+        for l, j in enumerate(nodes):
+            p = int(parent[b + j])
+            pl = -1 if p < 0 else loc[p]          # KeyError = ancestor closure (I2) violated
+            sel_node.append(j); sel_req.append(i); parent_local.append(pl)
+            sel_depth.append(int(depth[b + j]))
+            req_masks.append((1 << l) | (req_masks[pl] if pl >= 0 else 0))
+        masks += req_masks
+        sel_offsets[i + 1] = sel_offsets[i] + len(nodes)
+    anc = np.zeros((len(masks), 4), np.uint32)
+    for k, m in enumerate(masks):
+        for w in range(4):
+            anc[k, w] = (m >> (32 * w)) & 0xFFFFFFFF
+    return dict(n_selected=len(sel_node), sel_offsets=sel_offsets,
+                sel_node=np.asarray(sel_node, np.int32), sel_req=np.asarray(sel_req, np.int32),
+                parent_local=np.asarray(parent_local, np.int32),
+                sel_depth=np.asarray(sel_depth, np.uint8), anc_mask=anc, masks=masks)
+
+
+def gate_select(cand_offsets, parent, logq, depth_mask, log_tau, w_max, budget, static_k=0):
+    """S1-S5 end to end (what `echo_gate_select` must reproduce bit-exactly)."""
+    R = len(cand_offsets) - 1
+    S, depth = path_scores(cand_offsets, parent, logq)
+    if static_k > 0:
+        cut = np.full(R, INT32_MAX, np.int32)
+    else:
+        cut = gate_cut_depth(cand_offsets, S, depth, depth_mask, log_tau)
+    sel = select(cand_offsets, S, depth, cut, budget, w_max, static_k)
+    out = pack(cand_offsets, parent, depth, sel, R)
+    out.update(path_score=S, cand_depth=depth, cut_depth=cut)
+    return out
+
+
+# ---------------------------------------------------------------- O6 + O7 (S6, S7)
+def bf16_bits_to_f64(u16):
+    """exact bf16 (stored as uint16 bit patterns) -> float64."""
+    return (np.asarray(u16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def visible_positions(P_i, mask):
+    """prefix [0,P_i) then P_i + a for every set bit a of the ancestor-or-self mask (S:A-1, A-2)."""
+    return list(range(int(P_i))) + [int(P_i) + a for a in range(128) if (mask >> a) & 1]
+
+
+def verify_attn(sel, q_bits, k_pool_bits, v_pool_bits, page_table, prefix_len, Hq, Hkv, sm_scale,
+                layer=0, rows=None):
+    """Plain dense definition softmax(sm_scale * q K^T) V over the visible set, fp64, no
+    splitting, no online softmax (S:A-1..A-5).  q_bits uint16 [cap][Hq][128]; pools uint16
+    [layers][pages][Hkv][16][128].  `rows` = optional list of (packed node, head) pairs to
+    compute (sampled parity at full size); default all.  Returns {(k,h): (O[128], lse)} if
+    rows given else (out [n][Hq][128] f64, lse [n][Hq] f64)."""
+    G = Hq // Hkv
+    offs = sel["sel_offsets"]
+    n = int(sel["n_selected"])
+    sel_req = sel["sel_req"]
+    scale = float(np.float32(sm_scale))
+
+    def one(k, heads):
+        i = int(sel_req[k])
+        l = k - int(offs[i])
+        pos = visible_positions(prefix_len[i], sel["masks"][k] if "masks" in sel else
+                                sum(int(sel["anc_mask"][k, w]) << (32 * w) for w in range(4)))
+        pg = np.asarray([page_table[i][t // PAGE] for t in pos], np.int64)
+        sl = np.asarray([t % PAGE for t in pos], np.int64)
+        res = {}
+        cache = {}
+        for h in heads:
+            kvh = h // G
+            if kvh not in cache:
+                cache[kvh] = (bf16_bits_to_f64(k_pool_bits[layer, pg, kvh, sl, :]),
+                              bf16_bits_to_f64(v_pool_bits[layer, pg, kvh, sl, :]))
+            Kt, Vt = cache[kvh]
+            qv = bf16_bits_to_f64(q_bits[k, h, :])
+            s = scale * (Kt @ qv)
+            M = s.max()
+            e = np.exp(s - M)
+            Z = e.sum()
+            res[h] = ((e @ Vt) / Z, M + np.log(Z))
+        return res
+
+    if rows is not None:
+        out = {}
+        by_k = {}
+        for (k, h) in rows:
+            by_k.setdefault(int(k), []).append(int(h))
+        for k, hs in by_k.items():
+            r = one(k, hs)
+            for h in hs:
+                out[(k, h)] = r[h]
+        return out
+    O = np.zeros((n, Hq, D), np.float64)
+    L = np.zeros((n, Hq), np.float64)
+    for k in range(n):
+        r = one(k, range(Hq))
+        for h in range(Hq):
+            O[k, h], L[k, h] = r[h]
+    return O, L
+
+
+# ---------------------------------------------------------------- O8 (S8)
+def argmax_bf16(logits_bits, vocab):
+    """greedy target token: first maximum of each row over v < vocab (S:C-3).
+    numpy.argmax returns the first occurrence; pinned against an explicit strict-'>' scan."""
+    x = (np.asarray(logits_bits)[:, :vocab].astype(np.uint32) << 16).view(np.float32)
+    return np.argmax(x, axis=1).astype(np.int32)
+
+
+# ---------------------------------------------------------------- O9 (S9)
+def accept(sel, draft_token, prev_token, target_token, R):
+    """Greedy acceptance (S:C-1, C-2, C-4, C-5): acc[l] = parent accepted
+    and draft[l] == target token after the parent (roots: == prev_token); best = accepted
+    node of maximum depth, lowest local index; path = its ancestor-or-self set ascending."""
+    offs = sel["sel_offsets"]
+    accept_len = np.zeros(R, np.int32)
+    last_node = np.full(R, -1, np.int32)
+    bonus = np.full(R, -1, np.int32)
+    accept_idx = np.full((R, 32), -1, np.int32)
+    for i in range(R):
+        b, e = int(offs[i]), int(offs[i + 1])
+        acc = []
+        best, best_d = -1, -1
+        for l in range(e - b):
+            pl = int(sel["parent_local"][b + l])
+            if pl < 0:
+                a = int(draft_token[b + l]) == int(prev_token[i])
+            else:
+                a = acc[pl] and int(draft_token[b + l]) == int(target_token[b + pl])
+            acc.append(bool(a))
+            if a and int(sel["sel_depth"][b + l]) > best_d:
+                best, best_d = l, int(sel["sel_depth"][b + l])
+        if best < 0:
+            continue
+        m = sum(int(sel["anc_mask"][b + best, w]) << (32 * w) for w in range(4))
+        path = [a for a in range(128) if (m >> a) & 1]
+        accept_len[i] = len(path)
+        accept_idx[i, :len(path)] = [b + a for a in path]
+        last_node[i] = b + best
+        bonus[i] = int(target_token[b + best])
+    return dict(accept_len=accept_len, accept_idx=accept_idx, last_node=last_node, bonus_token=bonus)
+
+
+# ---------------------------------------------------------------- O10 (S10)
+def compact_kv(sel, acc, k_pool_bits, v_pool_bits, page_table, prefix_len, R):
+    """KV-slot compaction (S:C-6): path node t moves from position P_i + a_t to P_i + t;
+    slot(i,pos) = page_table[i][pos/16]*16 + pos%16; all layers, all KV heads, K and V; every
+    read happens before any write.  Pools (uint16 views) are updated IN PLACE."""
+    slot_src = np.full((R, 32), -1, np.int32)
+    slot_dst = np.full((R, 32), -1, np.int32)
+    new_len = np.zeros(R, np.int32)
+    offs = sel["sel_offsets"]
+    for i in range(R):
+        P = int(prefix_len[i])
+        L = int(acc["accept_len"][i])
+        new_len[i] = P + L
+        tmp = []
+        for t in range(L):
+            a = int(acc["accept_idx"][i, t]) - int(offs[i])
+            sp, dp = P + a, P + t
+            slot_src[i, t] = int(page_table[i][sp // PAGE]) * PAGE + sp % PAGE
+            slot_dst[i, t] = int(page_table[i][dp // PAGE]) * PAGE + dp % PAGE
+            s = int(slot_src[i, t])
+            tmp.append((k_pool_bits[:, s // PAGE, :, s % PAGE, :].copy(),
+                        v_pool_bits[:, s // PAGE, :, s % PAGE, :].copy()))
+        for t in range(L):
+            d = int(slot_dst[i, t])
+            k_pool_bits[:, d // PAGE, :, d % PAGE, :] = tmp[t][0]
+            v_pool_bits[:, d // PAGE, :, d % PAGE, :] = tmp[t][1]
+    return dict(slot_src=slot_src, slot_dst=slot_dst, new_len=new_len)
