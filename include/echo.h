@@ -1,0 +1,171 @@
+/* echo.h -- C ABI of libecho.so: the batch-wide "super-tree" verify step of ECHO
+ * (arxiv 2604.09603) as hand-written CUDA for one B200 (sm_100a).
+ *
+ * Citations: `P:<n>` = line <n> of the paper text; `R:<id>` = a reading of a
+ * point the paper leaves open, listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every pointer marked "dev" is DEVICE memory owned by the caller; it must stay valid
+ *     until the work queued on `stream` has finished.  Structs themselves are HOST memory,
+ *     read during the call only.
+ *   - All three compute calls are asynchronous on `stream`, never synchronise, never read a
+ *     device result on the host (CUDA-graph capturable).  Data-dependent sizes
+ *     (n_selected, K_i, P_i) live on the device only.
+ *   - Return value: ECHO_OK (0) or a negative EchoStatus.  Data-dependent precondition
+ *     violations cannot be seen by the host; they set bits in the device status word
+ *     (echo_device_status) and leave outputs unspecified.  Nothing traps.
+ *   - There is no CPU fallback and no dispatch on architecture: echo_create fails with
+ *     ECHO_ERR_ARCH unless the device has compute capability 10.0.
+ *   - R = number of requests (the paper's batch size B); the paper's budget K_max
+ *     (Eq. 4) is `budget`.
+ */
+#ifndef ECHO_H_
+#define ECHO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct EchoCtx EchoCtx;  /* opaque; owns the workspace */
+typedef void* echo_stream_t;     /* a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
+
+typedef enum {
+  ECHO_OK = 0,
+  ECHO_ERR_INVALID_ARG = -1, /* NULL pointer, negative size, capacity too small, misaligned pointer */
+  ECHO_ERR_UNSUPPORTED = -2, /* head_dim != 128, page_size != 16, Hq % Hkv != 0, max_cand_per_req > 128 */
+  ECHO_ERR_WORKSPACE = -3,   /* ctx workspace smaller than echo_workspace_bytes(...) for this call */
+  ECHO_ERR_ARCH = -4,        /* device is not sm_100 */
+  ECHO_ERR_CUDA = -5         /* a CUDA runtime / driver call failed; text via echo_last_error */
+} EchoStatus;
+
+/* bits of the device status word */
+#define ECHO_DEV_BAD_PARENT 1u   /* parent[j] >= j or < -1 */
+#define ECHO_DEV_BAD_LOGQ 2u     /* logq > 0 or NaN */
+#define ECHO_DEV_DEPTH_OVERFLOW 4u /* a candidate deeper than 31 */
+#define ECHO_DEV_PAGE_OVERFLOW 8u  /* P_i + K_i needs more than max_pages_per_req pages */
+
+/* test / tuning hooks for echo_set_option */
+#define ECHO_OPT_FORCE_SPLITS 1   /* >0: split every KV stream into exactly this many parts (<= 16) */
+#define ECHO_OPT_ATTN_PATH 2      /* 0 = auto, 1 = CUDA-core small-row kernel, 2 = tcgen05 kernel */
+#define ECHO_OPT_NUM_CTAS 3       /* >0: persistent grid size of the tcgen05 kernel (default: #SMs) */
+
+#define ECHO_MAX_CAND 128   /* C_i <= 128 candidates per request (R:G-14) */
+#define ECHO_MAX_DEPTH 32   /* depth < 32 (R:G-14) */
+#define ECHO_MAX_ACCEPT 32  /* an accepted path has <= 32 nodes (one per depth) */
+#define ECHO_CUT_NEVER 0x7fffffff
+
+/* ---- lifetime ------------------------------------------------------------------------ */
+/* Creates a context on `device` with a workspace of `workspace_bytes` (device memory, owned by
+ * the context, freed by echo_destroy).  ECHO_ERR_ARCH unless compute capability is 10.0. */
+int echo_create(EchoCtx** out, int device, size_t workspace_bytes);
+int echo_destroy(EchoCtx* ctx);
+/* Workspace needed by any call with at most these sizes: select keys [total_cand], split-KV
+ * partials for 16 splits [capacity][num_q_heads] x (128+2) fp32, plan arrays. */
+size_t echo_workspace_bytes(int32_t num_requests, int32_t total_cand, int32_t capacity, int32_t num_q_heads);
+const char* echo_strerror(int code);
+const char* echo_last_error(EchoCtx* ctx);  /* text of the last ECHO_ERR_CUDA on this context */
+/* Copies the device status word to *flags with a blocking 4-byte copy on `stream` and clears it. */
+int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream);
+int echo_set_option(EchoCtx* ctx, int key, int64_t value);
+
+/* ---- problem statement ----------------------------------- */
+/* Candidate draft trees G_i with parent function pa(j) and draft log-probabilities (Eq. 5). */
+typedef struct {
+  int32_t num_requests;     /* R >= 0 */
+  int32_t total_cand;       /* N = sum C_i */
+  int32_t max_cand_per_req; /* max C_i, <= ECHO_MAX_CAND */
+  const int32_t* cand_offsets; /* dev [R+1], CSR, cand_offsets[0] = 0 */
+  const int32_t* parent;       /* dev [N], request-local, -1 = root, parent[j] < j (topological) */
+  const float* logq;           /* dev [N], natural log of the draft confidence q(x|h), <= 0 (R:G-2) */
+} EchoTrees;
+
+/* Gate and scheduler parameters: Alg. 1 inputs (K_max, D_sig, tau, W_max). */
+typedef struct {
+  uint32_t depth_mask; /* bit d set <=> d in D_sig (Eq. 7) */
+  float log_tau[32];   /* natural log of tau_d; compared as max_j S > log_tau[d], strict (R:G-4) */
+  int32_t w_max;       /* Phase-2 width cap per truncated request; 0 = no widening */
+  int32_t budget;      /* K_max >= 0 (Eq. 4) */
+  int32_t static_k;    /* 0 = elastic global top-B; >0 = per-request top-static_k, gates off (R:G-15) */
+} EchoGate;
+
+/* Packed ragged batch ("Flatten & Pack", Fig. 3(3)): request asc, node asc (R:P-1). */
+typedef struct {
+  int32_t capacity;       /* >= budget (elastic) or >= min(N, R*static_k) (static) */
+  int32_t* n_selected;    /* dev [1] */
+  int32_t* sel_offsets;   /* dev [R+1] CSR over packed nodes; K_i = sel_offsets[i+1]-sel_offsets[i] */
+  int32_t* sel_node;      /* dev [capacity] request-local candidate id */
+  int32_t* sel_req;       /* dev [capacity] */
+  int32_t* parent_local;  /* dev [capacity] packed request-local parent index, -1 = root */
+  uint8_t* sel_depth;     /* dev [capacity] */
+  uint32_t* anc_mask;     /* dev [capacity][4] ancestor-or-self bits over packed local indices */
+  float* path_score;      /* dev [N]  S (Eq. 5) */
+  uint8_t* cand_depth;    /* dev [N] */
+  int32_t* cut_depth;     /* dev [R] first failing gated depth, ECHO_CUT_NEVER if none */
+} EchoSelection;
+
+/* Paged KV cache (R:A-2, A-3): pools bf16 [num_layers][num_pages][num_kv_heads][16][128];
+ * token position t of request i lives in page page_table[i][t/16], slot t%16.  The packed tree
+ * node with local index l is tentatively appended at position prefix_len[i] + l. */
+typedef struct {
+  int32_t num_kv_heads, head_dim /* 128 */, page_size /* 16 */, num_pages, max_pages_per_req, num_layers;
+  void* k_pool;              /* dev, 16-byte aligned */
+  void* v_pool;              /* dev, 16-byte aligned */
+  const int32_t* page_table; /* dev [R][max_pages_per_req] */
+  const int32_t* prefix_len; /* dev [R]  P_i >= 0 */
+} EchoPagedKV;
+
+/* What the target model said (greedy): tokens directly, or bf16 logits to argmax. */
+typedef struct {
+  const int32_t* draft_token;  /* dev [capacity] packed order */
+  const int32_t* prev_token;   /* dev [R] target's greedy token after the committed prefix (R:C-2) */
+  const int32_t* target_token; /* dev [capacity] target's greedy token AFTER each packed node, or NULL */
+  const void* target_logits;   /* dev bf16 [capacity][ld], 16-byte aligned, or NULL; exactly one of the two */
+  int32_t vocab;               /* V (argmax over columns < V) */
+  int64_t ld;                  /* row stride in elements, >= V, multiple of 8 */
+} EchoVerifyResult;
+
+typedef struct {
+  int32_t* accept_len;   /* dev [R] accepted draft nodes on the chosen path (R:C-5) */
+  int32_t* last_node;    /* dev [R] packed index of the deepest accepted node, -1 if none */
+  int32_t* bonus_token;  /* dev [R] target token after last_node, -1 if none */
+  int32_t* new_len;      /* dev [R] P_i + accept_len */
+  int32_t* accept_idx;   /* dev [R][32] packed indices along the path, -1 padded */
+  int32_t* slot_src;     /* dev [R][32] KV slot (page*16+offset) each path node is read from */
+  int32_t* slot_dst;     /* dev [R][32] KV slot it is moved to (position P_i + t) */
+  int32_t* target_token_out; /* dev [capacity] argmax result (logits form), may be NULL */
+} EchoAccept;
+
+/* ---- the three calls of the hot path ------------------------------------------------------ */
+
+/* S1-S5: fp32 path scores accumulated root->leaf (Eq. 5), layer confidence and sparse
+ * gate in the log domain (Eq. 6-7), budgeted global top-B selection with depth
+ * extension (tier 0) strictly before width expansion (tier 1) (Eq. 4, Alg. 1, priority
+ * P:162-167), ties by (score desc, request, node); then packing and 128-bit ancestor masks.
+ * Writes every field of `out`.  Needs workspace >= echo_workspace_bytes(R, N, capacity, 0). */
+int echo_gate_select(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, EchoSelection* out,
+                     echo_stream_t stream);
+
+/* S6-S7: ragged tree-masked paged GQA attention (the "specialized operators for irregular batch
+ * shapes"; definition R:A-1..A-8).  For packed node k = (i,l) and query head h
+ * (KV head h / (Hq/Hkv)): softmax over positions [0,P_i) and P_i + a for every set bit a of
+ * anc_mask[k], logits sm_scale * <q, k_t>; out = sum p_t v_t (bf16, RNE), lse = ln sum exp.
+ * q/out: dev bf16 [capacity][num_q_heads][128], 16-byte aligned; lse: dev f32 [capacity][num_q_heads].
+ * Rows k >= n_selected are not written.  Slots past P_i + K_i may hold any bits, NaN included. */
+int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer,
+                     int32_t num_q_heads, int32_t num_requests, const void* q, void* out, float* lse,
+                     float sm_scale, echo_stream_t stream);
+
+/* S8-S10: optional fused argmax over bf16 target logits (lowest index wins ties, R:C-3), greedy
+ * acceptance = longest accepted root-to-leaf path (max depth, then lowest local index; P:52,
+ * P:199, R:C-1..C-5), and in-place compaction of the accepted KV rows of all layers to positions
+ * P_i .. P_i+L-1, every read before any write to the same slot column (R:C-6). */
+int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t num_requests,
+                EchoPagedKV* kv, EchoAccept* out, echo_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ECHO_H_ */

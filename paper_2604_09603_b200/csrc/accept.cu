@@ -1,0 +1,217 @@
+// echo_accept: S8 (bf16 argmax over the vocabulary), S9 (greedy acceptance = longest accepted
+// root-to-leaf path) and S10 (in-place KV-slot compaction, R:C-6).
+#include "common.cuh"
+
+namespace {
+
+constexpr int D = 128;
+constexpr int PAGE = 16;
+
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+// (value, index) with "greater value, then lower index" order; -0 == +0 by float compare (R:C-3)
+__device__ __forceinline__ void amax_upd(float& bv, int& bi, float v, int i) {
+  if (v > bv || (v == bv && i < bi)) { bv = v; bi = i; }
+}
+
+__device__ __forceinline__ void amax_chunk(float& bv, int& bi, const uint4 u, int base) {
+  // ascending index with strict '>' keeps the first maximum
+  const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const float lo = __uint_as_float(w[c] << 16), hi = __uint_as_float(w[c] & 0xffff0000u);
+    if (lo > bv) { bv = lo; bi = base + 2 * c; }
+    if (hi > bv) { bv = hi; bi = base + 2 * c + 1; }
+  }
+}
+
+constexpr int AM_THREADS = 256;
+constexpr int AM_UNROLL = 4;
+
+// S8: one CTA per packed node row; 16-byte streaming loads, 4 in flight per thread.
+__global__ void __launch_bounds__(AM_THREADS) k_argmax_bf16(const int32_t* __restrict__ n_selected,
+                                                            const __nv_bfloat16* __restrict__ logits, int64_t ld,
+                                                            int vocab, int32_t* __restrict__ target_token) {
+  const int row = blockIdx.x;
+  if (row >= *n_selected) return;
+  const __nv_bfloat16* rp = logits + (size_t)row * ld;
+  const uint4* rp4 = reinterpret_cast<const uint4*>(rp);
+  const int nvec = vocab / 8;
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  int v = threadIdx.x;
+  for (; v + (AM_UNROLL - 1) * AM_THREADS < nvec; v += AM_UNROLL * AM_THREADS) {
+    uint4 u[AM_UNROLL];
+#pragma unroll
+    for (int t = 0; t < AM_UNROLL; ++t) u[t] = ldg_stream(rp4 + v + t * AM_THREADS);
+#pragma unroll
+    for (int t = 0; t < AM_UNROLL; ++t) amax_chunk(bv, bi, u[t], (v + t * AM_THREADS) * 8);
+  }
+  for (; v < nvec; v += AM_THREADS) amax_chunk(bv, bi, ldg_stream(rp4 + v), v * 8);
+  for (int c = nvec * 8 + threadIdx.x; c < vocab; c += AM_THREADS) {
+    const float x = __bfloat162float(rp[c]);
+    if (x > bv) { bv = x; bi = c; }
+  }
+  // an all -inf (or empty) slice leaves bi at INT_MAX; the tie rule then picks any real index
+#pragma unroll
+  for (int ofs = 16; ofs; ofs >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, bv, ofs);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, ofs);
+    amax_upd(bv, bi, ov, oi);
+  }
+  __shared__ float s_v[AM_THREADS / 32];
+  __shared__ int s_i[AM_THREADS / 32];
+  if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = bv; s_i[threadIdx.x >> 5] = bi; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < AM_THREADS / 32; ++w) amax_upd(bv, bi, s_v[w], s_i[w]);
+    if (bi == 0x7fffffff) bi = 0;  // every logit is -inf: first index (all-equal row => 0)
+    target_token[row] = bi;
+  }
+}
+
+constexpr int AC_THREADS = 128;
+
+// S9 + S10: one CTA per request.  Warp 0 decides the path; then every thread owns a column of
+// 16-byte chunks (layer, K|V, KV head, chunk) and moves it for path node t = 0,1,... in order:
+// sources are strictly increasing and src_t >= dst_t, so within a column every read of a slot
+// happens before the write that could overwrite it (R:C-6).
+__global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
+    const int32_t* __restrict__ sel_offsets, const int32_t* __restrict__ parent_local,
+    const uint8_t* __restrict__ sel_depth, const uint32_t* __restrict__ anc_mask,
+    const int32_t* __restrict__ draft_token, const int32_t* __restrict__ prev_token,
+    const int32_t* __restrict__ target_token, const int32_t* __restrict__ page_table,
+    const int32_t* __restrict__ prefix_len, int max_pages, int Hkv, int num_pages, int num_layers,
+    __nv_bfloat16* __restrict__ k_pool, __nv_bfloat16* __restrict__ v_pool, int32_t* __restrict__ accept_len,
+    int32_t* __restrict__ last_node, int32_t* __restrict__ bonus_token, int32_t* __restrict__ new_len,
+    int32_t* __restrict__ accept_idx, int32_t* __restrict__ slot_src, int32_t* __restrict__ slot_dst) {
+  __shared__ int s_L;
+  __shared__ int s_src[ECHO_MAX_ACCEPT], s_dst[ECHO_MAX_ACCEPT];
+  const int i = blockIdx.x;
+  const int b = sel_offsets[i], Ki = min(sel_offsets[i + 1] - b, ECHO_MAX_CAND);
+  const int P = prefix_len[i];
+  const int32_t* pt = page_table + (size_t)i * max_pages;
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x;
+    const int prev = prev_token[i];
+    // match[l]: draft token equals the target's greedy token after the parent (roots: prev_token)
+    uint32_t match[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int l = w * 32 + lane;
+      bool mt = false;
+      if (l < Ki) {
+        const int pl = parent_local[b + l];
+        mt = draft_token[b + l] == (pl < 0 ? prev : target_token[b + pl]);
+      }
+      match[w] = __ballot_sync(0xffffffffu, mt);
+    }
+    // acc[l] <=> every ancestor-or-self matches; best = max depth, then lowest l (R:C-4)
+    int best_key = -1;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int l = w * 32 + lane;
+      if (l < Ki) {
+        const uint4 m = reinterpret_cast<const uint4*>(anc_mask)[b + l];
+        const bool acc = !((m.x & ~match[0]) | (m.y & ~match[1]) | (m.z & ~match[2]) | (m.w & ~match[3]));
+        if (acc) best_key = max(best_key, ((int)sel_depth[b + l] << 8) | (ECHO_MAX_CAND - 1 - l));
+      }
+    }
+#pragma unroll
+    for (int ofs = 16; ofs; ofs >>= 1) best_key = max(best_key, __shfl_xor_sync(0xffffffffu, best_key, ofs));
+    int L = 0;
+    if (best_key >= 0) {
+      const int best = ECHO_MAX_CAND - 1 - (best_key & 0xff);
+      const uint4 m = reinterpret_cast<const uint4*>(anc_mask)[b + best];
+      const uint32_t mw[4] = {m.x, m.y, m.z, m.w};
+      L = min(__popc(m.x) + __popc(m.y) + __popc(m.z) + __popc(m.w), ECHO_MAX_ACCEPT);
+      // lane t finds the t-th set bit (path order = ascending local index, R:P-1)
+      int a = -1;
+      if (lane < L) {
+        int need = lane;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+          const int c = __popc(mw[w]);
+          if (a < 0) {
+            if (need < c) a = w * 32 + __fns(mw[w], 0, need + 1);
+            else need -= c;
+          }
+        }
+      }
+      if (lane < ECHO_MAX_ACCEPT) {
+        int src = -1, dst = -1, idx = -1;
+        if (lane < L) {
+          const int sp = P + a, dp = P + lane;
+          src = pt[sp / PAGE] * PAGE + sp % PAGE;
+          dst = pt[dp / PAGE] * PAGE + dp % PAGE;
+          idx = b + a;
+        }
+        accept_idx[i * ECHO_MAX_ACCEPT + lane] = idx;
+        slot_src[i * ECHO_MAX_ACCEPT + lane] = src;
+        slot_dst[i * ECHO_MAX_ACCEPT + lane] = dst;
+        s_src[lane] = src;
+        s_dst[lane] = dst;
+      }
+      if (lane == 0) { last_node[i] = b + best; bonus_token[i] = target_token[b + best]; }
+    } else {
+      accept_idx[i * ECHO_MAX_ACCEPT + lane] = -1;
+      slot_src[i * ECHO_MAX_ACCEPT + lane] = -1;
+      slot_dst[i * ECHO_MAX_ACCEPT + lane] = -1;
+      if (lane == 0) { last_node[i] = -1; bonus_token[i] = -1; }
+    }
+    if (lane == 0) { accept_len[i] = L; new_len[i] = P + L; s_L = L; }
+  }
+  __syncthreads();
+  const int L = s_L;
+  if (L == 0 || k_pool == nullptr) return;
+  // columns: (layer, kv in {K,V}, head, 16-byte chunk of the 256-byte row)
+  const int n_cols = num_layers * 2 * Hkv * (D * 2 / 16);
+  for (int col = threadIdx.x; col < n_cols; col += AC_THREADS) {
+    const int chunk = col % 16;
+    const int head = (col / 16) % Hkv;
+    const int kvsel = (col / (16 * Hkv)) % 2;
+    const int layer = col / (32 * Hkv);
+    __nv_bfloat16* pool = kvsel ? v_pool : k_pool;
+    uint4* base = reinterpret_cast<uint4*>(pool + (size_t)layer * num_pages * Hkv * PAGE * D);
+    for (int t = 0; t < L; ++t) {
+      const int s = s_src[t], d = s_dst[t];
+      if (s == d) continue;
+      const size_t so = (((size_t)(s / PAGE) * Hkv + head) * PAGE + (s % PAGE)) * (D * 2 / 16) + chunk;
+      const size_t dofs = (((size_t)(d / PAGE) * Hkv + head) * PAGE + (d % PAGE)) * (D * 2 / 16) + chunk;
+      base[dofs] = base[so];
+    }
+  }
+}
+
+}  // namespace
+
+int launch_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t R, EchoPagedKV* kv,
+                  EchoAccept* out, cudaStream_t st) {
+  const int32_t* tt = res->target_token;
+  if (res->target_logits) {
+    int32_t* tout = out->target_token_out ? out->target_token_out : reinterpret_cast<int32_t*>(ctx->workspace);
+    if (!out->target_token_out && (size_t)sel->capacity * sizeof(int32_t) > ctx->workspace_bytes)
+      return ECHO_ERR_WORKSPACE;
+    if (sel->capacity > 0)
+      k_argmax_bf16<<<sel->capacity, AM_THREADS, 0, st>>>(
+          sel->n_selected, reinterpret_cast<const __nv_bfloat16*>(res->target_logits), res->ld, res->vocab, tout);
+    tt = tout;
+  }
+  if (R > 0) {
+    const bool have_pools = kv->k_pool && kv->v_pool;  // NULL pools: slot maps only, no copy
+    k_accept_compact<<<R, AC_THREADS, 0, st>>>(
+        sel->sel_offsets, sel->parent_local, sel->sel_depth, sel->anc_mask, res->draft_token, res->prev_token, tt,
+        kv->page_table, kv->prefix_len, kv->max_pages_per_req, kv->num_kv_heads, kv->num_pages, kv->num_layers,
+        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->k_pool) : nullptr,
+        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->v_pool) : nullptr, out->accept_len, out->last_node,
+        out->bonus_token, out->new_len, out->accept_idx, out->slot_src, out->slot_dst);
+  }
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}

@@ -1,0 +1,163 @@
+// C-ABI entry points of libecho.so (include/echo.h): argument validation and launch only.
+#include "common.cuh"
+
+#include <new>
+
+static bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
+extern "C" {
+
+const char* echo_strerror(int code) {
+  switch (code) {
+    case ECHO_OK: return "ok";
+    case ECHO_ERR_INVALID_ARG: return "invalid argument";
+    case ECHO_ERR_UNSUPPORTED: return "unsupported shape";
+    case ECHO_ERR_WORKSPACE: return "workspace too small";
+    case ECHO_ERR_ARCH: return "device is not sm_100 (B200)";
+    case ECHO_ERR_CUDA: return "CUDA error (see echo_last_error)";
+    default: return "unknown error";
+  }
+}
+
+size_t echo_workspace_bytes(int32_t R, int32_t N, int32_t capacity, int32_t Hq) {
+  if (R < 0 || N < 0 || capacity < 0 || Hq < 0) return 0;
+  size_t keys = align_up((size_t)N * sizeof(uint64_t), 256);
+  size_t parts = align_up((size_t)16 * capacity * Hq * (128 + 2) * sizeof(float), 256);
+  size_t toks = align_up((size_t)capacity * sizeof(int32_t), 256);
+  size_t plan = align_up(((size_t)R * 64 + 1024) * sizeof(int32_t) * 8, 256);
+  size_t m = keys > parts ? keys : parts;
+  if (toks > m) m = toks;
+  return m + plan + 4096;
+}
+
+int echo_create(EchoCtx** out, int device, size_t workspace_bytes) {
+  if (!out) return ECHO_ERR_INVALID_ARG;
+  *out = nullptr;
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || device < 0 || device >= n) return ECHO_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return ECHO_ERR_CUDA;
+  if (prop.major != 10 || prop.minor != 0) return ECHO_ERR_ARCH;
+  EchoCtx* c = new (std::nothrow) EchoCtx();
+  if (!c) return ECHO_ERR_CUDA;
+  memset(c, 0, sizeof(*c));
+  c->device = device;
+  c->num_sms = prop.multiProcessorCount;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaSetDevice(device);
+  c->workspace_bytes = align_up(workspace_bytes ? workspace_bytes : 256, 256);
+  cudaError_t e = cudaMalloc(&c->workspace, c->workspace_bytes);
+  if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&c->dev_status), 256);
+  if (e == cudaSuccess) e = cudaMemset(c->dev_status, 0, 256);
+  cudaSetDevice(prev);
+  if (e != cudaSuccess) {
+    if (c->workspace) cudaFree(c->workspace);
+    delete c;
+    return ECHO_ERR_CUDA;
+  }
+  *out = c;
+  return ECHO_OK;
+}
+
+int echo_destroy(EchoCtx* ctx) {
+  if (!ctx) return ECHO_ERR_INVALID_ARG;
+  cudaFree(ctx->workspace);
+  cudaFree(ctx->dev_status);
+  delete ctx;
+  return ECHO_OK;
+}
+
+const char* echo_last_error(EchoCtx* ctx) { return ctx ? ctx->last_error : "null context"; }
+
+int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream) {
+  if (!ctx || !flags) return ECHO_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  ECHO_CUDA_TRY(ctx, cudaMemcpyAsync(flags, ctx->dev_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  ECHO_CUDA_TRY(ctx, cudaMemsetAsync(ctx->dev_status, 0, sizeof(uint32_t), st));
+  ECHO_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+  return ECHO_OK;
+}
+
+int echo_set_option(EchoCtx* ctx, int key, int64_t value) {
+  if (!ctx) return ECHO_ERR_INVALID_ARG;
+  switch (key) {
+    case ECHO_OPT_FORCE_SPLITS:
+      if (value < 0 || value > 16) return ECHO_ERR_INVALID_ARG;
+      ctx->opt_force_splits = value;
+      return ECHO_OK;
+    case ECHO_OPT_ATTN_PATH:
+      if (value < 0 || value > 2) return ECHO_ERR_INVALID_ARG;
+      ctx->opt_attn_path = value;
+      return ECHO_OK;
+    case ECHO_OPT_NUM_CTAS:
+      if (value < 0 || value > 4096) return ECHO_ERR_INVALID_ARG;
+      ctx->opt_num_ctas = value;
+      return ECHO_OK;
+    default: return ECHO_ERR_INVALID_ARG;
+  }
+}
+
+int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, echo_stream_t stream) {
+  if (!ctx || !t || !g || !o) return ECHO_ERR_INVALID_ARG;
+  if (t->num_requests < 0 || t->total_cand < 0 || t->max_cand_per_req < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->budget < 0 || g->w_max < 0 || g->static_k < 0 || o->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if (t->max_cand_per_req > ECHO_MAX_CAND) return ECHO_ERR_UNSUPPORTED;
+  if (!t->cand_offsets || !o->n_selected || !o->sel_offsets || !o->cut_depth) return ECHO_ERR_INVALID_ARG;
+  if (t->total_cand > 0 && (!t->parent || !t->logq || !o->path_score || !o->cand_depth)) return ECHO_ERR_INVALID_ARG;
+  long need = g->static_k > 0 ? (long)t->num_requests * g->static_k : (long)g->budget;
+  if (need > t->total_cand) need = t->total_cand;
+  if (o->capacity < need) return ECHO_ERR_INVALID_ARG;
+  if (o->capacity > 0 && (!o->sel_node || !o->sel_req || !o->parent_local || !o->sel_depth || !o->anc_mask))
+    return ECHO_ERR_INVALID_ARG;
+  if (misaligned(o->anc_mask, 16)) return ECHO_ERR_INVALID_ARG;
+  return launch_gate_select(ctx, t, g, o, reinterpret_cast<cudaStream_t>(stream));
+}
+
+static int check_kv(const EchoPagedKV* kv, bool need_pools) {
+  if (!kv) return ECHO_ERR_INVALID_ARG;
+  if (kv->head_dim != 128 || kv->page_size != 16) return ECHO_ERR_UNSUPPORTED;
+  if (kv->num_kv_heads <= 0 || kv->num_pages < 0 || kv->max_pages_per_req < 0 || kv->num_layers <= 0)
+    return ECHO_ERR_INVALID_ARG;
+  if (!kv->page_table || !kv->prefix_len) return ECHO_ERR_INVALID_ARG;
+  if (need_pools && (!kv->k_pool || !kv->v_pool)) return ECHO_ERR_INVALID_ARG;
+  if (misaligned(kv->k_pool, 16) || misaligned(kv->v_pool, 16)) return ECHO_ERR_INVALID_ARG;
+  return ECHO_OK;
+}
+
+int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer, int32_t Hq,
+                     int32_t R, const void* q, void* out, float* lse, float sm_scale, echo_stream_t stream) {
+  if (!ctx || !sel) return ECHO_ERR_INVALID_ARG;
+  int rc = check_kv(kv, true);
+  if (rc != ECHO_OK) return rc;
+  if (R < 0 || Hq <= 0 || sel->capacity < 0 || layer < 0 || layer >= kv->num_layers) return ECHO_ERR_INVALID_ARG;
+  if (Hq % kv->num_kv_heads != 0) return ECHO_ERR_UNSUPPORTED;
+  if (!sel->n_selected || !sel->sel_offsets) return ECHO_ERR_INVALID_ARG;
+  if (sel->capacity > 0 && (!q || !out || !lse || !sel->sel_req || !sel->anc_mask)) return ECHO_ERR_INVALID_ARG;
+  if (misaligned(q, 16) || misaligned(out, 16) || misaligned(sel->anc_mask, 16)) return ECHO_ERR_INVALID_ARG;
+  return launch_verify_attn(ctx, sel, kv, layer, Hq, R, q, out, lse, sm_scale, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t R, EchoPagedKV* kv,
+                EchoAccept* out, echo_stream_t stream) {
+  if (!ctx || !sel || !res || !out) return ECHO_ERR_INVALID_ARG;
+  int rc = check_kv(kv, false);
+  if (rc != ECHO_OK) return rc;
+  if (R < 0 || sel->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if ((res->target_token != nullptr) == (res->target_logits != nullptr)) return ECHO_ERR_INVALID_ARG;
+  if (res->target_logits) {
+    if (res->vocab <= 0 || res->ld < res->vocab) return ECHO_ERR_INVALID_ARG;
+    if (res->ld % 8 != 0) return ECHO_ERR_UNSUPPORTED;
+    if (misaligned(res->target_logits, 16)) return ECHO_ERR_INVALID_ARG;
+  }
+  if (!sel->sel_offsets || !sel->n_selected) return ECHO_ERR_INVALID_ARG;
+  if (R > 0 && (!res->prev_token || !out->accept_len || !out->last_node || !out->bonus_token || !out->new_len ||
+                !out->accept_idx || !out->slot_src || !out->slot_dst))
+    return ECHO_ERR_INVALID_ARG;
+  if (sel->capacity > 0 && (!res->draft_token || !sel->parent_local || !sel->sel_depth || !sel->anc_mask))
+    return ECHO_ERR_INVALID_ARG;
+  if (misaligned(sel->anc_mask, 16)) return ECHO_ERR_INVALID_ARG;
+  return launch_accept(ctx, sel, res, R, kv, out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

@@ -1,0 +1,55 @@
+// Shared internals of libecho.so (CUDA path only; the CPU oracle shares nothing with this).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/echo.h"
+
+struct EchoCtx {
+  int device;
+  int num_sms;
+  void* workspace;
+  size_t workspace_bytes;
+  uint32_t* dev_status;  // device status word (inside its own allocation)
+  int64_t opt_force_splits;
+  int64_t opt_attn_path;
+  int64_t opt_num_ctas;
+  char last_error[256];
+};
+
+#define ECHO_CUDA_TRY(ctx, expr)                                                              \
+  do {                                                                                        \
+    cudaError_t _e = (expr);                                                                  \
+    if (_e != cudaSuccess) {                                                                  \
+      snprintf((ctx)->last_error, sizeof((ctx)->last_error), "%s:%d %s: %s", __FILE__, __LINE__, \
+               #expr, cudaGetErrorString(_e));                                                \
+      return ECHO_ERR_CUDA;                                                                   \
+    }                                                                                         \
+  } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// launchers implemented by the .cu files
+int launch_gate_select(EchoCtx*, const EchoTrees*, const EchoGate*, EchoSelection*, cudaStream_t);
+int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
+                       const void* q, void* out, float* lse, float sm_scale, cudaStream_t);
+int launch_accept(EchoCtx*, const EchoSelection*, const EchoVerifyResult*, int32_t R, EchoPagedKV*, EchoAccept*,
+                  cudaStream_t);
+// tcgen05 path (verify_attn_tc.cu); returns ECHO_ERR_UNSUPPORTED when the shape cannot use it
+int launch_verify_attn_tc(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
+                          const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,
+                          float* part_ml, cudaStream_t);
+
+// order-preserving map fp32 -> u32 (ascending float <=> ascending unsigned)
+__host__ __device__ static inline uint32_t f32_ordered(float f) {
+#ifdef __CUDA_ARCH__
+  uint32_t u = __float_as_uint(f);
+#else
+  uint32_t u;
+  memcpy(&u, &f, 4);
+#endif
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}

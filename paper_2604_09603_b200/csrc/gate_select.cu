@@ -1,0 +1,283 @@
+// echo_gate_select: S1-S5 of the super-tree verify step (include/echo.h).
+//   k_score_gate  : one CTA per request -- path scores (Eq. 5), level maxima and the
+//                   sparse gate (Eq. 6-7), tier assignment (Alg. 1) and a
+//                   unique 64-bit selection key per candidate.
+//   k_select_pack : one CTA -- radix select of the budget-th smallest key (Eq. 4), then
+//                   Flatten & Pack (Fig. 3(3)) with local parents and 128-bit ancestor masks.
+// These steps move < 1 MB and are latency-bound: two launches, no host sync.
+#include "common.cuh"
+
+namespace {
+
+struct GateParams {
+  uint32_t depth_mask;
+  float log_tau[32];
+  int32_t w_max;
+  int32_t static_k;
+};
+
+__device__ __forceinline__ float f32_unordered(uint32_t o) {
+  uint32_t u = (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o;
+  return __uint_as_float(u);
+}
+
+constexpr uint64_t KEY_INELIGIBLE = ~0ull;
+
+// key order == (tier asc, S desc, request asc, node asc): tier in bit 63, inverted ordered score in
+// bits 31..62, global candidate index (monotone in (request, node)) in bits 0..30.
+__device__ __forceinline__ uint64_t make_key(int tier, float S, int g) {
+  return ((uint64_t)tier << 63) | ((uint64_t)(~f32_ordered(S)) << 31) | (uint64_t)(uint32_t)g;
+}
+
+__global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent, const float* __restrict__ logq,
+    const __grid_constant__ GateParams gp, float* __restrict__ path_score, uint8_t* __restrict__ cand_depth,
+    int32_t* __restrict__ cut_depth, uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
+  __shared__ int s_par[ECHO_MAX_CAND];
+  __shared__ float s_lq[ECHO_MAX_CAND];
+  __shared__ float s_S[ECHO_MAX_CAND];
+  __shared__ int s_d[ECHO_MAX_CAND];
+  __shared__ uint32_t s_lvlmax[ECHO_MAX_DEPTH];
+  __shared__ int s_cut;
+
+  const int i = blockIdx.x;
+  const int b = cand_offsets[i];
+  const int C = min(cand_offsets[i + 1] - b, ECHO_MAX_CAND);
+  const int j = threadIdx.x;
+  uint32_t bad = 0;
+  if (j < ECHO_MAX_DEPTH) s_lvlmax[j] = 0u;
+  if (j < C) {
+    int p = parent[b + j];
+    float lq = logq[b + j];
+    if (p >= j || p < -1) { bad |= ECHO_DEV_BAD_PARENT; p = -1; }
+    if (!(lq <= 0.0f)) bad |= ECHO_DEV_BAD_LOGQ;
+    s_par[j] = p;
+    s_lq[j] = lq;
+  }
+  __syncthreads();
+
+  float S = 0.0f;
+  int d = 0;
+  if (j < C) {
+    // S1: every node replays the root->leaf chain of fp32 adds in order, so the value is
+    // bit-identical to the sequential recurrence (R:G-3); __fadd_rn forbids contraction.
+    int chain[ECHO_MAX_DEPTH];
+    int n = 0, c = j;
+    while (c >= 0 && n < ECHO_MAX_DEPTH) { chain[n++] = c; c = s_par[c]; }
+    if (c >= 0) bad |= ECHO_DEV_DEPTH_OVERFLOW;
+    for (int k = n - 1; k >= 0; --k) S = __fadd_rn(S, s_lq[chain[k]]);
+    d = n - 1;
+    s_S[j] = S;
+    s_d[j] = d;
+    path_score[b + j] = S;
+    cand_depth[b + j] = (uint8_t)d;
+    atomicMax(&s_lvlmax[d], f32_ordered(S));  // S2: m[i][d] (Eq. 6 in the log domain)
+  }
+  if (bad) atomicOr(status, bad);
+  __syncthreads();
+
+  if (j == 0) {
+    int cut = ECHO_CUT_NEVER;
+    if (gp.static_k <= 0) {
+      for (int dd = 0; dd < ECHO_MAX_DEPTH; ++dd) {
+        if (!((gp.depth_mask >> dd) & 1u) || s_lvlmax[dd] == 0u) continue;  // ungated or absent level (R:G-5)
+        if (!(f32_unordered(s_lvlmax[dd]) > gp.log_tau[dd])) { cut = dd; break; }  // Eq. 7, strict (R:G-4)
+      }
+    }
+    s_cut = cut;
+    cut_depth[i] = cut;
+  }
+  __syncthreads();
+
+  if (j < C) {
+    const int cut = s_cut;
+    uint64_t key = KEY_INELIGIBLE;
+    if (gp.static_k > 0) {
+      int rank = 0;  // per-request top-static_k by (S desc, node asc) (R:G-15)
+      for (int t = 0; t < C; ++t) rank += (s_S[t] > S) || (s_S[t] == S && t < j);
+      if (rank < gp.static_k) key = make_key(0, 0.0f, b + j);
+    } else if (d < cut) {
+      key = make_key(0, S, b + j);  // tier 0: depth extension
+    } else if (d == cut) {
+      int rank = 0;  // tier 1: the w_max best nodes of the truncation level (R:G-7, G-8)
+      for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
+      if (rank < gp.w_max) key = make_key(1, S, b + j);
+    }
+    keys[b + j] = key;
+  }
+}
+
+constexpr int SEL_THREADS = 1024;
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += t;
+  }
+  return v;
+}
+
+__global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent,
+    const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys, int R, int N, int budget,
+    int capacity, int32_t* __restrict__ n_selected, int32_t* __restrict__ sel_offsets,
+    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
+    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
+  __shared__ int s_hist[256];
+  __shared__ int s_warp[32];
+  __shared__ uint64_t s_prefix;
+  __shared__ int s_k;
+  __shared__ int s_eligible;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+  // ---- S3: threshold T = budget-th smallest key (keys are unique => no ties to break) ----
+  if (tid == 0) s_eligible = 0;
+  __syncthreads();
+  {
+    int e = 0;
+    for (int g = tid; g < N; g += SEL_THREADS) e += keys[g] != KEY_INELIGIBLE;
+    e = warp_incl_scan(e, lane);
+    if (lane == 31 && e) atomicAdd(&s_eligible, e);
+  }
+  __syncthreads();
+  uint64_t T;
+  if (budget <= 0) {
+    T = 0;  // nothing selected (keys are > 0 unless tier 0, score +inf, g 0: excluded below by budget check)
+  } else if (s_eligible <= budget) {
+    T = KEY_INELIGIBLE - 1;  // everything eligible (R:G-12)
+  } else {
+    if (tid == 0) { s_prefix = 0; s_k = budget; }
+    for (int pass = 0; pass < 8; ++pass) {
+      const int shift = 56 - 8 * pass;
+      if (tid < 256) s_hist[tid] = 0;
+      __syncthreads();
+      const uint64_t prefix = s_prefix;
+      for (int g = tid; g < N; g += SEL_THREADS) {
+        uint64_t key = keys[g];
+        if (pass == 0 || (key >> (shift + 8)) == prefix) atomicAdd(&s_hist[(int)((key >> shift) & 0xff)], 1);
+      }
+      __syncthreads();
+      if (warp == 0) {  // find the digit that holds the k-th key
+        int c[8], sum = 0;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) { c[t] = s_hist[lane * 8 + t]; sum += c[t]; }
+        int incl = warp_incl_scan(sum, lane);
+        int excl = incl - sum;
+        const int k = s_k;
+        if (excl < k && k <= incl) {
+          int run = excl;
+#pragma unroll
+          for (int t = 0; t < 8; ++t) {
+            if (run < k && k <= run + c[t]) { s_prefix = (prefix << 8) | (uint64_t)(lane * 8 + t); s_k = k - run; }
+            run += c[t];
+          }
+        }
+      }
+      __syncthreads();
+    }
+    T = s_prefix;
+  }
+  const bool none = budget <= 0;
+
+  // ---- S4: per-request counts, CSR offsets ----
+  for (int r = warp; r < R; r += SEL_THREADS / 32) {
+    const int b = cand_offsets[r], C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
+    int cnt = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      int j = w * 32 + lane;
+      bool s = !none && j < C && keys[b + j] <= T;
+      cnt += __popc(__ballot_sync(0xffffffffu, s));
+    }
+    if (lane == 0) sel_offsets[r + 1] = cnt;
+  }
+  if (tid == 0) sel_offsets[0] = 0;
+  __syncthreads();
+  {  // in-place inclusive scan of sel_offsets[1..R]
+    const int per = (R + SEL_THREADS - 1) / SEL_THREADS;
+    const int lo = tid * per, hi = min(R, lo + per);
+    int sum = 0;
+    for (int r = lo; r < hi; ++r) sum += sel_offsets[r + 1];
+    int incl = warp_incl_scan(sum, lane);
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) s_warp[lane] = warp_incl_scan(s_warp[lane], lane);
+    __syncthreads();
+    int run = incl - sum + (warp ? s_warp[warp - 1] : 0);
+    for (int r = lo; r < hi; ++r) { run += sel_offsets[r + 1]; sel_offsets[r + 1] = run; }
+    if (tid == SEL_THREADS - 1) *n_selected = s_warp[31];
+  }
+  __syncthreads();
+
+  // ---- S4/S5: packed arrays, local parents, ancestor-or-self masks ----
+  for (int r = warp; r < R; r += SEL_THREADS / 32) {
+    const int b = cand_offsets[r], C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
+    const int base = sel_offsets[r];
+    uint32_t bal[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      int j = w * 32 + lane;
+      bal[w] = __ballot_sync(0xffffffffu, !none && j < C && keys[b + j] <= T);
+    }
+    auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
+      int l = 0;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        if (w < (c >> 5)) l += __popc(bal[w]);
+        else if (w == (c >> 5)) l += __popc(bal[w] & ((1u << (c & 31)) - 1u));
+      }
+      return l;
+    };
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      int j = w * 32 + lane;
+      if (!((bal[w] >> lane) & 1u)) continue;
+      const int l = local_of(j);
+      const int k = base + l;
+      if (k >= capacity) continue;
+      int p = parent[b + j];
+      if (p >= j) p = -1;
+      uint32_t m[4] = {0u, 0u, 0u, 0u};
+      m[l >> 5] |= 1u << (l & 31);
+      int pl = -1;
+      int c = p;
+      for (int step = 0; c >= 0 && step < ECHO_MAX_DEPTH; ++step) {
+        // ancestor closure (DESIGN.md invariant I2) guarantees every ancestor is selected
+        int la = local_of(c);
+        if (step == 0) pl = la;
+        m[la >> 5] |= 1u << (la & 31);
+        int pc = parent[b + c];
+        c = (pc >= c) ? -1 : pc;
+      }
+      sel_node[k] = j;
+      sel_req[k] = r;
+      sel_depth[k] = cand_depth[b + j];
+      parent_local[k] = pl;
+      reinterpret_cast<uint4*>(anc_mask)[k] = make_uint4(m[0], m[1], m[2], m[3]);
+    }
+  }
+}
+
+}  // namespace
+
+int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, cudaStream_t st) {
+  const int R = t->num_requests, N = t->total_cand;
+  uint64_t* keys = reinterpret_cast<uint64_t*>(ctx->workspace);
+  if ((size_t)N * sizeof(uint64_t) > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  GateParams gp;
+  gp.depth_mask = g->depth_mask;
+  for (int d = 0; d < 32; ++d) gp.log_tau[d] = g->log_tau[d] + 0.0f;  // canonicalise -0 (R:G-13)
+  gp.w_max = g->w_max;
+  gp.static_k = g->static_k;
+  if (R > 0) {
+    k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gp, o->path_score,
+                                               o->cand_depth, o->cut_depth, keys, ctx->dev_status);
+  }
+  const int budget = g->static_k > 0 ? N : g->budget;
+  k_select_pack<<<1, SEL_THREADS, 0, st>>>(t->cand_offsets, t->parent, o->cand_depth, keys, R, N, budget,
+                                           o->capacity, o->n_selected, o->sel_offsets, o->sel_node, o->sel_req,
+                                           o->parent_local, o->sel_depth, o->anc_mask);
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}

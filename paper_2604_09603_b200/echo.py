@@ -1,0 +1,319 @@
+"""Thin ctypes binding of libecho.so (include/echo.h).  Argument marshalling only: every step of
+the hot path runs in the CUDA kernels of `csrc/`.  torch is used for device memory and streams.
+
+There is no CPU fallback: importing works anywhere (so the symbol/ABI tests run without a GPU),
+but `EchoContext()` raises unless the library loads and the device is a B200 (sm_100).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libecho.so")
+
+ECHO_OK = 0
+ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5
+OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS = 1, 2, 3
+ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
+MAX_ACCEPT = 32
+CUT_NEVER = 0x7FFFFFFF
+DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
+
+EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
+           "echo_device_status", "echo_set_option", "echo_gate_select", "echo_verify_attn", "echo_accept"]
+
+
+class EchoTrees(C.Structure):
+    _fields_ = [("num_requests", C.c_int32), ("total_cand", C.c_int32), ("max_cand_per_req", C.c_int32),
+                ("cand_offsets", C.c_void_p), ("parent", C.c_void_p), ("logq", C.c_void_p)]
+
+
+class EchoGate(C.Structure):
+    _fields_ = [("depth_mask", C.c_uint32), ("log_tau", C.c_float * 32), ("w_max", C.c_int32),
+                ("budget", C.c_int32), ("static_k", C.c_int32)]
+
+
+class EchoSelection(C.Structure):
+    _fields_ = [("capacity", C.c_int32), ("n_selected", C.c_void_p), ("sel_offsets", C.c_void_p),
+                ("sel_node", C.c_void_p), ("sel_req", C.c_void_p), ("parent_local", C.c_void_p),
+                ("sel_depth", C.c_void_p), ("anc_mask", C.c_void_p), ("path_score", C.c_void_p),
+                ("cand_depth", C.c_void_p), ("cut_depth", C.c_void_p)]
+
+
+class EchoPagedKV(C.Structure):
+    _fields_ = [("num_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("page_size", C.c_int32),
+                ("num_pages", C.c_int32), ("max_pages_per_req", C.c_int32), ("num_layers", C.c_int32),
+                ("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("page_table", C.c_void_p),
+                ("prefix_len", C.c_void_p)]
+
+
+class EchoVerifyResult(C.Structure):
+    _fields_ = [("draft_token", C.c_void_p), ("prev_token", C.c_void_p), ("target_token", C.c_void_p),
+                ("target_logits", C.c_void_p), ("vocab", C.c_int32), ("ld", C.c_int64)]
+
+
+class EchoAccept(C.Structure):
+    _fields_ = [("accept_len", C.c_void_p), ("last_node", C.c_void_p), ("bonus_token", C.c_void_p),
+                ("new_len", C.c_void_p), ("accept_idx", C.c_void_p), ("slot_src", C.c_void_p),
+                ("slot_dst", C.c_void_p), ("target_token_out", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libecho.so and declare the prototypes.  Raises if the library was not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2604_09603_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    P = C.POINTER
+    lib.echo_create.argtypes = [P(C.c_void_p), C.c_int, C.c_size_t]
+    lib.echo_create.restype = C.c_int
+    lib.echo_destroy.argtypes = [C.c_void_p]
+    lib.echo_destroy.restype = C.c_int
+    lib.echo_workspace_bytes.argtypes = [C.c_int32] * 4
+    lib.echo_workspace_bytes.restype = C.c_size_t
+    lib.echo_strerror.argtypes = [C.c_int]
+    lib.echo_strerror.restype = C.c_char_p
+    lib.echo_last_error.argtypes = [C.c_void_p]
+    lib.echo_last_error.restype = C.c_char_p
+    lib.echo_device_status.argtypes = [C.c_void_p, P(C.c_uint32), C.c_void_p]
+    lib.echo_device_status.restype = C.c_int
+    lib.echo_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
+    lib.echo_set_option.restype = C.c_int
+    lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
+    lib.echo_gate_select.restype = C.c_int
+    lib.echo_verify_attn.argtypes = [C.c_void_p, P(EchoSelection), P(EchoPagedKV), C.c_int32, C.c_int32,
+                                     C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
+    lib.echo_verify_attn.restype = C.c_int
+    lib.echo_accept.argtypes = [C.c_void_p, P(EchoSelection), P(EchoVerifyResult), C.c_int32, P(EchoPagedKV),
+                                P(EchoAccept), C.c_void_p]
+    lib.echo_accept.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+class EchoError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"echo error {code}: {msg}")
+        self.code = code
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+@dataclass
+class Selection:
+    """Device-side output of echo_gate_select (torch tensors on the context's device)."""
+    capacity: int
+    R: int
+    n_selected: "torch.Tensor"
+    sel_offsets: "torch.Tensor"
+    sel_node: "torch.Tensor"
+    sel_req: "torch.Tensor"
+    parent_local: "torch.Tensor"
+    sel_depth: "torch.Tensor"
+    anc_mask: "torch.Tensor"
+    path_score: "torch.Tensor"
+    cand_depth: "torch.Tensor"
+    cut_depth: "torch.Tensor"
+
+    def c_struct(self) -> EchoSelection:
+        return EchoSelection(self.capacity, _ptr(self.n_selected), _ptr(self.sel_offsets), _ptr(self.sel_node),
+                             _ptr(self.sel_req), _ptr(self.parent_local), _ptr(self.sel_depth),
+                             _ptr(self.anc_mask), _ptr(self.path_score), _ptr(self.cand_depth),
+                             _ptr(self.cut_depth))
+
+    def to_host(self) -> dict:
+        """numpy copies trimmed to n_selected (synchronises)."""
+        n = int(self.n_selected.item())
+        return dict(n_selected=n, sel_offsets=self.sel_offsets.cpu().numpy(),
+                    sel_node=self.sel_node[:n].cpu().numpy(), sel_req=self.sel_req[:n].cpu().numpy(),
+                    parent_local=self.parent_local[:n].cpu().numpy(), sel_depth=self.sel_depth[:n].cpu().numpy(),
+                    anc_mask=self.anc_mask[:n].cpu().numpy().view(np.uint32),
+                    path_score=self.path_score.cpu().numpy(), cand_depth=self.cand_depth.cpu().numpy(),
+                    cut_depth=self.cut_depth.cpu().numpy())
+
+
+@dataclass
+class PagedKV:
+    k_pool: "torch.Tensor"      # bf16 [layers][pages][Hkv][16][128]
+    v_pool: "torch.Tensor"
+    page_table: "torch.Tensor"  # int32 [R][max_pages]
+    prefix_len: "torch.Tensor"  # int32 [R]
+
+    def c_struct(self) -> EchoPagedKV:
+        L, NP, Hkv, PS, Dh = self.k_pool.shape
+        return EchoPagedKV(Hkv, Dh, PS, NP, self.page_table.shape[1], L, _ptr(self.k_pool), _ptr(self.v_pool),
+                           _ptr(self.page_table), _ptr(self.prefix_len))
+
+
+@dataclass
+class Acceptance:
+    accept_len: "torch.Tensor"
+    last_node: "torch.Tensor"
+    bonus_token: "torch.Tensor"
+    new_len: "torch.Tensor"
+    accept_idx: "torch.Tensor"
+    slot_src: "torch.Tensor"
+    slot_dst: "torch.Tensor"
+    target_token: Optional["torch.Tensor"]
+
+    def to_host(self) -> dict:
+        return {k: getattr(self, k).cpu().numpy() for k in
+                ("accept_len", "last_node", "bonus_token", "new_len", "accept_idx", "slot_src", "slot_dst")}
+
+
+class EchoContext:
+    """Owns an EchoCtx (workspace) on one CUDA device."""
+
+    def __init__(self, device: int = 0, workspace_bytes: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("echo: no CUDA device (the hot path has no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        torch.cuda.init()
+        with torch.cuda.device(self.device):
+            torch.cuda.current_stream()  # make sure the primary context exists
+        self._h = C.c_void_p()
+        self.workspace_bytes = int(workspace_bytes)
+        rc = self.lib.echo_create(C.byref(self._h), device, self.workspace_bytes)
+        if rc != ECHO_OK:
+            raise EchoError(rc, self.lib.echo_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.lib.echo_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers -----------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != ECHO_OK:
+            msg = self.lib.echo_strerror(rc).decode()
+            if rc == ERR_CUDA:
+                msg += ": " + self.lib.echo_last_error(self._h).decode()
+            raise EchoError(rc, msg)
+
+    def _stream(self):
+        import torch
+        return C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
+
+    def ensure_workspace(self, R: int, N: int, capacity: int, Hq: int):
+        need = int(self.lib.echo_workspace_bytes(R, N, capacity, Hq))
+        if need > self.workspace_bytes:
+            import torch
+            torch.cuda.synchronize(self.device)
+            opts = (self.get_options() if hasattr(self, "_opts") else {})
+            self.lib.echo_destroy(self._h)
+            self._h = C.c_void_p()
+            self._check(self.lib.echo_create(C.byref(self._h), self.device.index, need))
+            self.workspace_bytes = need
+            for k, v in opts.items():
+                self.set_option(k, v)
+
+    def get_options(self) -> dict:
+        return dict(getattr(self, "_opts", {}))
+
+    def set_option(self, key: int, value: int):
+        self._check(self.lib.echo_set_option(self._h, key, int(value)))
+        if not hasattr(self, "_opts"):
+            self._opts = {}
+        self._opts[key] = int(value)
+
+    def device_status(self) -> int:
+        f = C.c_uint32(0)
+        self._check(self.lib.echo_device_status(self._h, C.byref(f), self._stream()))
+        return int(f.value)
+
+    # -- the three calls ----------------------------------------------------------------------
+    def alloc_selection(self, R: int, N: int, capacity: int) -> Selection:
+        import torch
+        d = self.device
+        i32 = dict(dtype=torch.int32, device=d)
+        cap = max(1, capacity)
+        return Selection(capacity, R, torch.zeros(1, **i32), torch.zeros(R + 1, **i32), torch.zeros(cap, **i32),
+                         torch.zeros(cap, **i32), torch.zeros(cap, **i32),
+                         torch.zeros(cap, dtype=torch.uint8, device=d), torch.zeros(cap, 4, **i32),
+                         torch.zeros(max(1, N), dtype=torch.float32, device=d),
+                         torch.zeros(max(1, N), dtype=torch.uint8, device=d), torch.zeros(max(1, R), **i32))
+
+    def gate_select(self, cand_offsets, parent, logq, depth_mask: int, log_tau, w_max: int, budget: int,
+                    static_k: int = 0, capacity: Optional[int] = None, max_cand: int = 128,
+                    out: Optional[Selection] = None) -> Selection:
+        """echo_gate_select.  cand_offsets/parent int32 and logq float32 device tensors."""
+        R = cand_offsets.numel() - 1
+        N = parent.numel()
+        if capacity is None:
+            capacity = min(N, R * static_k) if static_k > 0 else budget
+        self.ensure_workspace(R, N, capacity, 0)
+        sel = out if out is not None else self.alloc_selection(R, N, capacity)
+        trees = EchoTrees(R, N, max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
+        g = EchoGate()
+        g.depth_mask = int(depth_mask) & 0xFFFFFFFF
+        lt = np.asarray(log_tau, np.float32)
+        for d in range(32):
+            g.log_tau[d] = float(lt[d])
+        g.w_max, g.budget, g.static_k = int(w_max), int(budget), int(static_k)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_gate_select(self._h, C.byref(trees), C.byref(g), C.byref(cs), self._stream()))
+        return sel
+
+    def verify_attn(self, sel: Selection, kv: PagedKV, q, sm_scale: float, layer: int = 0, out=None, lse=None):
+        """echo_verify_attn.  q bf16 [capacity][Hq][128] -> (out bf16 same shape, lse f32 [capacity][Hq])."""
+        import torch
+        Hq = q.shape[1]
+        self.ensure_workspace(sel.R, 0, sel.capacity, Hq)
+        if out is None:
+            out = torch.zeros_like(q)
+        if lse is None:
+            lse = torch.zeros(q.shape[0], Hq, dtype=torch.float32, device=q.device)
+        cs, ck = sel.c_struct(), kv.c_struct()
+        self._check(self.lib.echo_verify_attn(self._h, C.byref(cs), C.byref(ck), layer, Hq, sel.R, _ptr(q),
+                                              _ptr(out), _ptr(lse), C.c_float(sm_scale), self._stream()))
+        return out, lse
+
+    def alloc_accept(self, R: int, capacity: int) -> Acceptance:
+        import torch
+        i32 = dict(dtype=torch.int32, device=self.device)
+        r = max(1, R)
+        return Acceptance(torch.zeros(r, **i32), torch.zeros(r, **i32), torch.zeros(r, **i32),
+                          torch.zeros(r, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
+                          torch.zeros(r, MAX_ACCEPT, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
+                          torch.zeros(max(1, capacity), **i32))
+
+    def accept(self, sel: Selection, kv: PagedKV, draft_token, prev_token, target_token=None,
+               target_logits=None, vocab: int = 0, out: Optional[Acceptance] = None,
+               compact: bool = True) -> Acceptance:
+        """echo_accept.  Exactly one of target_token (int32 [capacity]) / target_logits (bf16 [capacity][ld])."""
+        acc = out if out is not None else self.alloc_accept(sel.R, sel.capacity)
+        self.ensure_workspace(sel.R, 0, sel.capacity, 0)
+        res = EchoVerifyResult(_ptr(draft_token), _ptr(prev_token), _ptr(target_token), _ptr(target_logits),
+                               int(vocab), int(target_logits.stride(0)) if target_logits is not None else 0)
+        ck = kv.c_struct()
+        if not compact:
+            ck.k_pool = None
+            ck.v_pool = None
+        oa = EchoAccept(_ptr(acc.accept_len), _ptr(acc.last_node), _ptr(acc.bonus_token), _ptr(acc.new_len),
+                        _ptr(acc.accept_idx), _ptr(acc.slot_src), _ptr(acc.slot_dst),
+                        _ptr(acc.target_token) if target_logits is not None else None)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_accept(self._h, C.byref(cs), C.byref(res), sel.R, C.byref(ck), C.byref(oa),
+                                         self._stream()))
+        return acc

@@ -1,0 +1,141 @@
+"""-m gpu parity: echo_verify_attn (CUDA, through the C ABI) against the fp64 oracle.
+Bar (BASELINE.json north_star): max|O - O_oracle| <= 1e-2 on the bf16 output, max|lse - lse_oracle| <= 1e-3."""
+import numpy as np
+import pytest
+
+from oracle import echo_oracle as orc
+from paper_2604_09603_b200 import workloads as W
+from helpers import oracle_gate_select, torch_bf16_to_bits, bf16_bits_to_f32
+from gpu_util import dev, get_ctx, run_gate_select, make_kv
+
+pytestmark = pytest.mark.gpu
+TOL_O, TOL_LSE = 1e-2, 1e-3
+SM_SCALE = 1.0 / np.sqrt(128.0)
+
+
+def _setup(wl, gate=None, poison=False, q_zero=False):
+    ctx = get_ctx()
+    sel = run_gate_select(ctx, wl, gate)
+    want_sel = oracle_gate_select(orc, wl, gate)
+    cap = max(1, sel.capacity)
+    q, k, v = W.draw_qkv(wl, cap, device="cuda")
+    if q_zero:
+        q.zero_()
+    if poison:
+        K = np.diff(want_sel["sel_offsets"])
+        W.poison_unused_slots(wl, k, v, used_extra=K)
+    return ctx, sel, want_sel, q, k, v
+
+
+def _compare(wl, want_sel, q, k, v, out, lse, rows=None):
+    n = want_sel["n_selected"]
+    qb, kb, vb = torch_bf16_to_bits(q), torch_bf16_to_bits(k), torch_bf16_to_bits(v)
+    o_gpu = bf16_bits_to_f32(torch_bf16_to_bits(out)).astype(np.float64)
+    l_gpu = lse.cpu().numpy().astype(np.float64)
+    if rows is None:
+        O, L = orc.verify_attn(want_sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE)
+        eo = np.abs(o_gpu[:n] - O).max() if n else 0.0
+        el = np.abs(l_gpu[:n] - L).max() if n else 0.0
+    else:
+        res = orc.verify_attn(want_sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, rows=rows)
+        eo = max(np.abs(o_gpu[k_, h] - res[(k_, h)][0]).max() for (k_, h) in rows)
+        el = max(abs(l_gpu[k_, h] - res[(k_, h)][1]) for (k_, h) in rows)
+    assert np.isfinite(o_gpu[:n]).all() and np.isfinite(l_gpu[:n]).all()
+    assert eo <= TOL_O, f"max|dO| = {eo}"
+    assert el <= TOL_LSE, f"max|dlse| = {el}"
+    return eo, el
+
+
+PATHS = [1, 2]
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("splits", [0, 1, 2, 3, 7])
+@pytest.mark.parametrize("gated", [True, False])
+def test_attn_cfg0_full(path, splits, gated):
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(0, gated=gated)
+    ctx, sel, want_sel, q, k, v = _setup(wl, poison=True)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, splits)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    _compare(wl, want_sel, q, k, v, out, lse)
+    assert ctx.device_status() == 0
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_attn_q_zero_closed_form(path):
+    """Q = 0: O = mean of the visible V rows, lse = ln(P_i + depth + 1) (closed form, SURVEY 8(c) pin (i))."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(0, gated=False)
+    ctx, sel, want_sel, q, k, v = _setup(wl, q_zero=True, poison=True)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    n = want_sel["n_selected"]
+    expect = np.log(wl.prefix_len[want_sel["sel_req"]].astype(np.float64) + want_sel["sel_depth"] + 1.0)
+    got = lse.cpu().numpy()[:n]
+    assert np.abs(got - expect[:, None]).max() <= TOL_LSE
+    _compare(wl, want_sel, q, k, v, out, lse)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,R,static", [(1, 3, False), (2, 3, False), (2, 2, True), (3, 2, False), (4, 4, False)])
+def test_attn_scaled_configs_sampled(path, cfg, R, static):
+    """cfg1-4 shapes at reduced batch: several KV tiles, ragged tails, G = 4 / 8 / 16; sampled rows."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(cfg, R=R, static=static, gated=not static)
+    ctx, sel, want_sel, q, k, v = _setup(wl, poison=True)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    n = want_sel["n_selected"]
+    rng = np.random.default_rng(cfg)
+    rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(96)]
+    rows += [(0, 0), (n - 1, wl.Hq - 1)]
+    _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
+    assert ctx.device_status() == 0
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_attn_edge_prefix_zero_and_empty_request(path):
+    """P_i = 0 (tree only), a request that gets no budget (K_i = 0), P_i a multiple of the tile."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(0, gated=False, R=6)
+    wl.prefix_len[:] = np.asarray([0, 128, 1, 256, 15, 16], np.int32)
+    wl.page_table, wl.num_pages = W.paged_layout(np.random.default_rng(11), wl.prefix_len, np.diff(wl.cand_offsets))
+    wl.logq[wl.cand_offsets[2]:wl.cand_offsets[3]] = np.float32(-50.0)   # request 2 loses every slot
+    g = wl.gate.replace(budget=40)
+    ctx, sel, want_sel, q, k, v = _setup(wl, g, poison=True)
+    assert np.diff(want_sel["sel_offsets"])[2] == 0
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    for splits in (1, 2):
+        ctx.set_option(echo.OPT_FORCE_SPLITS, splits)
+        out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+        _compare(wl, want_sel, q, k, v, out, lse)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_attn_sibling_isolation(path):
+    """perturbing K/V of a non-ancestor tree node leaves a row unchanged bit for bit."""
+    import torch
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(0, gated=False)
+    ctx, sel, want_sel, q, k, v = _setup(wl)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 1)
+    kv = make_kv(wl, k, v)
+    out0, lse0 = ctx.verify_attn(sel, kv, q, SM_SCALE)
+    out0, lse0 = out0.clone(), lse0.clone()
+    offs = want_sel["sel_offsets"]
+    i = 3
+    Ki = int(offs[i + 1] - offs[i])
+    masks = want_sel["masks"][offs[i]:offs[i + 1]]
+    victim = Ki - 1                                    # last packed node of request 3: nobody's ancestor but itself
+    pos = int(wl.prefix_len[i]) + victim
+    pg, sl = int(wl.page_table[i, pos // 16]), pos % 16
+    k[0, pg, :, sl, :] = 3.0
+    v[0, pg, :, sl, :] = -7.0
+    out1, lse1 = ctx.verify_attn(sel, kv, q, SM_SCALE)
+    keep = [int(offs[i]) + l for l in range(Ki) if not (masks[l] >> victim) & 1]
+    assert len(keep) == Ki - 1
+    assert torch.equal(out0[keep], out1[keep]) and torch.equal(lse0[keep], lse1[keep])
+    assert not torch.equal(out0[int(offs[i]) + victim], out1[int(offs[i]) + victim])
