@@ -117,12 +117,18 @@ __global__ void k_attn_smallrow(const int32_t* __restrict__ n_selected, const in
 }
 
 // S7: lse = ln sum_s exp(lse_s), O = sum_s exp(lse_s - lse) O_s; one warp per (node, head) row.
-__global__ void k_lse_merge(const int32_t* __restrict__ n_selected, int Hq, size_t n_rows_cap, int splits,
-                            const float* __restrict__ part_o, const float* __restrict__ part_lse,
+__global__ void k_lse_merge(const int32_t* __restrict__ n_selected, const int32_t* __restrict__ sel_req,
+                            const int32_t* __restrict__ sel_offsets, const int32_t* __restrict__ prefix_len, int Hq,
+                            size_t n_rows_cap, int splits_cap, const float* __restrict__ part_o, const float* __restrict__ part_lse,
                             __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
   const size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (row >= (size_t)(*n_selected) * Hq) return;
+  // splits that hold no KV tile of this request were never written: same rule as the planners
+  const int i = sel_req[row / Hq];
+  const int n_tiles = (prefix_len[i] + sel_offsets[i + 1] - sel_offsets[i] + TILE - 1) / TILE;
+  const int tps = (n_tiles + splits_cap - 1) / splits_cap;
+  const int splits = (n_tiles + tps - 1) / tps;
   float mx = -INFINITY;
   for (int s = 0; s < splits; ++s) mx = fmaxf(mx, part_lse[(size_t)s * n_rows_cap + row]);
   float den = 0.f;
@@ -189,7 +195,8 @@ int launch_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV
   if (splits > 1) {
     const int wpb = 8;
     const unsigned blocks = (unsigned)((n_rows + wpb - 1) / wpb);
-    k_lse_merge<<<blocks, wpb * 32, 0, st>>>(sel->n_selected, Hq, n_rows, splits, part_o, part_lse,
+    k_lse_merge<<<blocks, wpb * 32, 0, st>>>(sel->n_selected, sel->sel_req, sel->sel_offsets, kv->prefix_len, Hq,
+                                             n_rows, splits, part_o, part_lse,
                                              reinterpret_cast<__nv_bfloat16*>(out), lse);
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());

@@ -1,6 +1,514 @@
-// tcgen05 / TMA verify-attention kernel -- placeholder until the real kernel lands.
+// S6 on the 5th-gen tensor cores: persistent, warp-specialised split-KV verify attention.
+//
+//   work item  = (request i, KV head, 128-row tile of (node, head-in-group) rows, KV split)
+//   warp 0     = TMA producer: Q tile (3-D tensor map over [node][head][d]) and, per 128-token KV tile,
+//                one 16x64 box per (page, d-half) for K and V (pages are looked up in the page table)
+//   warp 1     = MMA issuer (one lane): S = Q K^T (SS, K-major x K-major) into TMEM, O += P V (TS: P read
+//                from TMEM, V as the MN-major B operand) -- accumulators never leave TMEM
+//   warps 2-5  = softmax: thread = row; tcgen05.ld S, tree mask only in tiles that touch positions >= P_i,
+//                lazy rescale of O (only when the running max grows by > 2^8), P written back to TMEM as
+//                bf16 over S, epilogue normalises and stores out/lse (or the fp32 split partial)
+// Each KV page is read once per (KV head, row tile) and serves all rows of the tile; K/V rings and the S
+// double buffer keep TMA, tensor pipe and MUFU busy at the same time.
+// Operator definition: include/echo.h (paper: P:39, P:85 names it only; readings R:A-1..A-8).
+#include <cuda.h>
+
 #include "common.cuh"
-int launch_verify_attn_tc(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t, int32_t, int32_t, const void*,
-                          void*, float*, float, int, float*, float*, cudaStream_t) {
-  return ECHO_ERR_UNSUPPORTED;
+#include "tc_ptx.cuh"
+
+namespace {
+
+constexpr int D = 128;
+constexpr int PAGE = 16;
+constexpr int TILE_M = 128;
+constexpr int TILE_N = 128;
+constexpr int NSTAGE = 3;
+constexpr int HALF_BYTES = TILE_N * 128;     // [128 rows][64 bf16], 128-byte rows, SW128
+constexpr int TILE_BYTES = 2 * HALF_BYTES;   // both d-halves: 32 KB
+constexpr int PAGE_HALF_BYTES = PAGE * 128;  // one TMA box: 16 rows x 128 B
+constexpr int SMEM_Q = 0;
+constexpr int SMEM_K = SMEM_Q + TILE_BYTES;
+constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
+constexpr int SMEM_BAR = SMEM_V + NSTAGE * TILE_BYTES;
+constexpr int SMEM_TOTAL = SMEM_BAR + 256 + 1024;  // + barriers + slack for 1024-byte alignment
+constexpr int NTHREADS = 192;
+constexpr int TMEM_COLS = 512;  // S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_b aliases S_b[0,64)
+constexpr float LOG2E = 1.4426950408889634f;
+constexpr float LN2 = 0.6931471805599453f;
+constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 domain: P values stay <= 2^8
+
+constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
+constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
+
+// barrier indices (8 bytes each)
+enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 16,
+       B_PVDONE = 18, B_OFULL = 19, B_OFREE = 21, B_COUNT = 23 };
+
+struct AttnParams {
+  const int4* items;
+  const int32_t* n_items;
+  const int32_t* sel_offsets;
+  const uint4* anc_mask;
+  const int32_t* page_table;
+  const int32_t* prefix_len;
+  int max_pages, Hkv, Hq, G, log2G;
+  int page_row_base;  // layer * num_pages
+  __nv_bfloat16* out;
+  float* lse;
+  float scale_log2;
+  int splits;
+  float* part_o;
+  float* part_lse;
+  size_t n_rows_cap;
+  uint32_t* status;
+};
+
+struct Item { int req, kvh, rt, split, jt0, jt1; };
+__device__ __forceinline__ Item decode(const int4 v) {
+  Item it;
+  it.req = v.x; it.kvh = v.y & 0xff; it.rt = (v.y >> 8) & 0xff; it.split = (v.y >> 16) & 0xff; it.jt0 = v.z; it.jt1 = v.w;
+  return it;
+}
+// snake order over the length-sorted work list: round k of CTA c takes k*G+c (k even) or (k+1)*G-1-c (k odd)
+__device__ __forceinline__ int item_index(int k, int cta, int grid) {
+  return (k & 1) ? (k + 1) * grid - 1 - cta : k * grid + cta;
+}
+
+__device__ __forceinline__ uint32_t mask_word(const uint4& m, int w) {
+  return w == 0 ? m.x : w == 1 ? m.y : w == 2 ? m.z : w == 3 ? m.w : 0u;
+}
+// visibility of tokens t0..t0+31 for a row with ancestor mask m: t < P, or bit (t - P) of m (R:A-1, A-2)
+__device__ __forceinline__ uint32_t visible_word(const uint4& m, int P, int t0) {
+  const int npref = P - t0;
+  uint32_t bits = npref >= 32 ? 0xffffffffu : npref <= 0 ? 0u : ((1u << npref) - 1u);
+  const int a0 = t0 - P;
+  if (a0 >= 0) {
+    if (a0 < 128) bits |= __funnelshift_r(mask_word(m, a0 >> 5), mask_word(m, (a0 >> 5) + 1), a0 & 31);
+  } else if (a0 > -32) {
+    bits |= m.x << (-a0);
+  }
+  return bits;
+}
+
+__global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_constant__ CUtensorMap tmap_q,
+                                                                const __grid_constant__ CUtensorMap tmap_k,
+                                                                const __grid_constant__ CUtensorMap tmap_v,
+                                                                const AttnParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t sbase = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = sbase + SMEM_Q, sK = sbase + SMEM_K, sV = sbase + SMEM_V, sBar = sbase + SMEM_BAR;
+  uint8_t* gen_base = smem_raw + (sbase - tc::smem_u32(smem_raw));  // generic pointer to the aligned base
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_BAR + B_COUNT * 8);
+  auto bar = [&](int i) -> uint32_t { return sBar + 8u * i; };
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cta = blockIdx.x, grid = gridDim.x;
+  const int n_items = *p.n_items;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < B_COUNT; ++i) {
+      const uint32_t cnt = (i == B_PFULL || i == B_PFULL + 1 || i == B_OFREE || i == B_OFREE + 1) ? 128u : 1u;
+      tc::mbar_init(bar(i), cnt);
+    }
+    tc::fence_barrier_init();
+    tc::prefetch_tmap(&tmap_q);
+    tc::prefetch_tmap(&tmap_k);
+    tc::prefetch_tmap(&tmap_v);
+  }
+  if (warp == 1) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == 0) {
+    // ============================== TMA producer ==============================
+    int g = 0, itc = 0;
+    for (int k = 0; k * grid < n_items; ++k) {
+      const int idx = item_index(k, cta, grid);
+      if (idx >= n_items) continue;
+      const Item it = decode(p.items[idx]);
+      const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
+      const int total = P + (p.sel_offsets[it.req + 1] - off);
+      if (lane == 0) {
+        tc::mbar_wait(bar(B_QEMPTY), (itc & 1) ^ 1);
+        tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
+        const int node0 = off + it.rt * (TILE_M >> p.log2G);
+        tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
+        tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
+      }
+      const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
+      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+        const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
+        const int nvalid = min(TILE_N, total - j * TILE_N);
+        int npv = (nvalid + PAGE - 1) / PAGE;
+        if (j * 8 + npv > p.max_pages) {  // page table too short: flag, load what exists
+          if (lane == 0) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
+          npv = max(0, p.max_pages - j * 8);
+        }
+        // lanes 0-15: K boxes, lanes 16-31: V boxes; lane -> (page, d-half)
+        const int pg_i = (lane & 15) >> 1, half = lane & 1;
+        int row = 0;
+        if (pg_i < npv) row = ((p.page_row_base + pt[j * 8 + pg_i]) * p.Hkv + it.kvh) * PAGE;
+        const uint32_t dst_off = slot * TILE_BYTES + half * HALF_BYTES + pg_i * PAGE_HALF_BYTES;
+        tc::mbar_wait(bar(B_KEMPTY + slot), ph ^ 1);
+        if (lane == 0) tc::mbar_expect_tx(bar(B_KFULL + slot), npv * 2 * PAGE_HALF_BYTES);
+        __syncwarp();
+        if (lane < 16 && pg_i < npv) tc::tma_load_2d(sK + dst_off, &tmap_k, bar(B_KFULL + slot), half * 64, row);
+        tc::mbar_wait(bar(B_VEMPTY + slot), ph ^ 1);
+        if (lane == 16) tc::mbar_expect_tx(bar(B_VFULL + slot), npv * 2 * PAGE_HALF_BYTES);
+        __syncwarp();
+        if (lane >= 16 && pg_i < npv) tc::tma_load_2d(sV + dst_off, &tmap_v, bar(B_VFULL + slot), half * 64, row);
+      }
+      ++itc;
+    }
+  } else if (warp == 1) {
+    // ============================== MMA issuer (one lane) ==============================
+    if (lane == 0) {
+      int g = 0, itc = 0;
+      const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
+      auto issue_qk = [&](int gg) {
+        const int slot = gg % NSTAGE, b = gg & 1;
+        tc::mbar_wait(bar(B_KFULL + slot), (gg / NSTAGE) & 1);
+        tc::tc_fence_after();
+        const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, 1024);
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t o16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
+          tc::mma_ss(tmem + b * TILE_N, qdesc + o16, kdesc + o16, IDESC_QK, kk > 0);
+        }
+        tc::mma_commit(bar(B_SFULL + b));
+        tc::mma_commit(bar(B_KEMPTY + slot));
+      };
+      for (int k = 0; k * grid < n_items; ++k) {
+        const int idx = item_index(k, cta, grid);
+        if (idx >= n_items) continue;
+        const Item it = decode(p.items[idx]);
+        const int n = it.jt1 - it.jt0, opar = itc & 1;
+        const uint32_t tO = tmem + 2 * TILE_N + opar * D;
+        tc::mbar_wait(bar(B_QFULL), itc & 1);
+        tc::tc_fence_after();
+        issue_qk(g);
+        if (n == 1) tc::mma_commit(bar(B_QEMPTY));
+        for (int j = 0; j < n; ++j) {
+          if (j + 1 < n) {
+            issue_qk(g + j + 1);
+            if (j + 2 == n) tc::mma_commit(bar(B_QEMPTY));
+          }
+          const int gg = g + j, b = gg & 1, slot = gg % NSTAGE;
+          tc::mbar_wait(bar(B_PFULL + b), (gg >> 1) & 1);
+          tc::mbar_wait(bar(B_VFULL + slot), (gg / NSTAGE) & 1);
+          if (j == 0) tc::mbar_wait(bar(B_OFREE + opar), ((itc >> 1) & 1) ^ 1);
+          tc::tc_fence_after();
+          // V tile as MN-major B: 64-wide d atoms HALF_BYTES apart (LBO), 8-token groups 1024 B apart (SBO)
+          const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, HALF_BYTES, 1024);
+#pragma unroll
+          for (int kk = 0; kk < TILE_N / 16; ++kk)
+            tc::mma_ts(tO, tmem + b * TILE_N + kk * 8, vdesc + ((kk * 2048) >> 4), IDESC_PV, (j > 0) || (kk > 0));
+          tc::mma_commit(bar(B_VEMPTY + slot));
+          tc::mma_commit(bar(B_PVDONE));
+          if (j == n - 1) tc::mma_commit(bar(B_OFULL + opar));
+        }
+        g += n;
+        ++itc;
+      }
+    }
+    __syncwarp();
+  } else {
+    // ============================== softmax + epilogue (4 warps, thread = row) ==============================
+    const int wq = warp & 3;  // TMEM lane quarter this warp may access
+    const int row = wq * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
+    int g = 0, itc = 0;
+    for (int k = 0; k * grid < n_items; ++k) {
+      const int idx = item_index(k, cta, grid);
+      if (idx >= n_items) continue;
+      const Item it = decode(p.items[idx]);
+      const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
+      const int Ki = p.sel_offsets[it.req + 1] - off;
+      const int total = P + Ki;
+      const int r_glob = it.rt * TILE_M + row;
+      const int l = r_glob >> p.log2G, gq = r_glob & (p.G - 1);
+      const bool valid = l < Ki;
+      uint4 mk = make_uint4(0u, 0u, 0u, 0u);
+      if (valid) mk = p.anc_mask[off + l];
+      float m_used = -INFINITY, lsum = 0.f;
+      const int opar = itc & 1;
+      const uint32_t tO = tmem + 2 * TILE_N + opar * D + lane_addr;
+
+      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+        const int b = g & 1;
+        const uint32_t tS = tmem + b * TILE_N + lane_addr;
+        tc::mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
+        tc::tc_fence_after();
+        uint32_t s[4][32];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tc::tmem_ld32(tS + c * 32, s[c]);
+        tc::tmem_wait_ld();
+        const int tok0 = j * TILE_N;
+        if (tok0 + TILE_N > P) {  // tile touches tree positions or the ragged end: apply visibility
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const uint32_t vis = visible_word(mk, P, tok0 + c * 32);
+#pragma unroll
+            for (int e = 0; e < 32; ++e)
+              if (!((vis >> e) & 1u)) s[c][e] = 0xff800000u;  // -inf
+          }
+        }
+        float mx = -INFINITY;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+          for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(s[c][e]));
+        const float m_new = fmaxf(m_used, mx * p.scale_log2);
+        const bool need = m_new > m_used + RESCALE_THRESHOLD;
+        if (__any_sync(0xffffffffu, need)) {
+          float alpha = 1.f;
+          if (need) {
+            alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
+            m_used = m_new;
+          }
+          lsum *= alpha;
+          if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale in TMEM
+            tc::mbar_wait(bar(B_PVDONE), (g - 1) & 1);
+            tc::tc_fence_after();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint32_t o[32];
+              tc::tmem_ld32(tO + c * 32, o);
+              tc::tmem_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+              tc::tmem_st32(tO + c * 32, o);
+            }
+            tc::tmem_wait_st();
+          }
+        }
+        const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+        const float neg_m = -m_eff;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int e = 0; e < 32; e += 2) {
+            const float p0 = tc::ex2(fmaf(__uint_as_float(s[c][e]), p.scale_log2, neg_m));
+            const float p1 = tc::ex2(fmaf(__uint_as_float(s[c][e + 1]), p.scale_log2, neg_m));
+            lsum += p0 + p1;
+            pk[e >> 1] = tc::pack_bf16(p0, p1);
+          }
+#pragma unroll
+          for (int e = 0; e < 16; ++e) s[c >> 1][(c & 1) * 16 + e] = pk[e];  // reuse s[0..1] as the packed P row
+        }
+        tc::tmem_st32(tS, s[0]);
+        tc::tmem_st32(tS + 32, s[1]);
+        tc::tmem_wait_st();
+        if (tok0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
+          const int slot = g % NSTAGE;
+          tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
+          if (row >= total - tok0) {
+            uint4* z0 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + row * 128);
+            uint4* z1 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + HALF_BYTES + row * 128);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { z0[e] = make_uint4(0u, 0u, 0u, 0u); z1[e] = make_uint4(0u, 0u, 0u, 0u); }
+          }
+          tc::fence_proxy_async();
+        }
+        tc::tc_fence_before();
+        tc::mbar_arrive(bar(B_PFULL + b));
+      }
+
+      // ---- epilogue: O / l, lse = ln2 * (m + log2 l) ----
+      tc::mbar_wait(bar(B_OFULL + opar), (itc >> 1) & 1);
+      tc::tc_fence_after();
+      const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+      const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+      const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
+      const size_t rowg = (size_t)(off + l) * p.Hq + it.kvh * p.G + gq;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint32_t o[32];
+        tc::tmem_ld32(tO + c * 32, o);
+        tc::tmem_wait_ld();
+        if (valid) {
+          if (p.splits == 1) {
+            uint4* dst = reinterpret_cast<uint4*>(p.out + rowg * D + c * 32);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              uint4 w;
+              w.x = tc::pack_bf16(__uint_as_float(o[8 * e + 0]) * inv, __uint_as_float(o[8 * e + 1]) * inv);
+              w.y = tc::pack_bf16(__uint_as_float(o[8 * e + 2]) * inv, __uint_as_float(o[8 * e + 3]) * inv);
+              w.z = tc::pack_bf16(__uint_as_float(o[8 * e + 4]) * inv, __uint_as_float(o[8 * e + 5]) * inv);
+              w.w = tc::pack_bf16(__uint_as_float(o[8 * e + 6]) * inv, __uint_as_float(o[8 * e + 7]) * inv);
+              dst[e] = w;
+            }
+          } else {
+            float4* dst = reinterpret_cast<float4*>(p.part_o + ((size_t)it.split * p.n_rows_cap + rowg) * D + c * 32);
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+              dst[e] = make_float4(__uint_as_float(o[4 * e + 0]) * inv, __uint_as_float(o[4 * e + 1]) * inv,
+                                   __uint_as_float(o[4 * e + 2]) * inv, __uint_as_float(o[4 * e + 3]) * inv);
+          }
+        }
+      }
+      if (valid) {
+        if (p.splits == 1) p.lse[rowg] = lse_v;
+        else p.part_lse[(size_t)it.split * p.n_rows_cap + rowg] = lse_v;
+      }
+      tc::tc_fence_before();
+      tc::mbar_arrive(bar(B_OFREE + opar));
+      ++itc;
+    }
+  }
+
+  // ---- teardown ----
+  tc::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tc::tmem_dealloc(tmem, TMEM_COLS);
+}
+
+// Device-side planner: P_i and K_i exist only on the device, so the work list is built there.
+// Items are bucketed by KV-tile count (descending) so that the snake assignment balances CTAs.
+constexpr int PLAN_THREADS = 1024;
+constexpr int PLAN_BUCKETS = 4096;
+__global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict__ sel_offsets,
+                                                       const int32_t* __restrict__ prefix_len, int R, int Hkv, int G,
+                                                       int splits, int max_items, int4* __restrict__ items,
+                                                       int32_t* __restrict__ n_items) {
+  __shared__ int s_cnt[PLAN_BUCKETS];
+  __shared__ int s_warp[32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int b = tid; b < PLAN_BUCKETS; b += PLAN_THREADS) s_cnt[b] = 0;
+  __syncthreads();
+  auto for_items = [&](auto&& fn) {
+    for (int r = tid; r < R; r += PLAN_THREADS) {
+      const int Ki = sel_offsets[r + 1] - sel_offsets[r];
+      if (Ki <= 0) continue;
+      const int n_tiles = (prefix_len[r] + Ki + TILE_N - 1) / TILE_N;
+      const int n_rt = (Ki * G + TILE_M - 1) / TILE_M;
+      const int tps = (n_tiles + splits - 1) / splits;
+      for (int s = 0; s * tps < n_tiles; ++s) {
+        const int j0 = s * tps, j1 = min(n_tiles, j0 + tps);
+        fn(r, s, j0, j1, n_rt);
+      }
+    }
+  };
+  for_items([&](int, int, int j0, int j1, int n_rt) {
+    atomicAdd(&s_cnt[PLAN_BUCKETS - 1 - min(j1 - j0, PLAN_BUCKETS - 1)], Hkv * n_rt);
+  });
+  __syncthreads();
+  {  // exclusive scan over buckets (bucket 0 = longest)
+    const int per = PLAN_BUCKETS / PLAN_THREADS;
+    int loc[per], sum = 0;
+    for (int t = 0; t < per; ++t) { loc[t] = s_cnt[tid * per + t]; sum += loc[t]; }
+    int incl = sum;
+    for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+      int w = s_warp[lane];
+      for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += v; }
+      s_warp[lane] = w;
+    }
+    __syncthreads();
+    int run = incl - sum + (warp ? s_warp[warp - 1] : 0);
+    for (int t = 0; t < per; ++t) { s_cnt[tid * per + t] = run; run += loc[t]; }
+    if (tid == PLAN_THREADS - 1) *n_items = min(run, max_items);
+  }
+  __syncthreads();
+  for_items([&](int r, int s, int j0, int j1, int n_rt) {
+    const int pos0 = atomicAdd(&s_cnt[PLAN_BUCKETS - 1 - min(j1 - j0, PLAN_BUCKETS - 1)], Hkv * n_rt);
+    int pos = pos0;
+    for (int kvh = 0; kvh < Hkv; ++kvh)
+      for (int rt = 0; rt < n_rt; ++rt, ++pos)
+        if (pos < max_items) items[pos] = make_int4(r, kvh | (rt << 8) | (s << 16), j0, j1);
+  });
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+}  // namespace
+
+int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer, int32_t Hq,
+                          int32_t R, const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,
+                          float* part_lse, cudaStream_t st) {
+  const int Hkv = kv->num_kv_heads, G = Hq / Hkv, cap = sel->capacity;
+  int log2G = 0;
+  while ((1 << log2G) < G) ++log2G;
+  if ((1 << log2G) != G || G > 128 || !(sm_scale > 0.f)) return ECHO_ERR_UNSUPPORTED;
+  EncodeTiledFn enc = get_encode();
+  if (!enc) {
+    snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled entry point not found");
+    return ECHO_ERR_CUDA;
+  }
+  const size_t total_rows = (size_t)kv->num_layers * kv->num_pages * Hkv * PAGE;
+  if (total_rows >= (1ull << 31)) return ECHO_ERR_UNSUPPORTED;
+  CUtensorMap tq, tk, tv;
+  {
+    cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)cap};
+    cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
+    cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)(TILE_M / G)};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = enc(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(Q) failed: %d", (int)r);
+      return ECHO_ERR_CUDA;
+    }
+  }
+  for (int which = 0; which < 2; ++which) {
+    cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)total_rows};
+    cuuint64_t strides[1] = {(cuuint64_t)D * 2};
+    cuuint32_t box[2] = {64, (cuuint32_t)PAGE};
+    cuuint32_t es[2] = {1, 1};
+    CUresult r = enc(which ? &tv : &tk, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, which ? kv->v_pool : kv->k_pool, dims,
+                     strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(KV) failed: %d", (int)r);
+      return ECHO_ERR_CUDA;
+    }
+  }
+  // plan region sits behind the split partials in the workspace
+  const size_t n_rows = (size_t)cap * Hq;
+  const size_t part_bytes = splits > 1 ? align_up((size_t)splits * n_rows * (D + 1) * sizeof(float), 256) : 0;
+  const int max_rt = (int)(((size_t)(cap < ECHO_MAX_CAND ? cap : ECHO_MAX_CAND) * G + TILE_M - 1) / TILE_M);
+  const size_t max_items = (size_t)R * Hkv * max_rt * splits;
+  const size_t plan_bytes = 256 + max_items * sizeof(int4);
+  if (part_bytes + plan_bytes > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  uint8_t* plan = reinterpret_cast<uint8_t*>(ctx->workspace) + part_bytes;
+  int32_t* n_items = reinterpret_cast<int32_t*>(plan);
+  int4* items = reinterpret_cast<int4*>(plan + 256);
+  k_plan<<<1, PLAN_THREADS, 0, st>>>(sel->sel_offsets, kv->prefix_len, R, Hkv, G, splits, (int)max_items, items, n_items);
+
+  static bool attr_set = false;
+  if (!attr_set) {
+    ECHO_CUDA_TRY(ctx, cudaFuncSetAttribute(k_verify_attn_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL));
+    attr_set = true;
+  }
+  AttnParams p;
+  p.items = items; p.n_items = n_items; p.sel_offsets = sel->sel_offsets;
+  p.anc_mask = reinterpret_cast<const uint4*>(sel->anc_mask);
+  p.page_table = kv->page_table; p.prefix_len = kv->prefix_len; p.max_pages = kv->max_pages_per_req;
+  p.Hkv = Hkv; p.Hq = Hq; p.G = G; p.log2G = log2G; p.page_row_base = layer * kv->num_pages;
+  p.out = reinterpret_cast<__nv_bfloat16*>(out); p.lse = lse; p.scale_log2 = sm_scale * LOG2E; p.splits = splits;
+  p.part_o = part_o; p.part_lse = part_lse; p.n_rows_cap = n_rows; p.status = ctx->dev_status;
+  int grid = ctx->opt_num_ctas > 0 ? (int)ctx->opt_num_ctas : ctx->num_sms;
+  if ((size_t)grid > max_items) grid = (int)(max_items ? max_items : 1);
+  k_verify_attn_tc<<<grid, NTHREADS, SMEM_TOTAL, st>>>(tq, tk, tv, p);
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
 }
