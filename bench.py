@@ -1,0 +1,345 @@
+"""bench.py -- one "step" = one pass of the whole super-tree verify step (echo_gate_select ->
+echo_verify_attn (one layer) -> echo_accept) over one synthetic batch.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+Prints ONE JSON line (rank 0).  metric = verified draft tokens/s (BASELINE.json); `roofline` is
+the verify-attention kernel against the measured HBM peak; `cpu_baseline` is the CPU oracle timed
+on a bounded sample; `e2e` repeats the step with host buffers (pinned H2D of the step inputs,
+D2H of the results inside the timed region; the paged KV cache is resident serving state).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+SM_SCALE = 1.0 / np.sqrt(128.0)
+WORKLOADS = {1: "cfg1 LLaMA-3.1-8B shape BS=32 B=1024", 2: "cfg2 LLaMA-3.3-70B shape BS=128 B=2048",
+             3: "cfg3 Qwen3-235B shape BS=128 B=1024", 4: "cfg4 stress BS=256 B=4096 logits argmax",
+             0: "cfg0 tiny"}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """samples nvidia-smi clocks / throttle reasons during the timed region"""
+
+    def __init__(self, idx=0):
+        super().__init__(daemon=True)
+        self.idx, self.stop_flag, self.rows = idx, False, []
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self.stop_flag:
+            try:
+                o = subprocess.run(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                                   capture_output=True, text=True, timeout=5).stdout.strip()
+                if o:
+                    self.rows.append([x.strip() for x in o.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None, "reasons": reasons}
+
+
+def algorithmic_bytes(wl, sel_h):
+    """K and V of every visible page once per KV head + Q read + O write + LSE."""
+    K = np.diff(sel_h["sel_offsets"]).astype(np.int64)
+    P = wl.prefix_len.astype(np.int64)
+    act = K > 0
+    kvb = (2 * wl.Hkv * 128 * 2 * (P + K))[act].sum()
+    qo = (2 * K * wl.Hq * 128 * 2 + 4 * K * wl.Hq).sum()
+    depth = sel_h["sel_depth"].astype(np.int64)
+    flops = (4 * 128 * wl.Hq * (P[sel_h["sel_req"]] + depth + 1)).sum()
+    return int(kvb + qo), int(flops)
+
+
+def oracle_sample(wl, n_attn_nodes=6, qkv=None):
+    """The CPU oracle as it stands on a bounded sample: gating + acceptance on the whole batch,
+    attention (all Hq heads) for `n_attn_nodes` packed nodes.  Returns (tokens/s, description, cores)."""
+    from oracle import echo_oracle as orc           # cpu_baseline / reference arm only
+    g = wl.gate
+    t0 = time.perf_counter()
+    sel = orc.gate_select(wl.cand_offsets, wl.parent, wl.logq, g.depth_mask, g.log_tau, g.w_max, g.budget, g.static_k)
+    t_gate = time.perf_counter() - t0
+    n = sel["n_selected"]
+    glob = wl.cand_offsets[sel["sel_req"]] + sel["sel_node"]
+    t0 = time.perf_counter()
+    orc.accept(sel, wl.draft_token[glob], wl.prev_token, wl.target_after[glob], wl.R)
+    t_acc = time.perf_counter() - t0
+    rng = np.random.default_rng(1)
+    nodes = sorted(set(int(x) for x in rng.integers(0, max(1, n), size=n_attn_nodes)))
+    if qkv is None:
+        # same distribution as the GPU arm (bf16 N(0,1)), drawn on the host for the sampled requests only
+        # timing depends on shapes only: finite bf16 bit patterns (|x| in [2^-7, 2)) with random signs
+        def bits(shape):
+            return (rng.integers(0x3C00, 0x4000, size=shape, dtype=np.uint16) |
+                    (rng.integers(0, 2, size=shape, dtype=np.uint16) << 15))
+        qb = bits((max(1, n), wl.Hq, 128))
+        pool = bits((1, wl.num_pages, wl.Hkv, 16, 128))
+        kb = vb = pool
+    else:
+        qb, kb, vb = qkv
+    rows = [(k, h) for k in nodes for h in range(wl.Hq)]
+    t0 = time.perf_counter()
+    orc.verify_attn(sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, rows=rows)
+    t_attn = time.perf_counter() - t0
+    t_total = t_attn + (t_gate + t_acc) * len(nodes) / max(1, n)
+    desc = (f"{wl.name}: attention of {len(nodes)} packed nodes x {wl.Hq} heads ({t_attn:.2f}s) + the nodes' share of "
+            f"gating ({t_gate:.2f}s) and acceptance ({t_acc:.2f}s) over all {n} nodes")
+    return len(nodes) / t_total, desc, 1
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle (kind 'oracle') on the same config / metric, rank 0 only."""
+    if rank != 0:
+        return
+    from paper_2604_09603_b200 import workloads as W
+    wl = W.make_config(args.config)
+    vals = []
+    for _ in range(args.warmup):
+        oracle_sample(wl, n_attn_nodes=1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        v, desc, cores = oracle_sample(wl, n_attn_nodes=args.ref_nodes)
+        vals.append(v)
+    dt = time.perf_counter() - t0
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": "verified draft tokens/s", "value": value, "unit": "tokens/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config]},
+            "cpu_baseline": {"value": value, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_gpu(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2604_09603_b200 import build, echo, workloads as W
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    build.build_library()
+    wl = W.make_config(args.config, seed=W.SEED_BASE + args.config + 1000 * rank)
+    g = wl.gate
+    cap = wl.capacity()
+    ctx = echo.EchoContext(local_rank, 0)
+    ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq)
+    if args.attn_path:
+        ctx.set_option(echo.OPT_ATTN_PATH, args.attn_path)
+    if args.splits:
+        ctx.set_option(echo.OPT_FORCE_SPLITS, args.splits)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+
+    h_in = {"cand_offsets": pin(wl.cand_offsets), "parent": pin(wl.parent), "logq": pin(wl.logq),
+            "prev": pin(wl.prev_token)}
+    d_in = {k: v.to(dev) for k, v in h_in.items()}
+    q, k, v = W.draw_qkv(wl, cap, device=str(dev))
+    kv = echo.PagedKV(k, v, d(wl.page_table), d(wl.prefix_len))
+    sel = ctx.alloc_selection(wl.R, wl.N, cap)
+    acc = ctx.alloc_accept(wl.R, cap)
+    out = torch.zeros_like(q)
+    lse = torch.zeros(cap, wl.Hq, dtype=torch.float32, device=dev)
+
+    def gate(din):
+        return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
+                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel)
+
+    gate(d_in)
+    sel_h = sel.to_host()
+    n_sel = sel_h["n_selected"]
+    glob = (wl.cand_offsets[sel_h["sel_req"]] + sel_h["sel_node"]).astype(np.int64)
+    pad = lambda a: np.concatenate([a, np.zeros(cap - len(a), a.dtype)]).astype(np.int32)
+    h_in["draft"] = pin(pad(wl.draft_token[glob]))
+    h_in["target"] = pin(pad(wl.target_after[glob]))
+    d_in["draft"], d_in["target"] = h_in["draft"].to(dev), h_in["target"].to(dev)
+    logits = None
+    if args.config == 4:
+        logits = W.draw_logits(wl, glob, device=str(dev))
+        if logits.shape[0] < cap:
+            logits = torch.cat([logits, torch.zeros(cap - logits.shape[0], logits.shape[1], dtype=logits.dtype, device=dev)])
+    bytes_alg, flops_alg = algorithmic_bytes(wl, sel_h)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    attn_ev = [(ev(), ev()) for _ in range(args.steps)]
+    gate_ev = [(ev(), ev()) for _ in range(args.steps)]
+
+    def step(din, i=None, qq=q):
+        if i is not None:
+            gate_ev[i][0].record()
+        gate(din)
+        if i is not None:
+            gate_ev[i][1].record(); attn_ev[i][0].record()
+        ctx.verify_attn(sel, kv, qq, SM_SCALE, out=out, lse=lse)
+        if i is not None:
+            attn_ev[i][1].record()
+        if logits is not None:
+            ctx.accept(sel, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc)
+        else:
+            ctx.accept(sel, kv, din["draft"], din["prev"], target_token=din["target"], out=acc)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(d_in)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for i in range(args.steps):
+        step(d_in, i)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    sampler.stop_flag = True
+    t_attn = float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
+    t_gate = float(np.mean([a.elapsed_time(b) for a, b in gate_ev]))
+    accepted = int(acc.accept_len[:wl.R].sum().item())
+    return dict(torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
+                accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
+                out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
+
+
+def run_e2e(r, args):
+    """Same step through the public API with HOST buffers: pinned H2D of the step's inputs (trees, logq, Q,
+    tokens) and D2H of its results (out, lse, acceptance) inside the timed region; the paged KV cache is
+    resident serving state and is not re-uploaded."""
+    torch, dev = r["torch"], r["dev"]
+    h_in, d_in = r["h_in"], r["d_in"]
+    h_q = r["q"].cpu().pin_memory()
+    d_q = r["q"]
+    h_out = torch.empty_like(r["out"], device="cpu").pin_memory()
+    h_lse = torch.empty_like(r["lse"], device="cpu").pin_memory()
+    acc = r["acc"]
+    outs = [acc.accept_len, acc.accept_idx, acc.bonus_token, acc.new_len, r["sel"].n_selected]
+    h_outs = [torch.empty_like(t, device="cpu").pin_memory() for t in outs]
+    h2d = sum(t.numel() * t.element_size() for t in h_in.values()) + h_q.numel() * 2
+    d2h = h_out.numel() * 2 + h_lse.numel() * 4 + sum(t.numel() * t.element_size() for t in outs)
+
+    def one():
+        for k_, t in h_in.items():
+            d_in[k_].copy_(t, non_blocking=True)
+        d_q.copy_(h_q, non_blocking=True)
+        r["step"](d_in, None, d_q)
+        h_out.copy_(r["out"], non_blocking=True)
+        h_lse.copy_(r["lse"], non_blocking=True)
+        for ht, t in zip(h_outs, outs):
+            ht.copy_(t, non_blocking=True)
+        torch.cuda.synchronize()
+
+    for _ in range(max(1, args.warmup // 2)):
+        one()
+    r["barrier"]()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one()
+    r["barrier"]()
+    dt = time.perf_counter() - t0
+    return dt, int(h2d), int(d2h)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: BS=128)")
+    ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
+    ap.add_argument("--attn-path", type=int, default=0)
+    ap.add_argument("--splits", type=int, default=0)
+    ap.add_argument("--ref-nodes", type=int, default=32)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    r = run_gpu(args, rank, world, local_rank)
+    torch, dist = r["torch"], r["dist"]
+    e2e_dt, h2d, d2h = run_e2e(r, args)
+    stats = torch.tensor([r["ms"], e2e_dt, -float(r["n_sel"]), -float(r["accepted"])], dtype=torch.float64, device=r["dev"])
+    tot = torch.tensor([float(r["n_sel"]), float(r["accepted"])], dtype=torch.float64, device=r["dev"])
+    if world > 1:
+        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms, e2e_dt = float(stats[0]), float(stats[1])
+    n_sel_all, acc_all = float(tot[0]), float(tot[1])
+    if rank == 0:
+        peak, peak_src = peaks()
+        achieved = r["bytes_alg"] / (r["t_attn"] * 1e-3) / 1e9
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get(f"cfg{args.config}")
+        wl = r["wl"]
+        units = wl.R * wl.Hkv
+        splits = args.splits or 1
+        if not args.splits:
+            while splits < 8 and units * splits < 2 * torch.cuda.get_device_properties(0).multi_processor_count:
+                splits *= 2
+        launches = 2 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)
+        line = {"metric": "verified draft tokens/s", "value": n_sel_all * args.steps / (ms * 1e-3), "unit": "tokens/s",
+                "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": {"workload": WORKLOADS[args.config], "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
+                           "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
+                           if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
+                           "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],
+                           "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12},
+                "accepted_tokens_per_s": acc_all * args.steps / (ms * 1e-3),
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                             "traffic": traffic, "peak_source": peak_src, "kernel": "echo_verify_attn (plan + k_verify_attn_tc"
+                             + (" + k_lse_merge)" if splits > 1 else ")"), "bytes_per_launch": r["bytes_alg"]},
+                "e2e": {"value": n_sel_all * args.steps / e2e_dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d,
+                        "d2h_bytes_per_step": d2h},
+                "gpu_launches": launches * args.steps, "clocks": r["sampler"].summary()}
+        if not args.no_cpu_baseline:
+            try:
+                v, desc, cores = oracle_sample(wl, n_attn_nodes=args.ref_nodes)
+                line["cpu_baseline"] = {"value": v, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": desc}
+            except Exception as e:  # the baseline leg must never take the GPU number down with it
+                line["cpu_baseline"] = {"value": None, "unit": "tokens/s", "cores": 1, "kind": "oracle", "sample": f"failed: {e}"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

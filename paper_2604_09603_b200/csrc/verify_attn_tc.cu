@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const bool valid = l < Ki;
       uint4 mk = make_uint4(0u, 0u, 0u, 0u);
       if (valid) mk = p.anc_mask[off + l];
-      float m_used = -INFINITY, lsum = 0.f;
+      float m_used = -INFINITY, lsum = 0.f, lsum_r = 0.f;
       const int opar = itc & 1;
       const uint32_t tO = tmem + 2 * TILE_N + opar * D + lane_addr;
 
@@ -246,7 +246,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         for (int c = 0; c < 4; ++c) tc::tmem_ld32(tS + c * 32, s[c]);
         tc::tmem_wait_ld();
         const int tok0 = j * TILE_N;
-        if (tok0 + TILE_N > P) {  // tile touches tree positions or the ragged end: apply visibility
+        const bool tail = tok0 + TILE_N > P;
+        if (tail) {  // tile touches tree positions or the ragged end: apply visibility
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             const uint32_t vis = visible_word(mk, P, tok0 + c * 32);
@@ -269,6 +270,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             m_used = m_new;
           }
           lsum *= alpha;
+          lsum_r *= alpha;
           if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale in TMEM
             tc::mbar_wait(bar(B_PVDONE), (g - 1) & 1);
             tc::tc_fence_after();
@@ -286,6 +288,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         }
         const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
         const float neg_m = -m_eff;
+        float ts = 0.f, tr = 0.f;  // this tile's exact / bf16-rounded weight sums
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[16];
@@ -293,12 +296,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           for (int e = 0; e < 32; e += 2) {
             const float p0 = tc::ex2(fmaf(__uint_as_float(s[c][e]), p.scale_log2, neg_m));
             const float p1 = tc::ex2(fmaf(__uint_as_float(s[c][e + 1]), p.scale_log2, neg_m));
-            lsum += p0 + p1;
-            pk[e >> 1] = tc::pack_bf16(p0, p1);
+            const uint32_t w = tc::pack_bf16(p0, p1);
+            pk[e >> 1] = w;
+            ts += p0 + p1;
+            // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised
+            // by the sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact
+            // convex combination of V rows; lse always uses the exact fp32 sum
+            if (tail) tr += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
           }
 #pragma unroll
           for (int e = 0; e < 16; ++e) s[c >> 1][(c & 1) * 16 + e] = pk[e];  // reuse s[0..1] as the packed P row
         }
+        lsum += ts;
+        lsum_r += tail ? tr : ts;
         tc::tmem_st32(tS, s[0]);
         tc::tmem_st32(tS + 32, s[1]);
         tc::tmem_wait_st();
@@ -320,7 +330,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       // ---- epilogue: O / l, lse = ln2 * (m + log2 l) ----
       tc::mbar_wait(bar(B_OFULL + opar), (itc >> 1) & 1);
       tc::tc_fence_after();
-      const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+      const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
       const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
       const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
       const size_t rowg = (size_t)(off + l) * p.Hq + it.kvh * p.G + gq;
