@@ -31,7 +31,7 @@ constexpr int SMEM_K = SMEM_Q + TILE_BYTES;
 constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
 constexpr int SMEM_BAR = SMEM_V + NSTAGE * TILE_BYTES;
 constexpr int SMEM_TOTAL = SMEM_BAR + 256 + 1024;  // + barriers + slack for 1024-byte alignment
-constexpr int NTHREADS = 192;
+constexpr int NTHREADS = 224;  // warps: 0 Q+K producer, 1 MMA, 2-5 softmax, 6 V producer
 constexpr int TMEM_COLS = 512;  // S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_b aliases S_b[0,64)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
@@ -121,47 +121,62 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   tc::tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  if (warp == 0) {
-    // ============================== TMA producer ==============================
-    int g = 0, itc = 0;
-    for (int k = 0; k * grid < n_items; ++k) {
-      const int idx = item_index(k, cta, grid);
-      if (idx >= n_items) continue;
-      const Item it = decode(p.items[idx]);
-      const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
-      const int total = P + (p.sel_offsets[it.req + 1] - off);
-      if (lane == 0) {
-        tc::mbar_wait(bar(B_QEMPTY), (itc & 1) ^ 1);
-        tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
-        const int node0 = off + it.rt * (TILE_M >> p.log2G);
-        tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
-        tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
-      }
-      const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
-      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
-        const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
-        const int nvalid = min(TILE_N, total - j * TILE_N);
-        int npv = (nvalid + PAGE - 1) / PAGE;
-        if (j * 8 + npv > p.max_pages) {  // page table too short: flag, load what exists
-          if (lane == 0) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
-          npv = max(0, p.max_pages - j * 8);
+  if (warp == 0 || warp == 6) {
+    // ============================== TMA producers: warp 0 = Q + K, warp 6 = V (one lane each) ==============
+    // The whole loop runs in one thread so that every TMA operand is warp-uniform by construction; page ids
+    // of tile j+1 are fetched while tile j is being issued, so no dependent global load sits between tiles.
+    if (lane == 0) {
+      const bool is_k = warp == 0;
+      const uint32_t s_dst = is_k ? sK : sV;
+      const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
+      const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
+      int g = 0, itc = 0;
+      for (int k = 0; k * grid < n_items; ++k) {
+        const int idx = item_index(k, cta, grid);
+        if (idx >= n_items) continue;
+        const Item it = decode(p.items[idx]);
+        const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
+        const int total = P + (p.sel_offsets[it.req + 1] - off);
+        if (is_k) {
+          tc::mbar_wait(bar(B_QEMPTY), (itc & 1) ^ 1);
+          tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
+          const int node0 = off + it.rt * (TILE_M >> p.log2G);
+          tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
+          tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
         }
-        // lanes 0-15: K boxes, lanes 16-31: V boxes; lane -> (page, d-half)
-        const int pg_i = (lane & 15) >> 1, half = lane & 1;
-        int row = 0;
-        if (pg_i < npv) row = ((p.page_row_base + pt[j * 8 + pg_i]) * p.Hkv + it.kvh) * PAGE;
-        const uint32_t dst_off = slot * TILE_BYTES + half * HALF_BYTES + pg_i * PAGE_HALF_BYTES;
-        tc::mbar_wait(bar(B_KEMPTY + slot), ph ^ 1);
-        if (lane == 0) tc::mbar_expect_tx(bar(B_KFULL + slot), npv * 2 * PAGE_HALF_BYTES);
-        __syncwarp();
-        if (lane < 16 && pg_i < npv) tc::tma_load_2d(sK + dst_off, &tmap_k, bar(B_KFULL + slot), half * 64, row);
-        tc::mbar_wait(bar(B_VEMPTY + slot), ph ^ 1);
-        if (lane == 16) tc::mbar_expect_tx(bar(B_VFULL + slot), npv * 2 * PAGE_HALF_BYTES);
-        __syncwarp();
-        if (lane >= 16 && pg_i < npv) tc::tma_load_2d(sV + dst_off, &tmap_v, bar(B_VFULL + slot), half * 64, row);
+        const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
+        int npages = (total + PAGE - 1) / PAGE;
+        if (npages > p.max_pages) {  // page table too short: flag, load what exists
+          if (is_k) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
+          npages = p.max_pages;
+        }
+        int cur[8], nxt[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) cur[e] = (it.jt0 * 8 + e < npages) ? pt[it.jt0 * 8 + e] : 0;
+        for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+#pragma unroll
+          for (int e = 0; e < 8; ++e) nxt[e] = (j + 1 < it.jt1 && (j + 1) * 8 + e < npages) ? pt[(j + 1) * 8 + e] : 0;
+          const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
+          const int npv = max(0, min(8, npages - j * 8));  // pages of this tile that hold tokens
+          const uint32_t dst = s_dst + slot * TILE_BYTES;
+          const uint32_t fb = bar(b_full + slot);
+          tc::mbar_wait(bar(b_empty + slot), ph ^ 1);
+          tc::mbar_expect_tx(fb, npv * 2 * PAGE_HALF_BYTES);
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            if (e < npv) {
+              const int row = ((p.page_row_base + cur[e]) * p.Hkv + it.kvh) * PAGE;
+              tc::tma_load_2d(dst + e * PAGE_HALF_BYTES, tmap, fb, 0, row);
+              tc::tma_load_2d(dst + HALF_BYTES + e * PAGE_HALF_BYTES, tmap, fb, 64, row);
+            }
+          }
+#pragma unroll
+          for (int e = 0; e < 8; ++e) cur[e] = nxt[e];
+        }
+        ++itc;
       }
-      ++itc;
     }
+    __syncwarp();
   } else if (warp == 1) {
     // ============================== MMA issuer (one lane) ==============================
     if (lane == 0) {
@@ -214,7 +229,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       }
     }
     __syncwarp();
-  } else {
+  } else if (warp < 6) {
     // ============================== softmax + epilogue (4 warps, thread = row) ==============================
     const int wq = warp & 3;  // TMEM lane quarter this warp may access
     const int row = wq * 32 + lane;
