@@ -35,7 +35,7 @@ constexpr int NTHREADS = 224;  // warps: 0 Q+K producer, 1 MMA, 2-5 softmax, 6 V
 constexpr int TMEM_COLS = 512;  // S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_b aliases S_b[0,64)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
-constexpr float RESCALE_THRESHOLD = 8.0f;  // log2 domain: P values stay <= 2^8
+constexpr float WEIGHT_SUM_LIMIT = 4294967296.f;  // a tile whose weight sum exceeds 2^32 is redone against its own maximum
 
 constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
@@ -88,6 +88,66 @@ __device__ __forceinline__ uint32_t visible_word(const uint4& m, int P, int t0) 
     bits |= m.x << (-a0);
   }
   return bits;
+}
+
+// ---- softmax passes over one S row (thread = row, 128 fp32 columns in TMEM), 32 columns per tcgen05.ld, the
+// load of chunk c+1 in flight while chunk c is processed ----
+__device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
+#pragma unroll
+  for (int e = 0; e < 32; ++e)
+    if (!((vis >> e) & 1u)) s[e] = 0xff800000u;  // -inf
+}
+
+// weights p = 2^(s*scale_log2 + neg_m) for the whole row: packed to bf16 in pk, exact fp32 sum in ts and (tail
+// tiles only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the FMA-pipe work.
+__device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[4], bool tail, float scale_log2,
+                                             float neg_m, uint32_t (&pk)[64], float& ts, float& tr) {
+  const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
+  uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
+  float trr[2] = {0.f, 0.f};
+  uint32_t s[2][32];
+  tc::tmem_ld32(tS, s[0]);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    tc::tmem_wait_ld();
+    if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
+    uint32_t(&sc)[32] = s[c & 1];
+    if (tail) mask_chunk(sc, vis[c]);
+#pragma unroll
+    for (int e = 0; e < 32; e += 2) {
+      float x0, x1;
+      tc::unpack_f32x2(tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2), x0, x1);
+      const float p0 = tc::ex2(x0), p1 = tc::ex2(x1);
+      const uint32_t w = tc::pack_bf16(p0, p1);
+      pk[c * 16 + (e >> 1)] = w;
+      acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
+      // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
+      // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
+      // combination of V rows; lse always uses the exact fp32 sum
+      if (tail) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
+    }
+  }
+  float a0, a1;
+  tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
+  ts = a0 + a1;
+  tr = trr[0] + trr[1];
+}
+
+__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4], bool tail) {
+  float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  uint32_t s[2][32];
+  tc::tmem_ld32(tS, s[0]);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    tc::tmem_wait_ld();
+    if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
+    uint32_t(&sc)[32] = s[c & 1];
+    if (tail) mask_chunk(sc, vis[c]);
+#pragma unroll
+    for (int e = 0; e < 32; e += 2)
+      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(sc[e]), __uint_as_float(sc[e + 1]));
+  }
+  return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_constant__ CUtensorMap tmap_q,
@@ -256,31 +316,29 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const uint32_t tS = tmem + b * TILE_N + lane_addr;
         tc::mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
         tc::tc_fence_after();
-        uint32_t s[4][32];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) tc::tmem_ld32(tS + c * 32, s[c]);
-        tc::tmem_wait_ld();
         const int tok0 = j * TILE_N;
-        const bool tail = tok0 + TILE_N > P;
-        if (tail) {  // tile touches tree positions or the ragged end: apply visibility
+        const bool tail = tok0 + TILE_N > P;  // tile touches tree positions or the ragged end: apply visibility
+        uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
+        if (tail) {
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const uint32_t vis = visible_word(mk, P, tok0 + c * 32);
-#pragma unroll
-            for (int e = 0; e < 32; ++e)
-              if (!((vis >> e) & 1u)) s[c][e] = 0xff800000u;  // -inf
-          }
+          for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tok0 + c * 32);
         }
-        float mx = -INFINITY;
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-#pragma unroll
-          for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(s[c][e]));
-        const float m_new = fmaxf(m_used, mx * p.scale_log2);
-        const bool need = m_new > m_used + RESCALE_THRESHOLD;
-        if (__any_sync(0xffffffffu, need)) {
+        uint32_t pk[64];  // the bf16 P row
+        float ts = 0.f, tr = 0.f;  // this tile's exact / bf16-rounded weight sums
+        // Fast path: the weights are taken against the running reference m_used without looking at this tile's
+        // maximum first; only if a weight sum leaves [0, 2^32] (reference too low, or no reference yet) does
+        // the warp fall back to the two-pass form (row maximum, rescale, weights).  P is stored only after that
+        // check, so S is still intact for the second pass.
+        bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);
+        if (!slow) {
+          weights_pass(tS, vis, tail, p.scale_log2, -m_used, pk, ts, tr);
+          slow = __any_sync(0xffffffffu, !(ts <= WEIGHT_SUM_LIMIT));
+        }
+        if (slow) {
+          float mx = row_max_pass(tS, vis, tail);
+          const float m_new = fmaxf(m_used, mx * p.scale_log2);
           float alpha = 1.f;
-          if (need) {
+          if (m_new > m_used) {
             alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
             m_used = m_new;
           }
@@ -300,32 +358,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             }
             tc::tmem_wait_st();
           }
-        }
-        const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-        const float neg_m = -m_eff;
-        float ts = 0.f, tr = 0.f;  // this tile's exact / bf16-rounded weight sums
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int e = 0; e < 32; e += 2) {
-            const float p0 = tc::ex2(fmaf(__uint_as_float(s[c][e]), p.scale_log2, neg_m));
-            const float p1 = tc::ex2(fmaf(__uint_as_float(s[c][e + 1]), p.scale_log2, neg_m));
-            const uint32_t w = tc::pack_bf16(p0, p1);
-            pk[e >> 1] = w;
-            ts += p0 + p1;
-            // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised
-            // by the sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact
-            // convex combination of V rows; lse always uses the exact fp32 sum
-            if (tail) tr += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
-          }
-#pragma unroll
-          for (int e = 0; e < 16; ++e) s[c >> 1][(c & 1) * 16 + e] = pk[e];  // reuse s[0..1] as the packed P row
+          const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+          weights_pass(tS, vis, tail, p.scale_log2, -m_eff, pk, ts, tr);
         }
         lsum += ts;
         lsum_r += tail ? tr : ts;
-        tc::tmem_st32(tS, s[0]);
-        tc::tmem_st32(tS + 32, s[1]);
+        tc::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+        tc::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
         tc::tmem_wait_st();
         if (tok0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
           const int slot = g % NSTAGE;
