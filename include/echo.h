@@ -56,6 +56,8 @@ typedef enum {
 #define ECHO_MAX_DEPTH 32   /* depth < 32 (R:G-14) */
 #define ECHO_MAX_ACCEPT 32  /* an accepted path has <= 32 nodes (one per depth) */
 #define ECHO_CUT_NEVER 0x7fffffff
+#define ECHO_PROF_CTAS 256  /* echo_debug_wait_prof: rows (persistent CTAs) ... */
+#define ECHO_PROF_SLOTS 32  /* ... x counters per CTA */
 
 /* ---- lifetime ------------------------------------------------------------------------ */
 /* Creates a context on `device` with a workspace of `workspace_bytes` (device memory, owned by
@@ -70,6 +72,13 @@ const char* echo_last_error(EchoCtx* ctx);  /* text of the last ECHO_ERR_CUDA on
 /* Copies the device status word to *flags with a blocking 4-byte copy on `stream` and clears it. */
 int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream);
 int echo_set_option(EchoCtx* ctx, int key, int64_t value);
+/* Debug hook (only in a library built with -DECHO_WAIT_PROF; ECHO_ERR_UNSUPPORTED otherwise): copies the
+ * per-CTA mbarrier wait-cycle counters of the last tcgen05 verify-attention launch to HOST memory
+ * host_out[n_ctas][ECHO_PROF_SLOTS] (uint64) after a device synchronise.  Slots: K producer 0 total,
+ * 1 wait K-empty, 2 wait Q-empty; V producer 4 total, 5 wait V-empty; MMA issuer 8 total, 9 K-full,
+ * 10 P-full, 11 V-full, 12 O-free, 13 Q-full; softmax warp 16 total, 17 S-full, 18 O-full, 19 PV-done,
+ * 20 V-full (ragged tile).  Returns the number of rows written or a negative EchoStatus. */
+int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas);
 
 /* ---- problem statement ----------------------------------- */
 /* Candidate draft trees G_i with parent function pa(j) and draft log-probabilities (Eq. 5). */

@@ -17,6 +17,11 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
+def _flags():
+    # ECHO_WAIT_PROF=1 builds the mbarrier wait-time profile into the tcgen05 kernel (echo_debug_wait_prof)
+    return NVCC_FLAGS + (["-DECHO_WAIT_PROF"] if os.environ.get("ECHO_WAIT_PROF") == "1" else [])
+
+
 def _nvcc() -> str:
     for c in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
         if c and (os.path.isabs(c) and os.path.exists(c) or not os.path.isabs(c)):
@@ -40,7 +45,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         src = os.path.join(CSRC, s)
         obj = os.path.join(HERE, "build", s.replace(".cu", ".o"))
         if force or _stale(obj, [src] + headers):
-            cmd = [_nvcc()] + NVCC_FLAGS + ["-c", src, "-o", obj]
+            cmd = [_nvcc()] + _flags() + ["-I", os.path.join(os.path.dirname(HERE), "include"), "-c", src, "-o", obj]
             r = subprocess.run(cmd, capture_output=True, text=True)
             if verbose or r.returncode != 0:
                 sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)

@@ -98,6 +98,12 @@ int echo_set_option(EchoCtx* ctx, int key, int64_t value) {
   }
 }
 
+int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas) {
+  if (!ctx || !host_out || n_ctas <= 0) return ECHO_ERR_INVALID_ARG;
+  ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
+  return debug_wait_prof(reinterpret_cast<unsigned long long*>(host_out), n_ctas);
+}
+
 int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, echo_stream_t stream) {
   if (!ctx || !t || !g || !o) return ECHO_ERR_INVALID_ARG;
   if (t->num_requests < 0 || t->total_cand < 0 || t->max_cand_per_req < 0) return ECHO_ERR_INVALID_ARG;

@@ -39,6 +39,7 @@ int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32
 int launch_accept(EchoCtx*, const EchoSelection*, const EchoVerifyResult*, int32_t R, EchoPagedKV*, EchoAccept*,
                   cudaStream_t);
 // tcgen05 path (verify_attn_tc.cu); returns ECHO_ERR_UNSUPPORTED when the shape cannot use it
+int debug_wait_prof(unsigned long long* host_out, int n_ctas);
 int launch_verify_attn_tc(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
                           const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,
                           float* part_ml, cudaStream_t);

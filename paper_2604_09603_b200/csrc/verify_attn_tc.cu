@@ -63,6 +63,27 @@ struct AttnParams {
   uint32_t* status;
 };
 
+// Optional wait-time profile (build with -DECHO_WAIT_PROF): cycles each role spends blocked on each mbarrier,
+// per CTA, read back with echo_debug_wait_prof.  Compiled out otherwise.
+#ifdef ECHO_WAIT_PROF
+__device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
+#define PROF_T0() const long long prof_t0_ = clock64()
+#define PROF_ADD(slot) prof_[slot] += clock64() - prof_t0_
+#define PROF_WAIT(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait(b, ph); prof_[slot] += clock64() - t_; } while (0)
+#define PROF_DECL(n) unsigned long long prof_[n] = {}
+#define PROF_FLUSH(base, n) do { if (blockIdx.x < ECHO_PROF_CTAS) for (int q_ = 0; q_ < n; ++q_) g_wait_prof[blockIdx.x][(base) + q_] = prof_[q_]; } while (0)
+#define PROF_SPAN_BEGIN() const long long span_t_ = clock64()
+#define PROF_SPAN_END(slot) prof_[slot] += clock64() - span_t_
+#else
+#define PROF_T0() do {} while (0)
+#define PROF_ADD(slot) do {} while (0)
+#define PROF_WAIT(slot, b, ph) tc::mbar_wait(b, ph)
+#define PROF_DECL(n) do {} while (0)
+#define PROF_FLUSH(base, n) do {} while (0)
+#define PROF_SPAN_BEGIN() do {} while (0)
+#define PROF_SPAN_END(slot) do {} while (0)
+#endif
+
 struct Item { int req, kvh, rt, split, jt0, jt1; };
 __device__ __forceinline__ Item decode(const int4 v) {
   Item it;
@@ -191,6 +212,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
       int g = 0, itc = 0;
+      PROF_DECL(3);
+      PROF_T0();
       for (int k = 0; k * grid < n_items; ++k) {
         const int idx = item_index(k, cta, grid);
         if (idx >= n_items) continue;
@@ -198,7 +221,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
         const int total = P + (p.sel_offsets[it.req + 1] - off);
         if (is_k) {
-          tc::mbar_wait(bar(B_QEMPTY), (itc & 1) ^ 1);
+          PROF_WAIT(2, bar(B_QEMPTY), (itc & 1) ^ 1);
           tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
           const int node0 = off + it.rt * (TILE_M >> p.log2G);
           tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
@@ -220,7 +243,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           const int npv = max(0, min(8, npages - j * 8));  // pages of this tile that hold tokens
           const uint32_t dst = s_dst + slot * TILE_BYTES;
           const uint32_t fb = bar(b_full + slot);
-          tc::mbar_wait(bar(b_empty + slot), ph ^ 1);
+          PROF_WAIT(1, bar(b_empty + slot), ph ^ 1);
           tc::mbar_expect_tx(fb, npv * 2 * PAGE_HALF_BYTES);
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
@@ -235,16 +258,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         }
         ++itc;
       }
+      PROF_ADD(0);
+      PROF_FLUSH(is_k ? 0 : 4, 3);
+#ifdef ECHO_WAIT_PROF
+      g_wait_prof[blockIdx.x][is_k ? 3 : 7] = g;
+#endif
     }
     __syncwarp();
   } else if (warp == 1) {
     // ============================== MMA issuer (one lane) ==============================
     if (lane == 0) {
       int g = 0, itc = 0;
+      PROF_DECL(6);
+      PROF_T0();
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
       auto issue_qk = [&](int gg) {
         const int slot = gg % NSTAGE, b = gg & 1;
-        tc::mbar_wait(bar(B_KFULL + slot), (gg / NSTAGE) & 1);
+        PROF_WAIT(1, bar(B_KFULL + slot), (gg / NSTAGE) & 1);
         tc::tc_fence_after();
         const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, 1024);
 #pragma unroll
@@ -261,7 +291,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const Item it = decode(p.items[idx]);
         const int n = it.jt1 - it.jt0, opar = itc & 1;
         const uint32_t tO = tmem + 2 * TILE_N + opar * D;
-        tc::mbar_wait(bar(B_QFULL), itc & 1);
+        PROF_WAIT(5, bar(B_QFULL), itc & 1);
         tc::tc_fence_after();
         issue_qk(g);
         if (n == 1) tc::mma_commit(bar(B_QEMPTY));
@@ -271,9 +301,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             if (j + 2 == n) tc::mma_commit(bar(B_QEMPTY));
           }
           const int gg = g + j, b = gg & 1, slot = gg % NSTAGE;
-          tc::mbar_wait(bar(B_PFULL + b), (gg >> 1) & 1);
-          tc::mbar_wait(bar(B_VFULL + slot), (gg / NSTAGE) & 1);
-          if (j == 0) tc::mbar_wait(bar(B_OFREE + opar), ((itc >> 1) & 1) ^ 1);
+          PROF_WAIT(2, bar(B_PFULL + b), (gg >> 1) & 1);
+          PROF_WAIT(3, bar(B_VFULL + slot), (gg / NSTAGE) & 1);
+          if (j == 0) PROF_WAIT(4, bar(B_OFREE + opar), ((itc >> 1) & 1) ^ 1);
           tc::tc_fence_after();
           // V tile as MN-major B: 64-wide d atoms HALF_BYTES apart (LBO), 8-token groups 1024 B apart (SBO)
           const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, HALF_BYTES, 1024);
@@ -287,6 +317,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         g += n;
         ++itc;
       }
+      PROF_ADD(0);
+      PROF_FLUSH(8, 6);
     }
     __syncwarp();
   } else if (warp < 6) {
@@ -295,6 +327,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     const int row = wq * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
     int g = 0, itc = 0;
+    PROF_DECL(7);
+    PROF_T0();
     for (int k = 0; k * grid < n_items; ++k) {
       const int idx = item_index(k, cta, grid);
       if (idx >= n_items) continue;
@@ -314,7 +348,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       for (int j = it.jt0; j < it.jt1; ++j, ++g) {
         const int b = g & 1;
         const uint32_t tS = tmem + b * TILE_N + lane_addr;
-        tc::mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
+        PROF_WAIT(1, bar(B_SFULL + b), (g >> 1) & 1);
         tc::tc_fence_after();
         const int tok0 = j * TILE_N;
         const bool tail = tok0 + TILE_N > P;  // tile touches tree positions or the ragged end: apply visibility
@@ -331,8 +365,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         // check, so S is still intact for the second pass.
         bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);
         if (!slow) {
+          PROF_SPAN_BEGIN();
           weights_pass(tS, vis, tail, p.scale_log2, -m_used, pk, ts, tr);
           slow = __any_sync(0xffffffffu, !(ts <= WEIGHT_SUM_LIMIT));
+          PROF_SPAN_END(5);
         }
         if (slow) {
           float mx = row_max_pass(tS, vis, tail);
@@ -345,7 +381,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           lsum *= alpha;
           lsum_r *= alpha;
           if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale in TMEM
-            tc::mbar_wait(bar(B_PVDONE), (g - 1) & 1);
+            PROF_WAIT(3, bar(B_PVDONE), (g - 1) & 1);
             tc::tc_fence_after();
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -363,12 +399,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         }
         lsum += ts;
         lsum_r += tail ? tr : ts;
+        PROF_SPAN_BEGIN();
         tc::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
         tc::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
         tc::tmem_wait_st();
         if (tok0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
           const int slot = g % NSTAGE;
-          tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
+          PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
           if (row >= total - tok0) {
             uint4* z0 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + row * 128);
             uint4* z1 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + HALF_BYTES + row * 128);
@@ -379,10 +416,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         }
         tc::tc_fence_before();
         tc::mbar_arrive(bar(B_PFULL + b));
+        PROF_SPAN_END(6);
       }
 
       // ---- epilogue: O / l, lse = ln2 * (m + log2 l) ----
-      tc::mbar_wait(bar(B_OFULL + opar), (itc >> 1) & 1);
+      PROF_WAIT(2, bar(B_OFULL + opar), (itc >> 1) & 1);
       tc::tc_fence_after();
       const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
       const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
@@ -422,6 +460,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       tc::mbar_arrive(bar(B_OFREE + opar));
       ++itc;
     }
+    PROF_ADD(0);
+    if (warp == 2 && lane == 0) PROF_FLUSH(16, 7);
   }
 
   // ---- teardown ----
@@ -504,6 +544,17 @@ EncodeTiledFn get_encode() {
 }
 
 }  // namespace
+
+int debug_wait_prof(unsigned long long* host_out, int n_ctas) {
+#ifdef ECHO_WAIT_PROF
+  if (n_ctas > ECHO_PROF_CTAS) n_ctas = ECHO_PROF_CTAS;
+  return cudaMemcpyFromSymbol(host_out, g_wait_prof, sizeof(unsigned long long) * ECHO_PROF_SLOTS * n_ctas) == cudaSuccess
+             ? n_ctas : ECHO_ERR_CUDA;
+#else
+  (void)host_out; (void)n_ctas;
+  return ECHO_ERR_UNSUPPORTED;
+#endif
+}
 
 int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer, int32_t Hq,
                           int32_t R, const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,

@@ -25,7 +25,7 @@ CUT_NEVER = 0x7FFFFFFF
 DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
-           "echo_device_status", "echo_set_option", "echo_gate_select", "echo_verify_attn", "echo_accept"]
+           "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept"]
 
 
 class EchoTrees(C.Structure):
@@ -90,6 +90,8 @@ def load_library():
     lib.echo_device_status.restype = C.c_int
     lib.echo_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
     lib.echo_set_option.restype = C.c_int
+    lib.echo_debug_wait_prof.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+    lib.echo_debug_wait_prof.restype = C.c_int
     lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
     lib.echo_gate_select.restype = C.c_int
     lib.echo_verify_attn.argtypes = [C.c_void_p, P(EchoSelection), P(EchoPagedKV), C.c_int32, C.c_int32,
@@ -236,6 +238,15 @@ class EchoContext:
         if not hasattr(self, "_opts"):
             self._opts = {}
         self._opts[key] = int(value)
+
+    def debug_wait_prof(self, n_ctas: int = 148):
+        """[n_ctas][32] uint64 wait-cycle counters of the last tcgen05 launch (library built with ECHO_WAIT_PROF=1)."""
+        import numpy as np
+        buf = np.zeros((n_ctas, 32), np.uint64)
+        rc = self.lib.echo_debug_wait_prof(self._h, buf.ctypes.data, n_ctas)
+        if rc < 0:
+            self._check(rc)
+        return buf[:rc]
 
     def device_status(self) -> int:
         f = C.c_uint32(0)
