@@ -24,7 +24,7 @@ size_t echo_workspace_bytes(int32_t R, int32_t N, int32_t capacity, int32_t Hq) 
   size_t keys = align_up((size_t)N * sizeof(uint64_t), 256);
   size_t parts = align_up((size_t)16 * capacity * Hq * (128 + 2) * sizeof(float), 256);
   size_t toks = align_up((size_t)capacity * sizeof(int32_t), 256);
-  size_t plan = align_up((size_t)R * (Hq > 0 ? Hq : 1) * 16 * 16 + 65536, 256);  // <= R*Hkv*row_tiles*16 splits items
+  size_t plan = align_up((size_t)R * (Hq > 0 ? Hq : 1) * 16 * 32 + 65536, 256);  // <= R*Hkv*row_tiles*16 splits items of 32 B
   size_t m = keys > parts ? keys : parts;
   if (toks > m) m = toks;
   return m + plan + 4096;  // partials and plan are used together; keys/tokens alias the partials

@@ -29,10 +29,17 @@ constexpr int PAGE_HALF_BYTES = PAGE * 128;  // one TMA box: 16 rows x 128 B
 constexpr int SMEM_Q = 0;
 constexpr int SMEM_K = SMEM_Q + TILE_BYTES;
 constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
-constexpr int SMEM_BAR = SMEM_V + NSTAGE * TILE_BYTES;
-constexpr int SMEM_TOTAL = SMEM_BAR + 256 + 1024;  // + barriers + slack for 1024-byte alignment
-constexpr int NTHREADS = 224;  // warps: 0 Q+K producer, 1 MMA, 2-5 softmax, 6 V producer
-constexpr int TMEM_COLS = 512;  // S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_b aliases S_b[0,64)
+constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;  // float stats[2 item parities][2][128]: 1 / l_rounded, lse
+constexpr int SMEM_BAR = SMEM_STATS + 2 * 2 * TILE_M * 4;
+constexpr int SMEM_TOTAL = SMEM_BAR + 256;  // dynamic smem is declared 1024-byte aligned: no slack
+// warpgroup 0 (warps 0-3) softmax, warpgroup 1 (warps 4-7) epilogue, warpgroup 2: warp 8 Q+K producer, 9 MMA issuer,
+// 10 V producer, 11 idle (pads the warpgroup so that setmaxnreg applies)
+constexpr int NTHREADS = 384;
+constexpr int W_PROD_K = 8, W_MMA = 9, W_PROD_V = 10;
+constexpr int REGS_SOFTMAX = 248, REGS_EPILOGUE = 120, REGS_AUX = 64;  // 128 * (248 + 120 + 64) <= 64 K registers
+constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
+constexpr int TMEM_O = NSBUF * TILE_N;
+constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 constexpr float WEIGHT_SUM_LIMIT = 4294967296.f;  // a tile whose weight sum exceeds 2^32 is redone against its own maximum
@@ -41,8 +48,8 @@ constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
-enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 16,
-       B_PVDONE = 18, B_OFULL = 19, B_OFREE = 21, B_COUNT = 23 };
+enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
+       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_COUNT = 25 };
 
 struct AttnParams {
   const int4* items;
@@ -70,6 +77,7 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_T0() const long long prof_t0_ = clock64()
 #define PROF_ADD(slot) prof_[slot] += clock64() - prof_t0_
 #define PROF_WAIT(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait(b, ph); prof_[slot] += clock64() - t_; } while (0)
+#define PROF_WAIT_RELAXED(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait_relaxed(b, ph); prof_[slot] += clock64() - t_; } while (0)
 #define PROF_DECL(n) unsigned long long prof_[n] = {}
 #define PROF_FLUSH(base, n) do { if (blockIdx.x < ECHO_PROF_CTAS) for (int q_ = 0; q_ < n; ++q_) g_wait_prof[blockIdx.x][(base) + q_] = prof_[q_]; } while (0)
 #define PROF_SPAN_BEGIN() const long long span_t_ = clock64()
@@ -78,18 +86,22 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_T0() do {} while (0)
 #define PROF_ADD(slot) do {} while (0)
 #define PROF_WAIT(slot, b, ph) tc::mbar_wait(b, ph)
+#define PROF_WAIT_RELAXED(slot, b, ph) tc::mbar_wait_relaxed(b, ph)
 #define PROF_DECL(n) do {} while (0)
 #define PROF_FLUSH(base, n) do {} while (0)
 #define PROF_SPAN_BEGIN() do {} while (0)
 #define PROF_SPAN_END(slot) do {} while (0)
 #endif
 
-struct Item { int req, kvh, rt, split, jt0, jt1; };
-__device__ __forceinline__ Item decode(const int4 v) {
+// work item record written by k_plan: two int4 = {req, kvh | rt<<8 | split<<16, jt0, jt1} {P_i, sel_offsets[i], K_i, 0}
+struct Item { int req, kvh, rt, split, jt0, jt1, P, off, Ki; };
+__device__ __forceinline__ Item decode(const int4 v, const int4 w) {
   Item it;
   it.req = v.x; it.kvh = v.y & 0xff; it.rt = (v.y >> 8) & 0xff; it.split = (v.y >> 16) & 0xff; it.jt0 = v.z; it.jt1 = v.w;
+  it.P = w.x; it.off = w.y; it.Ki = w.z;
   return it;
 }
+__device__ __forceinline__ Item load_item(const int4* items, int idx) { return decode(items[2 * idx], items[2 * idx + 1]); }
 // snake order over the length-sorted work list: round k of CTA c takes k*G+c (k even) or (k+1)*G-1-c (k odd)
 __device__ __forceinline__ int item_index(int k, int cta, int grid) {
   return (k & 1) ? (k + 1) * grid - 1 - cta : k * grid + cta;
@@ -121,8 +133,11 @@ __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
 
 // weights p = 2^(s*scale_log2 + neg_m) for the whole row: packed to bf16 in pk, exact fp32 sum in ts and (tail
 // tiles only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the FMA-pipe work.
-__device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[4], bool tail, float scale_log2,
-                                             float neg_m, uint32_t (&pk)[64], float& ts, float& tr) {
+// TAIL = false (tile entirely inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP / FADD2 with no
+// visibility selects and no rounded sum: 2.5 issue slots per weight.
+template <bool TAIL>
+__device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
+                                             uint32_t (&pk)[64], float& ts, float& tr) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
   float trr[2] = {0.f, 0.f};
@@ -133,7 +148,7 @@ __device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[
     tc::tmem_wait_ld();
     if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
     uint32_t(&sc)[32] = s[c & 1];
-    if (tail) mask_chunk(sc, vis[c]);
+    if (TAIL) mask_chunk(sc, vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2) {
       float x0, x1;
@@ -145,16 +160,16 @@ __device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[
       // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
       // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
       // combination of V rows; lse always uses the exact fp32 sum
-      if (tail) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
+      if (TAIL) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
     }
   }
   float a0, a1;
   tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
   ts = a0 + a1;
-  tr = trr[0] + trr[1];
+  tr = TAIL ? trr[0] + trr[1] : ts;
 }
 
-__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4], bool tail) {
+__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   uint32_t s[2][32];
   tc::tmem_ld32(tS, s[0]);
@@ -163,7 +178,7 @@ __device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)
     tc::tmem_wait_ld();
     if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
     uint32_t(&sc)[32] = s[c & 1];
-    if (tail) mask_chunk(sc, vis[c]);
+    mask_chunk(sc, vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2)
       mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(sc[e]), __uint_as_float(sc[e + 1]));
@@ -175,11 +190,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
                                                                 const __grid_constant__ CUtensorMap tmap_k,
                                                                 const __grid_constant__ CUtensorMap tmap_v,
                                                                 const AttnParams p) {
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t sbase = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t sbase = tc::smem_u32(smem_raw);
   const uint32_t sQ = sbase + SMEM_Q, sK = sbase + SMEM_K, sV = sbase + SMEM_V, sBar = sbase + SMEM_BAR;
-  uint8_t* gen_base = smem_raw + (sbase - tc::smem_u32(smem_raw));  // generic pointer to the aligned base
+  uint8_t* gen_base = smem_raw;
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_BAR + B_COUNT * 8);
+  float* stats = reinterpret_cast<float*>(gen_base + SMEM_STATS);
   auto bar = [&](int i) -> uint32_t { return sBar + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -187,8 +203,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   const int n_items = *p.n_items;
 
   if (threadIdx.x == 0) {
+    if (sbase & 1023u) __trap();  // SW128 operand tiles need 1024-byte alignment
     for (int i = 0; i < B_COUNT; ++i) {
-      const uint32_t cnt = (i == B_PFULL || i == B_PFULL + 1 || i == B_OFREE || i == B_OFREE + 1) ? 128u : 1u;
+      const uint32_t cnt = ((i >= B_PFULL && i < B_PFULL + NSBUF) || i == B_OFREE || i == B_STATS || i == B_STATS + 1)
+                               ? 128u : 1u;
       tc::mbar_init(bar(i), cnt);
     }
     tc::fence_barrier_init();
@@ -196,34 +214,37 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     tc::prefetch_tmap(&tmap_k);
     tc::prefetch_tmap(&tmap_v);
   }
-  if (warp == 1) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
+  if (warp == W_MMA) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  if (warp == 0 || warp == 6) {
-    // ============================== TMA producers: warp 0 = Q + K, warp 6 = V (one lane each) ==============
+  if (warp >= 8) tc::setmaxnreg_dec<REGS_AUX>();
+  if (warp == W_PROD_K || warp == W_PROD_V) {
+    // ============================== TMA producers: Q + K ring, V ring (one lane each) ==============
     // The whole loop runs in one thread so that every TMA operand is warp-uniform by construction; page ids
     // of tile j+1 are fetched while tile j is being issued, so no dependent global load sits between tiles.
     if (lane == 0) {
-      const bool is_k = warp == 0;
+      const bool is_k = warp == W_PROD_K;
       const uint32_t s_dst = is_k ? sK : sV;
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
       int g = 0, itc = 0;
       PROF_DECL(3);
       PROF_T0();
-      for (int k = 0; k * grid < n_items; ++k) {
-        const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) continue;
-        const Item it = decode(p.items[idx]);
-        const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
-        const int total = P + (p.sel_offsets[it.req + 1] - off);
+      Item nx = {};
+      bool more = item_index(0, cta, grid) < n_items;  // item indices grow with k
+      if (more) nx = load_item(p.items, item_index(0, cta, grid));
+      for (int k = 1; more; ++k) {
+        const Item it = nx;
+        more = item_index(k, cta, grid) < n_items;
+        if (more) nx = load_item(p.items, item_index(k, cta, grid));
+        const int total = it.P + it.Ki;
         if (is_k) {
           PROF_WAIT(2, bar(B_QEMPTY), (itc & 1) ^ 1);
           tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
-          const int node0 = off + it.rt * (TILE_M >> p.log2G);
+          const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
           tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
           tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
         }
@@ -265,7 +286,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 #endif
     }
     __syncwarp();
-  } else if (warp == 1) {
+  } else if (warp == W_MMA) {
     // ============================== MMA issuer (one lane) ==============================
     if (lane == 0) {
       int g = 0, itc = 0;
@@ -273,7 +294,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       PROF_T0();
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
       auto issue_qk = [&](int gg) {
-        const int slot = gg % NSTAGE, b = gg & 1;
+        const int slot = gg % NSTAGE, b = gg % NSBUF;
         PROF_WAIT(1, bar(B_KFULL + slot), (gg / NSTAGE) & 1);
         tc::tc_fence_after();
         const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, 1024);
@@ -285,25 +306,28 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         tc::mma_commit(bar(B_SFULL + b));
         tc::mma_commit(bar(B_KEMPTY + slot));
       };
-      for (int k = 0; k * grid < n_items; ++k) {
+      for (int k = 0;; ++k) {
         const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) continue;
-        const Item it = decode(p.items[idx]);
-        const int n = it.jt1 - it.jt0, opar = itc & 1;
-        const uint32_t tO = tmem + 2 * TILE_N + opar * D;
+        if (idx >= n_items) break;  // item indices grow with k
+        const int4 rec = p.items[2 * idx];
+        const int n = rec.w - rec.z;
+        const uint32_t tO = tmem + TMEM_O;
         PROF_WAIT(5, bar(B_QFULL), itc & 1);
         tc::tc_fence_after();
-        issue_qk(g);
-        if (n == 1) tc::mma_commit(bar(B_QEMPTY));
+        // the QK^T products run NSBUF-1 tiles ahead of the PV products
+        for (int a = 0; a < NSBUF - 1 && a < n; ++a) {
+          issue_qk(g + a);
+          if (a + 1 == n) tc::mma_commit(bar(B_QEMPTY));
+        }
         for (int j = 0; j < n; ++j) {
-          if (j + 1 < n) {
-            issue_qk(g + j + 1);
-            if (j + 2 == n) tc::mma_commit(bar(B_QEMPTY));
+          if (j + NSBUF - 1 < n) {
+            issue_qk(g + j + NSBUF - 1);
+            if (j + NSBUF == n) tc::mma_commit(bar(B_QEMPTY));
           }
-          const int gg = g + j, b = gg & 1, slot = gg % NSTAGE;
-          PROF_WAIT(2, bar(B_PFULL + b), (gg >> 1) & 1);
+          const int gg = g + j, b = gg % NSBUF, slot = gg % NSTAGE;
+          PROF_WAIT(2, bar(B_PFULL + b), (gg / NSBUF) & 1);
           PROF_WAIT(3, bar(B_VFULL + slot), (gg / NSTAGE) & 1);
-          if (j == 0) PROF_WAIT(4, bar(B_OFREE + opar), ((itc >> 1) & 1) ^ 1);
+          if (j == 0) PROF_WAIT(4, bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
           tc::tc_fence_after();
           // V tile as MN-major B: 64-wide d atoms HALF_BYTES apart (LBO), 8-token groups 1024 B apart (SBO)
           const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, HALF_BYTES, 1024);
@@ -312,7 +336,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             tc::mma_ts(tO, tmem + b * TILE_N + kk * 8, vdesc + ((kk * 2048) >> 4), IDESC_PV, (j > 0) || (kk > 0));
           tc::mma_commit(bar(B_VEMPTY + slot));
           tc::mma_commit(bar(B_PVDONE));
-          if (j == n - 1) tc::mma_commit(bar(B_OFULL + opar));
+          if (j == n - 1) tc::mma_commit(bar(B_OFULL));
         }
         g += n;
         ++itc;
@@ -321,34 +345,44 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       PROF_FLUSH(8, 6);
     }
     __syncwarp();
-  } else if (warp < 6) {
-    // ============================== softmax + epilogue (4 warps, thread = row) ==============================
+  } else if (warp < 4) {
+    // ============================== softmax (warpgroup 0, thread = row) ==============================
+    tc::setmaxnreg_inc<REGS_SOFTMAX>();
     const int wq = warp & 3;  // TMEM lane quarter this warp may access
     const int row = wq * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
     int g = 0, itc = 0;
     PROF_DECL(7);
     PROF_T0();
-    for (int k = 0; k * grid < n_items; ++k) {
-      const int idx = item_index(k, cta, grid);
-      if (idx >= n_items) continue;
-      const Item it = decode(p.items[idx]);
-      const int P = p.prefix_len[it.req], off = p.sel_offsets[it.req];
-      const int Ki = p.sel_offsets[it.req + 1] - off;
-      const int total = P + Ki;
-      const int r_glob = it.rt * TILE_M + row;
-      const int l = r_glob >> p.log2G, gq = r_glob & (p.G - 1);
-      const bool valid = l < Ki;
-      uint4 mk = make_uint4(0u, 0u, 0u, 0u);
-      if (valid) mk = p.anc_mask[off + l];
+    // Item records are fetched two items ahead and the row's ancestor mask one item ahead, so that no global-load
+    // latency sits between the last tile of one item and the first tile of the next.
+    auto row_mask = [&](const int4& r0, const int4& r1) -> uint4 {
+      const int l = ((((r0.y >> 8) & 0xff) * TILE_M + row) >> p.log2G);
+      return l < r1.z ? p.anc_mask[r1.y + l] : make_uint4(0u, 0u, 0u, 0u);
+    };
+    const int4 zero4 = make_int4(0, 0, 0, 0);
+    int4 a0 = zero4, a1 = zero4, b0 = zero4, b1 = zero4;  // records of the next item (a) and the one after (b)
+    uint4 mk_next = make_uint4(0u, 0u, 0u, 0u);
+    bool more = item_index(0, cta, grid) < n_items;
+    if (more) { a0 = p.items[2 * item_index(0, cta, grid)]; a1 = p.items[2 * item_index(0, cta, grid) + 1]; }
+    if (item_index(1, cta, grid) < n_items) { b0 = p.items[2 * item_index(1, cta, grid)]; b1 = p.items[2 * item_index(1, cta, grid) + 1]; }
+    if (more) mk_next = row_mask(a0, a1);
+    for (int k = 0; more; ++k) {
+      const Item it = decode(a0, a1);
+      const uint4 mk = mk_next;
+      more = item_index(k + 1, cta, grid) < n_items;
+      a0 = b0; a1 = b1;
+      if (item_index(k + 2, cta, grid) < n_items) { b0 = p.items[2 * item_index(k + 2, cta, grid)]; b1 = p.items[2 * item_index(k + 2, cta, grid) + 1]; }
+      if (more) mk_next = row_mask(a0, a1);
+      const int P = it.P, total = it.P + it.Ki;
       float m_used = -INFINITY, lsum = 0.f, lsum_r = 0.f;
       const int opar = itc & 1;
-      const uint32_t tO = tmem + 2 * TILE_N + opar * D + lane_addr;
+      const uint32_t tO = tmem + TMEM_O + lane_addr;
 
       for (int j = it.jt0; j < it.jt1; ++j, ++g) {
-        const int b = g & 1;
+        const int b = g % NSBUF;
         const uint32_t tS = tmem + b * TILE_N + lane_addr;
-        PROF_WAIT(1, bar(B_SFULL + b), (g >> 1) & 1);
+        PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
         tc::tc_fence_after();
         const int tok0 = j * TILE_N;
         const bool tail = tok0 + TILE_N > P;  // tile touches tree positions or the ragged end: apply visibility
@@ -366,12 +400,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);
         if (!slow) {
           PROF_SPAN_BEGIN();
-          weights_pass(tS, vis, tail, p.scale_log2, -m_used, pk, ts, tr);
+          if (tail) weights_pass<true>(tS, vis, p.scale_log2, -m_used, pk, ts, tr);
+          else weights_pass<false>(tS, vis, p.scale_log2, -m_used, pk, ts, tr);
           slow = __any_sync(0xffffffffu, !(ts <= WEIGHT_SUM_LIMIT));
           PROF_SPAN_END(5);
         }
         if (slow) {
-          float mx = row_max_pass(tS, vis, tail);
+          float mx = row_max_pass(tS, vis);
           const float m_new = fmaxf(m_used, mx * p.scale_log2);
           float alpha = 1.f;
           if (m_new > m_used) {
@@ -395,10 +430,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             tc::tmem_wait_st();
           }
           const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-          weights_pass(tS, vis, tail, p.scale_log2, -m_eff, pk, ts, tr);
+          weights_pass<true>(tS, vis, p.scale_log2, -m_eff, pk, ts, tr);  // vis is all ones off the tail
         }
         lsum += ts;
-        lsum_r += tail ? tr : ts;
+        lsum_r += tr;
         PROF_SPAN_BEGIN();
         tc::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
         tc::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
@@ -419,36 +454,71 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         PROF_SPAN_END(6);
       }
 
-      // ---- epilogue: O / l, lse = ln2 * (m + log2 l) ----
-      PROF_WAIT(2, bar(B_OFULL + opar), (itc >> 1) & 1);
+      // ---- hand 1 / l_rounded and lse = ln2 * (m + log2 l) to the epilogue warpgroup ----
+      {
+        const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
+        const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+        const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
+        tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of item itc-1 is done, so statistics buffer opar is free
+        stats[(opar * 2 + 0) * TILE_M + row] = inv;
+        stats[(opar * 2 + 1) * TILE_M + row] = lse_v;
+        tc::mbar_arrive(bar(B_STATS + opar));
+      }
+      ++itc;
+    }
+    PROF_ADD(0);
+    if (warp == 0 && lane == 0) PROF_FLUSH(16, 7);
+  } else if (warp < 8) {
+    // ============================== epilogue (warpgroup 1, thread = row) ==============================
+    // O of item n is normalised and stored here while the softmax warpgroup is already on item n+1 (O and the
+    // statistics are double buffered by item parity).
+    tc::setmaxnreg_dec<REGS_EPILOGUE>();
+    const int wq = warp & 3;
+    const int row = wq * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
+    int itc = 0;
+    PROF_DECL(3);
+    PROF_T0();
+    for (int k = 0;; ++k) {
+      const int idx = item_index(k, cta, grid);
+      if (idx >= n_items) break;
+      const Item it = load_item(p.items, idx);
+      const int r_glob = it.rt * TILE_M + row;
+      const int l = r_glob >> p.log2G, gq = r_glob & (p.G - 1);
+      const bool valid = l < it.Ki;
+      const int opar = itc & 1;
+      const uint32_t tO = tmem + TMEM_O + lane_addr;
+      const size_t rowg = (size_t)(it.off + l) * p.Hq + it.kvh * p.G + gq;
+      PROF_WAIT_RELAXED(1, bar(B_STATS + opar), (itc >> 1) & 1);
+      const float inv = stats[(opar * 2 + 0) * TILE_M + row];
+      const float lse_v = stats[(opar * 2 + 1) * TILE_M + row];
+      PROF_WAIT(2, bar(B_OFULL), itc & 1);
       tc::tc_fence_after();
-      const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
-      const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-      const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
-      const size_t rowg = (size_t)(off + l) * p.Hq + it.kvh * p.G + gq;
+      uint32_t o[2][32];
+      tc::tmem_ld32(tO, o[0]);
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        uint32_t o[32];
-        tc::tmem_ld32(tO + c * 32, o);
         tc::tmem_wait_ld();
+        if (c < 3) tc::tmem_ld32(tO + (c + 1) * 32, o[(c + 1) & 1]);
+        uint32_t(&oc)[32] = o[c & 1];
         if (valid) {
           if (p.splits == 1) {
             uint4* dst = reinterpret_cast<uint4*>(p.out + rowg * D + c * 32);
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
               uint4 w;
-              w.x = tc::pack_bf16(__uint_as_float(o[8 * e + 0]) * inv, __uint_as_float(o[8 * e + 1]) * inv);
-              w.y = tc::pack_bf16(__uint_as_float(o[8 * e + 2]) * inv, __uint_as_float(o[8 * e + 3]) * inv);
-              w.z = tc::pack_bf16(__uint_as_float(o[8 * e + 4]) * inv, __uint_as_float(o[8 * e + 5]) * inv);
-              w.w = tc::pack_bf16(__uint_as_float(o[8 * e + 6]) * inv, __uint_as_float(o[8 * e + 7]) * inv);
+              w.x = tc::pack_bf16(__uint_as_float(oc[8 * e + 0]) * inv, __uint_as_float(oc[8 * e + 1]) * inv);
+              w.y = tc::pack_bf16(__uint_as_float(oc[8 * e + 2]) * inv, __uint_as_float(oc[8 * e + 3]) * inv);
+              w.z = tc::pack_bf16(__uint_as_float(oc[8 * e + 4]) * inv, __uint_as_float(oc[8 * e + 5]) * inv);
+              w.w = tc::pack_bf16(__uint_as_float(oc[8 * e + 6]) * inv, __uint_as_float(oc[8 * e + 7]) * inv);
               dst[e] = w;
             }
           } else {
             float4* dst = reinterpret_cast<float4*>(p.part_o + ((size_t)it.split * p.n_rows_cap + rowg) * D + c * 32);
 #pragma unroll
             for (int e = 0; e < 8; ++e)
-              dst[e] = make_float4(__uint_as_float(o[4 * e + 0]) * inv, __uint_as_float(o[4 * e + 1]) * inv,
-                                   __uint_as_float(o[4 * e + 2]) * inv, __uint_as_float(o[4 * e + 3]) * inv);
+              dst[e] = make_float4(__uint_as_float(oc[4 * e + 0]) * inv, __uint_as_float(oc[4 * e + 1]) * inv,
+                                   __uint_as_float(oc[4 * e + 2]) * inv, __uint_as_float(oc[4 * e + 3]) * inv);
           }
         }
       }
@@ -457,17 +527,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         else p.part_lse[(size_t)it.split * p.n_rows_cap + rowg] = lse_v;
       }
       tc::tc_fence_before();
-      tc::mbar_arrive(bar(B_OFREE + opar));
+      tc::mbar_arrive(bar(B_OFREE));
       ++itc;
     }
     PROF_ADD(0);
-    if (warp == 2 && lane == 0) PROF_FLUSH(16, 7);
+    if (warp == 4 && lane == 0) PROF_FLUSH(24, 3);
   }
 
   // ---- teardown ----
   tc::tc_fence_before();
   __syncthreads();
-  if (warp == 1) tc::tmem_dealloc(tmem, TMEM_COLS);
+  if (warp == W_MMA) tc::tmem_dealloc(tmem, TMEM_COLS);
 }
 
 // Device-side planner: P_i and K_i exist only on the device, so the work list is built there.
@@ -485,18 +555,18 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
   __syncthreads();
   auto for_items = [&](auto&& fn) {
     for (int r = tid; r < R; r += PLAN_THREADS) {
-      const int Ki = sel_offsets[r + 1] - sel_offsets[r];
+      const int off = sel_offsets[r], Ki = sel_offsets[r + 1] - off, P = prefix_len[r];
       if (Ki <= 0) continue;
-      const int n_tiles = (prefix_len[r] + Ki + TILE_N - 1) / TILE_N;
+      const int n_tiles = (P + Ki + TILE_N - 1) / TILE_N;
       const int n_rt = (Ki * G + TILE_M - 1) / TILE_M;
       const int tps = (n_tiles + splits - 1) / splits;
       for (int s = 0; s * tps < n_tiles; ++s) {
         const int j0 = s * tps, j1 = min(n_tiles, j0 + tps);
-        fn(r, s, j0, j1, n_rt);
+        fn(r, s, j0, j1, n_rt, P, off, Ki);
       }
     }
   };
-  for_items([&](int, int, int j0, int j1, int n_rt) {
+  for_items([&](int, int, int j0, int j1, int n_rt, int, int, int) {
     atomicAdd(&s_cnt[PLAN_BUCKETS - 1 - min(j1 - j0, PLAN_BUCKETS - 1)], Hkv * n_rt);
   });
   __syncthreads();
@@ -519,12 +589,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
     if (tid == PLAN_THREADS - 1) *n_items = min(run, max_items);
   }
   __syncthreads();
-  for_items([&](int r, int s, int j0, int j1, int n_rt) {
+  for_items([&](int r, int s, int j0, int j1, int n_rt, int P, int off, int Ki) {
     const int pos0 = atomicAdd(&s_cnt[PLAN_BUCKETS - 1 - min(j1 - j0, PLAN_BUCKETS - 1)], Hkv * n_rt);
     int pos = pos0;
     for (int kvh = 0; kvh < Hkv; ++kvh)
       for (int rt = 0; rt < n_rt; ++rt, ++pos)
-        if (pos < max_items) items[pos] = make_int4(r, kvh | (rt << 8) | (s << 16), j0, j1);
+        if (pos < max_items) {
+          items[2 * pos] = make_int4(r, kvh | (rt << 8) | (s << 16), j0, j1);
+          items[2 * pos + 1] = make_int4(P, off, Ki, 0);
+        }
   });
 }
 
@@ -602,7 +675,7 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   const size_t part_bytes = splits > 1 ? align_up((size_t)splits * n_rows * (D + 1) * sizeof(float), 256) : 0;
   const int max_rt = (int)(((size_t)(cap < ECHO_MAX_CAND ? cap : ECHO_MAX_CAND) * G + TILE_M - 1) / TILE_M);
   const size_t max_items = (size_t)R * Hkv * max_rt * splits;
-  const size_t plan_bytes = 256 + max_items * sizeof(int4);
+  const size_t plan_bytes = 256 + max_items * 2 * sizeof(int4);
   if (part_bytes + plan_bytes > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
   uint8_t* plan = reinterpret_cast<uint8_t*>(ctx->workspace) + part_bytes;
   int32_t* n_items = reinterpret_cast<int32_t*>(plan);
