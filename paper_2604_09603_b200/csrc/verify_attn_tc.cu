@@ -23,20 +23,23 @@ constexpr int PAGE = 16;
 constexpr int TILE_M = 128;
 constexpr int TILE_N = 128;
 constexpr int NSTAGE = 3;
-constexpr int HALF_BYTES = TILE_N * 128;     // [128 rows][64 bf16], 128-byte rows, SW128
+constexpr int HALF_BYTES = TILE_N * 128;     // Q tile: [128 rows][64 bf16] per d-half, 128-byte rows, SW128
 constexpr int TILE_BYTES = 2 * HALF_BYTES;   // both d-halves: 32 KB
-constexpr int PAGE_HALF_BYTES = PAGE * 128;  // one TMA box: 16 rows x 128 B
+constexpr int PAGE_BYTES = PAGE * D * 2;  // one TMA box: [2 token groups][2 d-halves][8 tokens][64 d], 4 KB
+constexpr int GROUP_BYTES = 2048;         // 8 tokens x 128 d: d-half 0 (1 KB SW128 atom), then d-half 1
 constexpr int SMEM_Q = 0;
 constexpr int SMEM_K = SMEM_Q + TILE_BYTES;
 constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
-constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;  // float stats[2 item parities][2][128]: 1 / l_rounded, lse
-constexpr int SMEM_BAR = SMEM_STATS + 2 * 2 * TILE_M * 4;
+constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;  // float stats[2][128]: 1 / l_rounded, lse of the item just finished
+constexpr int SMEM_XCHG = SMEM_STATS + 2 * TILE_M * 4;  // float xchg[2 warpgroups][128]: half-row maxima / sums
+constexpr int SMEM_BAR = SMEM_XCHG + 2 * TILE_M * 4;
 constexpr int SMEM_TOTAL = SMEM_BAR + 256;  // dynamic smem is declared 1024-byte aligned: no slack
-// warpgroup 0 (warps 0-3) softmax, warpgroup 1 (warps 4-7) epilogue, warpgroup 2: warp 8 Q+K producer, 9 MMA issuer,
-// 10 V producer, 11 idle (pads the warpgroup so that setmaxnreg applies)
-constexpr int NTHREADS = 384;
-constexpr int W_PROD_K = 8, W_MMA = 9, W_PROD_V = 10;
-constexpr int REGS_SOFTMAX = 248, REGS_EPILOGUE = 120, REGS_AUX = 64;  // 128 * (248 + 120 + 64) <= 64 K registers
+// warpgroups 0 and 1 (warps 0-3, 4-7) softmax: warpgroup w takes columns [64 w, 64 w + 64) of every S row, so each
+// SM sub-partition has two softmax warps to issue from; warpgroup 2 (warps 8-11) epilogue; warpgroup 3: warp 12 Q+K
+// producer, 13 QK^T MMA issuer, 14 V producer, 15 PV MMA issuer
+constexpr int NTHREADS = 640;
+constexpr int W_EPI = 8, W_PROD_K0 = 12, W_MMA_QK = 13, W_PROD_V0 = 14, W_MMA_PV = 15, W_PROD_K1 = 16, W_PROD_V1 = 17;
+constexpr int REGS_SOFTMAX = 160, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 160 + 80 + 2 * 40) = 640 * 96, the launch allocation
 constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
 constexpr int TMEM_O = NSBUF * TILE_N;
 constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
@@ -49,7 +52,7 @@ constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
 enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
-       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_COUNT = 25 };
+       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_SFREE = 24, B_COUNT = 27 };
 
 struct AttnParams {
   const int4* items;
@@ -123,31 +126,32 @@ __device__ __forceinline__ uint32_t visible_word(const uint4& m, int P, int t0) 
   return bits;
 }
 
-// ---- softmax passes over one S row (thread = row, 128 fp32 columns in TMEM), 32 columns per tcgen05.ld, the
-// load of chunk c+1 in flight while chunk c is processed ----
+// ---- softmax passes over this thread's half of an S row (64 fp32 columns in TMEM), two 32-column tcgen05.ld, the
+// second in flight while the first is processed ----
 __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
 #pragma unroll
   for (int e = 0; e < 32; ++e)
     if (!((vis >> e) & 1u)) s[e] = 0xff800000u;  // -inf
 }
 
-// weights p = 2^(s*scale_log2 + neg_m) for the whole row: packed to bf16 in pk, exact fp32 sum in ts and (tail
-// tiles only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the FMA-pipe work.
-// TAIL = false (tile entirely inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP / FADD2 with no
+// weights p = 2^(s*scale_log2 + neg_m) for 64 columns: packed to bf16 in pk, exact fp32 sum in ts and (tail tiles
+// only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the issue slots.
+// TAIL = false (all 64 keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP / FADD2 with no
 // visibility selects and no rounded sum: 2.5 issue slots per weight.
 template <bool TAIL>
-__device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
-                                             uint32_t (&pk)[64], float& ts, float& tr) {
+__device__ __forceinline__ void weights_pass(uint32_t tSh, const uint32_t (&vis)[2], float scale_log2, float neg_m,
+                                             uint32_t (&pk)[32], float& ts, float& tr) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
   float trr[2] = {0.f, 0.f};
   uint32_t s[2][32];
-  tc::tmem_ld32(tS, s[0]);
+  tc::tmem_ld32(tSh, s[0]);
+  tc::tmem_wait_ld();
+  tc::tmem_ld32(tSh + 32, s[1]);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    tc::tmem_wait_ld();
-    if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
-    uint32_t(&sc)[32] = s[c & 1];
+  for (int c = 0; c < 2; ++c) {
+    if (c == 1) tc::tmem_wait_ld();
+    uint32_t(&sc)[32] = s[c];
     if (TAIL) mask_chunk(sc, vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2) {
@@ -169,21 +173,36 @@ __device__ __forceinline__ void weights_pass(uint32_t tS, const uint32_t (&vis)[
   tr = TAIL ? trr[0] + trr[1] : ts;
 }
 
-__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
+__device__ __forceinline__ float row_max_pass(uint32_t tSh, const uint32_t (&vis)[2]) {
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   uint32_t s[2][32];
-  tc::tmem_ld32(tS, s[0]);
+  tc::tmem_ld32(tSh, s[0]);
+  tc::tmem_ld32(tSh + 32, s[1]);
+  tc::tmem_wait_ld();
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    tc::tmem_wait_ld();
-    if (c < 3) tc::tmem_ld32(tS + (c + 1) * 32, s[(c + 1) & 1]);
-    uint32_t(&sc)[32] = s[c & 1];
-    mask_chunk(sc, vis[c]);
+  for (int c = 0; c < 2; ++c) {
+    mask_chunk(s[c], vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2)
-      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(sc[e]), __uint_as_float(sc[e + 1]));
+      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c][e]), __uint_as_float(s[c][e + 1]));
   }
   return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+}
+
+// named barrier over the two warps that share a TMEM lane quarter (one per softmax warpgroup), ids 1-4
+__device__ __forceinline__ bool pair_or(int quarter, bool pred) {
+  uint32_t r;
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\t"
+      "barrier.cta.red.or.pred q, %2, 64, p;\n\t"
+      "selp.u32 %0, 1, 0, q;\n\t}"
+      : "=r"(r)
+      : "r"((uint32_t)pred), "r"(quarter + 1)
+      : "memory");
+  return r != 0;
+}
+__device__ __forceinline__ void pair_sync(int quarter) {
+  asm volatile("barrier.cta.sync %0, 64;" ::"r"(quarter + 1) : "memory");
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_constant__ CUtensorMap tmap_q,
@@ -196,6 +215,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   uint8_t* gen_base = smem_raw;
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_BAR + B_COUNT * 8);
   float* stats = reinterpret_cast<float*>(gen_base + SMEM_STATS);
+  float* xchg = reinterpret_cast<float*>(gen_base + SMEM_XCHG);
   auto bar = [&](int i) -> uint32_t { return sBar + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -205,8 +225,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();  // SW128 operand tiles need 1024-byte alignment
     for (int i = 0; i < B_COUNT; ++i) {
-      const uint32_t cnt = ((i >= B_PFULL && i < B_PFULL + NSBUF) || i == B_OFREE || i == B_STATS || i == B_STATS + 1)
-                               ? 128u : 1u;
+      const uint32_t cnt = (i >= B_KFULL && i < B_KFULL + NSTAGE) || (i >= B_VFULL && i < B_VFULL + NSTAGE) ? 2u
+                           : (i >= B_PFULL && i < B_PFULL + NSBUF) ? 8u  /* one arrival per softmax warp */
+                           : (i == B_OFREE || i == B_STATS) ? 128u : 1u;
       tc::mbar_init(bar(i), cnt);
     }
     tc::fence_barrier_init();
@@ -214,19 +235,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     tc::prefetch_tmap(&tmap_k);
     tc::prefetch_tmap(&tmap_v);
   }
-  if (warp == W_MMA) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
+  if (warp == W_MMA_QK) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  if (warp >= 8) tc::setmaxnreg_dec<REGS_AUX>();
-  if (warp == W_PROD_K || warp == W_PROD_V) {
-    // ============================== TMA producers: Q + K ring, V ring (one lane each) ==============
-    // The whole loop runs in one thread so that every TMA operand is warp-uniform by construction; page ids
-    // of tile j+1 are fetched while tile j is being issued, so no dependent global load sits between tiles.
+  if (warp >= 12) tc::setmaxnreg_dec<REGS_AUX>();
+  if (warp == W_PROD_K0 || warp == W_PROD_V0 || warp == W_PROD_K1 || warp == W_PROD_V1) {
+    // ============================== TMA producers: Q + K ring, V ring ==============================
+    // One cp.async.bulk.tensor costs its issuing thread 110-170 cycles whatever the box size (measured), so a page
+    // (16 tokens x 128 d of one KV head, 4 KB contiguous in the pool) is one 4-D box {64 d, 8 tokens, 2 d-halves,
+    // 2 token groups} and each ring has two issuing threads in different warps: thread h takes pages 4h..4h+3 of
+    // every 128-token tile.  The whole loop runs in one lane so that every TMA operand is warp-uniform; page ids of
+    // tile j+1 are fetched while tile j is being issued.
     if (lane == 0) {
-      const bool is_k = warp == W_PROD_K;
+      const bool is_k = warp == W_PROD_K0 || warp == W_PROD_K1;
+      const int half = (warp == W_PROD_K1 || warp == W_PROD_V1) ? 1 : 0;
+      const bool loads_q = warp == W_PROD_K0;
       const uint32_t s_dst = is_k ? sK : sV;
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
@@ -241,7 +267,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         more = item_index(k, cta, grid) < n_items;
         if (more) nx = load_item(p.items, item_index(k, cta, grid));
         const int total = it.P + it.Ki;
-        if (is_k) {
+        if (loads_q) {
           PROF_WAIT(2, bar(B_QEMPTY), (itc & 1) ^ 1);
           tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
           const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
@@ -251,106 +277,126 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
         int npages = (total + PAGE - 1) / PAGE;
         if (npages > p.max_pages) {  // page table too short: flag, load what exists
-          if (is_k) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
+          if (loads_q) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
           npages = p.max_pages;
         }
-        int cur[8], nxt[8];
+        int cur[4], nxt[4];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) cur[e] = (it.jt0 * 8 + e < npages) ? pt[it.jt0 * 8 + e] : 0;
+        for (int e = 0; e < 4; ++e) {
+          const int pi = it.jt0 * 8 + half * 4 + e;
+          cur[e] = pi < npages ? pt[pi] : 0;
+        }
         for (int j = it.jt0; j < it.jt1; ++j, ++g) {
 #pragma unroll
-          for (int e = 0; e < 8; ++e) nxt[e] = (j + 1 < it.jt1 && (j + 1) * 8 + e < npages) ? pt[(j + 1) * 8 + e] : 0;
+          for (int e = 0; e < 4; ++e) {
+            const int pi = (j + 1) * 8 + half * 4 + e;
+            nxt[e] = (j + 1 < it.jt1 && pi < npages) ? pt[pi] : 0;
+          }
           const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
-          const int npv = max(0, min(8, npages - j * 8));  // pages of this tile that hold tokens
-          const uint32_t dst = s_dst + slot * TILE_BYTES;
+          const int npv = max(0, min(4, npages - j * 8 - half * 4));  // my pages of this tile that hold tokens
+          const uint32_t dst = s_dst + slot * TILE_BYTES + half * 4 * PAGE_BYTES;
           const uint32_t fb = bar(b_full + slot);
           PROF_WAIT(1, bar(b_empty + slot), ph ^ 1);
-          tc::mbar_expect_tx(fb, npv * 2 * PAGE_HALF_BYTES);
+          tc::mbar_expect_tx(fb, npv * PAGE_BYTES);
 #pragma unroll
-          for (int e = 0; e < 8; ++e) {
+          for (int e = 0; e < 4; ++e) {
             if (e < npv) {
-              const int row = ((p.page_row_base + cur[e]) * p.Hkv + it.kvh) * PAGE;
-              tc::tma_load_2d(dst + e * PAGE_HALF_BYTES, tmap, fb, 0, row);
-              tc::tma_load_2d(dst + HALF_BYTES + e * PAGE_HALF_BYTES, tmap, fb, 64, row);
+              const int grp = ((p.page_row_base + cur[e]) * p.Hkv + it.kvh) * (PAGE / 8);  // 8-token group index
+              tc::tma_load_4d(dst + e * PAGE_BYTES, tmap, fb, 0, 0, 0, grp);
             }
           }
 #pragma unroll
-          for (int e = 0; e < 8; ++e) cur[e] = nxt[e];
+          for (int e = 0; e < 4; ++e) cur[e] = nxt[e];
         }
         ++itc;
       }
       PROF_ADD(0);
-      PROF_FLUSH(is_k ? 0 : 4, 3);
-#ifdef ECHO_WAIT_PROF
-      g_wait_prof[blockIdx.x][is_k ? 3 : 7] = g;
-#endif
+      if (half == 0) PROF_FLUSH(is_k ? 0 : 4, 3);
     }
     __syncwarp();
-  } else if (warp == W_MMA) {
-    // ============================== MMA issuer (one lane) ==============================
+  } else if (warp == W_MMA_QK) {
+    // ============================== MMA issuer for S = Q K^T (one lane) ==============================
+    // Two issuing threads, one per product: a single thread retires a 128x128x16 tcgen05.mma only every ~110
+    // cycles, two threads keep the tensor pipe at 70-85 cycles per instruction (measured).  This thread runs up to
+    // NSBUF tiles ahead of the PV issuer; S/P buffer b is handed back through B_SFREE when the PV that read P_b is done.
     if (lane == 0) {
       int g = 0, itc = 0;
       PROF_DECL(6);
       PROF_T0();
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
-      auto issue_qk = [&](int gg) {
-        const int slot = gg % NSTAGE, b = gg % NSBUF;
-        PROF_WAIT(1, bar(B_KFULL + slot), (gg / NSTAGE) & 1);
-        tc::tc_fence_after();
-        const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, 1024);
-#pragma unroll
-        for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t o16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
-          tc::mma_ss(tmem + b * TILE_N, qdesc + o16, kdesc + o16, IDESC_QK, kk > 0);
-        }
-        tc::mma_commit(bar(B_SFULL + b));
-        tc::mma_commit(bar(B_KEMPTY + slot));
-      };
       for (int k = 0;; ++k) {
         const int idx = item_index(k, cta, grid);
         if (idx >= n_items) break;  // item indices grow with k
         const int4 rec = p.items[2 * idx];
         const int n = rec.w - rec.z;
-        const uint32_t tO = tmem + TMEM_O;
         PROF_WAIT(5, bar(B_QFULL), itc & 1);
-        tc::tc_fence_after();
-        // the QK^T products run NSBUF-1 tiles ahead of the PV products
-        for (int a = 0; a < NSBUF - 1 && a < n; ++a) {
-          issue_qk(g + a);
-          if (a + 1 == n) tc::mma_commit(bar(B_QEMPTY));
-        }
-        for (int j = 0; j < n; ++j) {
-          if (j + NSBUF - 1 < n) {
-            issue_qk(g + j + NSBUF - 1);
-            if (j + NSBUF == n) tc::mma_commit(bar(B_QEMPTY));
-          }
-          const int gg = g + j, b = gg % NSBUF, slot = gg % NSTAGE;
-          PROF_WAIT(2, bar(B_PFULL + b), (gg / NSBUF) & 1);
-          PROF_WAIT(3, bar(B_VFULL + slot), (gg / NSTAGE) & 1);
-          if (j == 0) PROF_WAIT(4, bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
+        for (int j = 0; j < n; ++j, ++g) {
+          const int slot = g % NSTAGE, b = g % NSBUF;
+          PROF_WAIT(1, bar(B_KFULL + slot), (g / NSTAGE) & 1);
+          PROF_WAIT(2, bar(B_SFREE + b), ((g / NSBUF) & 1) ^ 1);  // PV of tile g - NSBUF has read P_b
           tc::tc_fence_after();
-          // V tile as MN-major B: 64-wide d atoms HALF_BYTES apart (LBO), 8-token groups 1024 B apart (SBO)
-          const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, HALF_BYTES, 1024);
+          // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half h at +1 KB inside a group
+          const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, GROUP_BYTES);
 #pragma unroll
-          for (int kk = 0; kk < TILE_N / 16; ++kk)
-            tc::mma_ts(tO, tmem + b * TILE_N + kk * 8, vdesc + ((kk * 2048) >> 4), IDESC_PV, (j > 0) || (kk > 0));
-          tc::mma_commit(bar(B_VEMPTY + slot));
-          tc::mma_commit(bar(B_PVDONE));
-          if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+          for (int kk = 0; kk < D / 16; ++kk) {
+            const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
+            const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
+            tc::mma_ss(tmem + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
+          }
+          tc::mma_commit(bar(B_SFULL + b));
+          tc::mma_commit(bar(B_KEMPTY + slot));
+          if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
         }
-        g += n;
         ++itc;
       }
       PROF_ADD(0);
       PROF_FLUSH(8, 6);
     }
     __syncwarp();
-  } else if (warp < 4) {
-    // ============================== softmax (warpgroup 0, thread = row) ==============================
+  } else if (warp == W_MMA_PV) {
+    // ============================== MMA issuer for O += P V (one lane) ==============================
+    if (lane == 0) {
+      int g = 0, itc = 0;
+      const uint32_t tO = tmem + TMEM_O;
+      for (int k = 0;; ++k) {
+        const int idx = item_index(k, cta, grid);
+        if (idx >= n_items) break;
+        const int4 rec = p.items[2 * idx];
+        const int n = rec.w - rec.z;
+        for (int j = 0; j < n; ++j, ++g) {
+          const int b = g % NSBUF, slot = g % NSTAGE;
+          tc::mbar_wait(bar(B_PFULL + b), (g / NSBUF) & 1);
+          tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
+          if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
+          tc::tc_fence_after();
+          // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO).
+          // P of tokens [0,64) sits in columns [0,32) of S_b, P of tokens [64,128) in columns [64,96): each softmax
+          // warpgroup overwrites only columns of its own half of S.
+          const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, 1024, GROUP_BYTES);
+#pragma unroll
+          for (int kk = 0; kk < TILE_N / 16; ++kk)
+            tc::mma_ts(tO, tmem + b * TILE_N + (kk >> 2) * 64 + (kk & 3) * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV,
+                       (j > 0) || (kk > 0));
+          tc::mma_commit(bar(B_VEMPTY + slot));
+          tc::mma_commit(bar(B_SFREE + b));
+          tc::mma_commit(bar(B_PVDONE));
+          if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+        }
+        ++itc;
+      }
+    }
+    __syncwarp();
+  } else if (warp < W_EPI) {
+    // ============================== softmax (warpgroups 0 and 1, thread = half of a row) ==============================
+    // Both halves of a row keep the same running reference m_used (it changes only in the pair-synchronised
+    // two-pass branch) and their own partial weight sums, added up once per item.
     tc::setmaxnreg_inc<REGS_SOFTMAX>();
-    const int wq = warp & 3;  // TMEM lane quarter this warp may access
+    const int wg = warp >> 2;  // which 64 columns of every S row
+    const int wq = warp & 3;   // TMEM lane quarter this warp may access
     const int row = wq * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
+    float* xchg_mine = xchg + wg * TILE_M + row;
+    const float* xchg_other = xchg + (wg ^ 1) * TILE_M + row;
     int g = 0, itc = 0;
     PROF_DECL(7);
     PROF_T0();
@@ -376,37 +422,40 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       if (more) mk_next = row_mask(a0, a1);
       const int P = it.P, total = it.P + it.Ki;
       float m_used = -INFINITY, lsum = 0.f, lsum_r = 0.f;
-      const int opar = itc & 1;
-      const uint32_t tO = tmem + TMEM_O + lane_addr;
+      const uint32_t tOh = tmem + TMEM_O + wg * 64 + lane_addr;
 
       for (int j = it.jt0; j < it.jt1; ++j, ++g) {
         const int b = g % NSBUF;
-        const uint32_t tS = tmem + b * TILE_N + lane_addr;
+        const uint32_t tSh = tmem + b * TILE_N + wg * 64 + lane_addr;  // my 64 columns of S; P goes to their first 32
         PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
         tc::tc_fence_after();
-        const int tok0 = j * TILE_N;
-        const bool tail = tok0 + TILE_N > P;  // tile touches tree positions or the ragged end: apply visibility
-        uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
+        const int tile0 = j * TILE_N, tok0 = tile0 + wg * 64;
+        const bool tail = tok0 + 64 > P;  // my keys touch tree positions or the ragged end: apply visibility
+        uint32_t vis[2] = {0xffffffffu, 0xffffffffu};
         if (tail) {
-#pragma unroll
-          for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tok0 + c * 32);
+          vis[0] = visible_word(mk, P, tok0);
+          vis[1] = visible_word(mk, P, tok0 + 32);
         }
-        uint32_t pk[64];  // the bf16 P row
+        uint32_t pk[32];  // my half of the bf16 P row
         float ts = 0.f, tr = 0.f;  // this tile's exact / bf16-rounded weight sums
         // Fast path: the weights are taken against the running reference m_used without looking at this tile's
-        // maximum first; only if a weight sum leaves [0, 2^32] (reference too low, or no reference yet) does
-        // the warp fall back to the two-pass form (row maximum, rescale, weights).  P is stored only after that
-        // check, so S is still intact for the second pass.
-        bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);
+        // maximum first; only if a weight sum leaves [0, 2^32] (reference too low, or no reference yet) do the
+        // two warps of the row quarter fall back to the two-pass form (row maximum, rescale, weights).  P is
+        // stored only after that check, so S is still intact for the second pass.
+        bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);  // the same in both halves
         if (!slow) {
           PROF_SPAN_BEGIN();
-          if (tail) weights_pass<true>(tS, vis, p.scale_log2, -m_used, pk, ts, tr);
-          else weights_pass<false>(tS, vis, p.scale_log2, -m_used, pk, ts, tr);
-          slow = __any_sync(0xffffffffu, !(ts <= WEIGHT_SUM_LIMIT));
+          if (tail) weights_pass<true>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
+          else weights_pass<false>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
+          slow = pair_or(wq, !(ts <= WEIGHT_SUM_LIMIT));
           PROF_SPAN_END(5);
         }
         if (slow) {
-          float mx = row_max_pass(tS, vis);
+          float mx = row_max_pass(tSh, vis);
+          *xchg_mine = mx;
+          pair_sync(wq);
+          mx = fmaxf(mx, *xchg_other);
+          pair_sync(wq);  // both halves have read before the slots are written again
           const float m_new = fmaxf(m_used, mx * p.scale_log2);
           float alpha = 1.f;
           if (m_new > m_used) {
@@ -415,61 +464,70 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           }
           lsum *= alpha;
           lsum_r *= alpha;
-          if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale in TMEM
+          if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale my 64 columns in TMEM
             PROF_WAIT(3, bar(B_PVDONE), (g - 1) & 1);
             tc::tc_fence_after();
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
+            for (int c = 0; c < 2; ++c) {
               uint32_t o[32];
-              tc::tmem_ld32(tO + c * 32, o);
+              tc::tmem_ld32(tOh + c * 32, o);
               tc::tmem_wait_ld();
 #pragma unroll
               for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-              tc::tmem_st32(tO + c * 32, o);
+              tc::tmem_st32(tOh + c * 32, o);
             }
             tc::tmem_wait_st();
           }
           const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-          weights_pass<true>(tS, vis, p.scale_log2, -m_eff, pk, ts, tr);  // vis is all ones off the tail
+          weights_pass<true>(tSh, vis, p.scale_log2, -m_eff, pk, ts, tr);  // vis is all ones off the tail
         }
         lsum += ts;
         lsum_r += tr;
         PROF_SPAN_BEGIN();
-        tc::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
-        tc::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
+        tc::tmem_st32(tSh, pk);
         tc::tmem_wait_st();
-        if (tok0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
+        if (tile0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
           const int slot = g % NSTAGE;
           PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
-          if (row >= total - tok0) {
-            uint4* z0 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + row * 128);
-            uint4* z1 = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + HALF_BYTES + row * 128);
+          if (row >= total - tile0) {  // warpgroup w clears d-half w of V row `row`
+            uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (row >> 3) * GROUP_BYTES + wg * 1024 +
+                                               (row & 7) * 128);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) { z0[e] = make_uint4(0u, 0u, 0u, 0u); z1[e] = make_uint4(0u, 0u, 0u, 0u); }
+            for (int e = 0; e < 8; ++e) z[e] = make_uint4(0u, 0u, 0u, 0u);
           }
           tc::fence_proxy_async();
         }
         tc::tc_fence_before();
-        tc::mbar_arrive(bar(B_PFULL + b));
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
         PROF_SPAN_END(6);
       }
 
-      // ---- hand 1 / l_rounded and lse = ln2 * (m + log2 l) to the epilogue warpgroup ----
-      {
+      // ---- add the two halves' sums; warpgroup 0 hands 1 / l_rounded and lse = ln2 * (m + log2 l) to the epilogue ----
+      if (wg == 1) {
+        xchg_mine[0] = lsum;
+        // the rounded sum travels in warpgroup 0's slot, which warpgroup 0 itself does not write here
+        const_cast<float*>(xchg_other)[0] = lsum_r;
+      }
+      pair_sync(wq);
+      if (wg == 0) {
+        lsum += *xchg_other;
+        lsum_r += *xchg_mine;
         const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
         const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
         const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
-        tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of item itc-1 is done, so statistics buffer opar is free
-        stats[(opar * 2 + 0) * TILE_M + row] = inv;
-        stats[(opar * 2 + 1) * TILE_M + row] = lse_v;
-        tc::mbar_arrive(bar(B_STATS + opar));
+        tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of item itc-1 has read its statistics
+        stats[row] = inv;
+        stats[TILE_M + row] = lse_v;
+        tc::mbar_arrive(bar(B_STATS));
       }
+      pair_sync(wq);  // the exchange slots are free again
       ++itc;
     }
     PROF_ADD(0);
     if (warp == 0 && lane == 0) PROF_FLUSH(16, 7);
-  } else if (warp < 8) {
-    // ============================== epilogue (warpgroup 1, thread = row) ==============================
+  } else if (warp < W_PROD_K0) {
+    // ============================== epilogue (warpgroup 2, thread = row) ==============================
     // O of item n is normalised and stored here while the softmax warpgroup is already on item n+1 (O and the
     // statistics are double buffered by item parity).
     tc::setmaxnreg_dec<REGS_EPILOGUE>();
@@ -489,9 +547,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const int opar = itc & 1;
       const uint32_t tO = tmem + TMEM_O + lane_addr;
       const size_t rowg = (size_t)(it.off + l) * p.Hq + it.kvh * p.G + gq;
-      PROF_WAIT_RELAXED(1, bar(B_STATS + opar), (itc >> 1) & 1);
-      const float inv = stats[(opar * 2 + 0) * TILE_M + row];
-      const float lse_v = stats[(opar * 2 + 1) * TILE_M + row];
+      PROF_WAIT_RELAXED(1, bar(B_STATS), itc & 1);
+      const float inv = stats[row];
+      const float lse_v = stats[TILE_M + row];
       PROF_WAIT(2, bar(B_OFULL), itc & 1);
       tc::tc_fence_after();
       uint32_t o[2][32];
@@ -531,13 +589,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       ++itc;
     }
     PROF_ADD(0);
-    if (warp == 4 && lane == 0) PROF_FLUSH(24, 3);
+    if (warp == W_EPI && lane == 0) PROF_FLUSH(24, 3);
   }
 
   // ---- teardown ----
   tc::tc_fence_before();
   __syncthreads();
-  if (warp == W_MMA) tc::tmem_dealloc(tmem, TMEM_COLS);
+  if (warp == W_MMA_QK) tc::tmem_dealloc(tmem, TMEM_COLS);
 }
 
 // Device-side planner: P_i and K_i exist only on the device, so the work list is built there.
@@ -658,11 +716,12 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
     }
   }
   for (int which = 0; which < 2; ++which) {
-    cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)total_rows};
-    cuuint64_t strides[1] = {(cuuint64_t)D * 2};
-    cuuint32_t box[2] = {64, (cuuint32_t)PAGE};
-    cuuint32_t es[2] = {1, 1};
-    CUresult r = enc(which ? &tv : &tk, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, which ? kv->v_pool : kv->k_pool, dims,
+    // pool rows [token][128 d] seen as [8-token group][d-half][token in group][64 d]: one box = one page
+    cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)(total_rows / 8)};
+    cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)D * 2 * 8};
+    cuuint32_t box[4] = {64, 8, 2, (cuuint32_t)(PAGE / 8)};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = enc(which ? &tv : &tk, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, which ? kv->v_pool : kv->k_pool, dims,
                      strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
