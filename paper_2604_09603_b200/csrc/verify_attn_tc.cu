@@ -46,6 +46,10 @@ constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,51
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 constexpr float WEIGHT_SUM_LIMIT = 4294967296.f;  // a tile whose weight sum exceeds 2^32 is redone against its own maximum
+// Every item starts from the reference 0 instead of the first tile's row maxima: weights are floating point, so any
+// reference within 2^-64 .. 2^32 of the true one gives the same O and lse; a first tile whose weight sum falls outside
+// that range is redone in the two-pass form, which takes the reference from the data.
+constexpr float WEIGHT_SUM_FLOOR = 5.421010862427522e-20f;  // 2^-64
 
 constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
@@ -421,7 +425,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       if (item_index(k + 2, cta, grid) < n_items) { b0 = p.items[2 * item_index(k + 2, cta, grid)]; b1 = p.items[2 * item_index(k + 2, cta, grid) + 1]; }
       if (more) mk_next = row_mask(a0, a1);
       const int P = it.P, total = it.P + it.Ki;
-      float m_used = -INFINITY, lsum = 0.f, lsum_r = 0.f;
+      float m_used = 0.f, lsum = 0.f, lsum_r = 0.f;
       const uint32_t tOh = tmem + TMEM_O + wg * 64 + lane_addr;
 
       for (int j = it.jt0; j < it.jt1; ++j, ++g) {
@@ -447,10 +451,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           PROF_SPAN_BEGIN();
           if (tail) weights_pass<true>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
           else weights_pass<false>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
-          slow = pair_or(wq, !(ts <= WEIGHT_SUM_LIMIT));
+          slow = pair_or(wq, !(ts <= WEIGHT_SUM_LIMIT) || (j == it.jt0 && ts < WEIGHT_SUM_FLOOR));
           PROF_SPAN_END(5);
         }
         if (slow) {
+          if (j == it.jt0) m_used = -INFINITY;  // nothing accumulated yet: drop the guessed reference
           float mx = row_max_pass(tSh, vis);
           *xchg_mine = mx;
           pair_sync(wq);

@@ -139,3 +139,39 @@ def test_attn_sibling_isolation(path):
     assert len(keep) == Ki - 1
     assert torch.equal(out0[keep], out1[keep]) and torch.equal(lse0[keep], lse1[keep])
     assert not torch.equal(out0[int(offs[i]) + victim], out1[int(offs[i]) + victim])
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("regime", ["all_low", "low_then_normal", "late_spike"])
+def test_attn_extreme_scores(path, regime):
+    """Scores far from the reference the tcgen05 kernel starts every item with (0): a first tile whose weights all
+    underflow (two-pass fallback takes the reference from the data), a later tile that overflows it (O rescaled in
+    TMEM), and one dominant key deep in the prefix.  Oracle: plain fp64 softmax, no running maximum."""
+    import torch
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(1, R=3, gated=True)
+    ctx, sel, want_sel, q, k, v = _setup(wl, poison=False)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    K = np.diff(want_sel["sel_offsets"])
+
+    def set_k0(i, positions, value):
+        pos = np.asarray(positions)
+        pg = torch.from_numpy(wl.page_table[i, pos // 16].astype(np.int64)).cuda()
+        sl = torch.from_numpy((pos % 16).astype(np.int64)).cuda()
+        k[0, pg, :, sl, 0] = value
+
+    q[:, :, 0] = 40.0                      # score = (40 k_0 + N(0, 127)) / sqrt(128)
+    for i in range(wl.R):
+        total = int(wl.prefix_len[i] + K[i])
+        if regime == "all_low":            # every score near -141 (log2 domain -204)
+            set_k0(i, np.arange(total), -40.0)
+        elif regime == "low_then_normal":  # first KV tile near -141, the rest N(0, 3.5^2)
+            set_k0(i, np.arange(min(128, total)), -40.0)
+        else:                              # one key at +106 in the third tile
+            set_k0(i, [300], 30.0)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    n = want_sel["n_selected"]
+    rng = np.random.default_rng(5)
+    rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(48)] + [(0, 0), (n - 1, wl.Hq - 1)]
+    _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
+    assert ctx.device_status() == 0
