@@ -43,6 +43,11 @@ constexpr int REGS_SOFTMAX = 160, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (
 constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
 constexpr int TMEM_O = NSBUF * TILE_N;
 constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
+// of every POLY_PERIOD weight pairs in a prefix tile, POLY_COUNT take 2^x on the FMA pipe, the rest on MUFU
+#ifndef ECHO_POLY_COUNT
+#define ECHO_POLY_COUNT 1
+#endif
+constexpr int POLY_PERIOD = 4, POLY_COUNT = ECHO_POLY_COUNT;  // measured best: 1 of 4 (2 of 4 and 3 of 8 are slower)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 constexpr float WEIGHT_SUM_LIMIT = 4294967296.f;  // a tile whose weight sum exceeds 2^32 is redone against its own maximum
@@ -138,6 +143,29 @@ __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
     if (!((vis >> e) & 1u)) s[e] = 0xff800000u;  // -inf
 }
 
+// 2^x for a pair of finite x on the FMA pipe instead of MUFU (16 ex2 per clock per SM, the busiest pipe of the
+// softmax): n = round(x) by the 1.5*2^23 trick, f = x - n in [-0.5, 0.5], 2^f by a degree-3 minimax polynomial
+// (relative error 7.5e-5, far below the bf16 rounding of P), then n is added to the exponent field.  x is clamped
+// to [-125, 126]: 2^-125 instead of less is negligible against the reference weight 1 (so this form is used only
+// where no key is masked), and 2^126 sends the tile to the two-pass fallback.
+__device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  tc::unpack_f32x2(x2, x0, x1);
+  x2 = tc::pack_f32x2(fminf(fmaxf(x0, -125.f), 126.f), fminf(fmaxf(x1, -125.f), 126.f));
+  const uint64_t magic = tc::pack_f32x2(12582912.f, 12582912.f), nmagic = tc::pack_f32x2(-12582912.f, -12582912.f);
+  const uint64_t t = tc::add_f32x2(x2, magic);
+  const uint64_t n = tc::add_f32x2(t, nmagic);
+  const uint64_t f = tc::fma_f32x2(n, tc::pack_f32x2(-1.f, -1.f), x2);
+  uint64_t q = tc::fma_f32x2(f, tc::pack_f32x2(0x1.c3f76p-5f, 0x1.c3f76p-5f), tc::pack_f32x2(0x1.f0de1ap-3f, 0x1.f0de1ap-3f));
+  q = tc::fma_f32x2(q, f, tc::pack_f32x2(0x1.62f31ap-1f, 0x1.62f31ap-1f));
+  q = tc::fma_f32x2(q, f, tc::pack_f32x2(0x1.fff692p-1f, 0x1.fff692p-1f));
+  float q0, q1, t0, t1;
+  tc::unpack_f32x2(q, q0, q1);
+  tc::unpack_f32x2(t, t0, t1);
+  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
+  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
+}
+
 // weights p = 2^(s*scale_log2 + neg_m) for 64 columns: packed to bf16 in pk, exact fp32 sum in ts and (tail tiles
 // only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the issue slots.
 // TAIL = false (all 64 keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP / FADD2 with no
@@ -159,9 +187,16 @@ __device__ __forceinline__ void weights_pass(uint32_t tSh, const uint32_t (&vis)
     if (TAIL) mask_chunk(sc, vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2) {
-      float x0, x1;
-      tc::unpack_f32x2(tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2), x0, x1);
-      const float p0 = tc::ex2(x0), p1 = tc::ex2(x1);
+      const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
+      float p0, p1;
+      if (!TAIL && ((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
+        ex2_poly_x2(x2, p0, p1);
+      } else {
+        float x0, x1;
+        tc::unpack_f32x2(x2, x0, x1);
+        p0 = tc::ex2(x0);
+        p1 = tc::ex2(x1);
+      }
       const uint32_t w = tc::pack_bf16(p0, p1);
       pk[c * 16 + (e >> 1)] = w;
       acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
