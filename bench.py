@@ -314,7 +314,7 @@ def main():
         if not args.splits:
             while splits < 8 and units * splits < 2 * torch.cuda.get_device_properties(0).multi_processor_count:
                 splits *= 2
-        launches = 2 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)
+        launches = 3 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)  # gate 3, plan + attn, merge, accept, argmax
         line = {"metric": "verified draft tokens/s", "value": n_sel_all * args.steps / (ms * 1e-3), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",

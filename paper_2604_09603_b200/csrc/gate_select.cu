@@ -2,9 +2,11 @@
 //   k_score_gate  : one CTA per request -- path scores (Eq. 5), level maxima and the
 //                   sparse gate (Eq. 6-7), tier assignment (Alg. 1) and a
 //                   unique 64-bit selection key per candidate.
-//   k_select_pack : one CTA -- radix select of the budget-th smallest key (Eq. 4), then
-//                   Flatten & Pack (Fig. 3(3)) with local parents and 128-bit ancestor masks.
-// These steps move < 1 MB and are latency-bound: two launches, no host sync.
+//   k_select      : one CTA -- radix select of the budget-th smallest key (Eq. 4), per-request
+//                   counts and CSR offsets.
+//   k_pack        : one CTA per request -- Flatten & Pack (Fig. 3(3)) with local parents and 128-bit
+//                   ancestor masks.
+// These steps move < 1 MB and are latency-bound: three launches, no host sync.
 #include "common.cuh"
 
 namespace {
@@ -108,6 +110,7 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
 }
 
 constexpr int SEL_THREADS = 1024;
+constexpr int SEL_KPT = 16;  // keys per thread kept in registers by the radix select
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 #pragma unroll
@@ -118,25 +121,39 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   return v;
 }
 
-__global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
-    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent,
-    const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys, int R, int N, int budget,
-    int capacity, int32_t* __restrict__ n_selected, int32_t* __restrict__ sel_offsets,
-    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
-    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
+__global__ void __launch_bounds__(SEL_THREADS) k_select(
+    const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ keys, int R, int N, int budget,
+    int32_t* __restrict__ n_selected, int32_t* __restrict__ sel_offsets, uint64_t* __restrict__ threshold) {
   __shared__ int s_hist[256];
   __shared__ int s_warp[32];
   __shared__ uint64_t s_prefix;
   __shared__ int s_k;
   __shared__ int s_eligible;
+  __shared__ int s_done;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   // ---- S3: threshold T = budget-th smallest key (keys are unique => no ties to break) ----
+  // Keys stay in registers across the passes when N <= SEL_THREADS * SEL_KPT (every config of BASELINE.json),
+  // histogram updates are aggregated per thread and per warp (the top bytes of the keys -- tier, sign, exponent --
+  // take one or two values, which would serialise 10 240 shared-memory atomics on one address), and the digit loop
+  // stops as soon as the bucket that holds the budget-th key is taken whole.
+  const bool cached = N <= SEL_THREADS * SEL_KPT;
+  uint64_t rk[SEL_KPT];
+#pragma unroll
+  for (int i = 0; i < SEL_KPT; ++i) {
+    const int g = tid + i * SEL_THREADS;
+    rk[i] = (cached && g < N) ? keys[g] : KEY_INELIGIBLE;
+  }
   if (tid == 0) s_eligible = 0;
   __syncthreads();
   {
     int e = 0;
-    for (int g = tid; g < N; g += SEL_THREADS) e += keys[g] != KEY_INELIGIBLE;
+    if (cached) {
+#pragma unroll
+      for (int i = 0; i < SEL_KPT; ++i) e += rk[i] != KEY_INELIGIBLE;
+    } else {
+      for (int g = tid; g < N; g += SEL_THREADS) e += keys[g] != KEY_INELIGIBLE;
+    }
     e = warp_incl_scan(e, lane);
     if (lane == 31 && e) atomicAdd(&s_eligible, e);
   }
@@ -147,15 +164,41 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
   } else if (s_eligible <= budget) {
     T = KEY_INELIGIBLE - 1;  // everything eligible (R:G-12)
   } else {
-    if (tid == 0) { s_prefix = 0; s_k = budget; }
-    for (int pass = 0; pass < 8; ++pass) {
-      const int shift = 56 - 8 * pass;
+    if (tid == 0) { s_prefix = 0; s_k = budget; s_done = 0; }
+    int shift = 56;
+    for (int pass = 0; pass < 8; ++pass, shift -= 8) {
       if (tid < 256) s_hist[tid] = 0;
       __syncthreads();
       const uint64_t prefix = s_prefix;
-      for (int g = tid; g < N; g += SEL_THREADS) {
-        uint64_t key = keys[g];
-        if (pass == 0 || (key >> (shift + 8)) == prefix) atomicAdd(&s_hist[(int)((key >> shift) & 0xff)], 1);
+      auto in_prefix = [&](uint64_t key) { return key != KEY_INELIGIBLE && (pass == 0 || (key >> (shift + 8)) == prefix); };
+      if (cached) {
+        // the thread's keys that share the digit of its first participating key go in as one count; if the whole
+        // warp agrees on that digit, as one atomic per warp
+        int d0 = -1, cnt0 = 0;
+#pragma unroll
+        for (int i = 0; i < SEL_KPT; ++i) {
+          if (in_prefix(rk[i])) {
+            const int digit = (int)((rk[i] >> shift) & 0xff);
+            if (d0 < 0) d0 = digit;
+            if (digit == d0) ++cnt0;
+            else atomicAdd(&s_hist[digit], 1);
+          }
+        }
+        const unsigned have = __ballot_sync(0xffffffffu, d0 >= 0);
+        if (have) {
+          const int lead = __shfl_sync(0xffffffffu, d0, __ffs(have) - 1);
+          if (__all_sync(0xffffffffu, d0 < 0 || d0 == lead)) {
+            const int total = __reduce_add_sync(0xffffffffu, cnt0);
+            if (lane == 0) atomicAdd(&s_hist[lead], total);
+          } else if (d0 >= 0) {
+            atomicAdd(&s_hist[d0], cnt0);
+          }
+        }
+      } else {
+        for (int g = tid; g < N; g += SEL_THREADS) {
+          const uint64_t key = keys[g];
+          if (in_prefix(key)) atomicAdd(&s_hist[(int)((key >> shift) & 0xff)], 1);
+        }
       }
       __syncthreads();
       if (warp == 0) {  // find the digit that holds the k-th key
@@ -169,14 +212,20 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
           int run = excl;
 #pragma unroll
           for (int t = 0; t < 8; ++t) {
-            if (run < k && k <= run + c[t]) { s_prefix = (prefix << 8) | (uint64_t)(lane * 8 + t); s_k = k - run; }
+            if (run < k && k <= run + c[t]) {
+              s_prefix = (prefix << 8) | (uint64_t)(lane * 8 + t);
+              s_k = k - run;
+              if (k - run == c[t]) s_done = 1;  // the whole bucket is selected: lower digits do not matter
+            }
             run += c[t];
           }
         }
       }
       __syncthreads();
+      if (s_done) break;
     }
-    T = s_prefix;
+    // keys with the found prefix (and everything below it) are selected; pad the undecided low digits with ones
+    T = shift > 0 ? ((s_prefix << shift) | ((1ull << shift) - 1ull)) : s_prefix;
   }
   const bool none = budget <= 0;
 
@@ -208,18 +257,36 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
     for (int r = lo; r < hi; ++r) { run += sel_offsets[r + 1]; sel_offsets[r + 1] = run; }
     if (tid == SEL_THREADS - 1) *n_selected = s_warp[31];
   }
-  __syncthreads();
+  if (tid == 0) *threshold = none ? 0ull : T + 1ull;  // k_pack selects keys < threshold (0 = nothing; T < 2^64 - 1)
+}
 
-  // ---- S4/S5: packed arrays, local parents, ancestor-or-self masks ----
-  for (int r = warp; r < R; r += SEL_THREADS / 32) {
+// S4/S5: packed arrays, local parents, ancestor-or-self masks.  One CTA per request, thread = candidate.
+__global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent,
+    const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys,
+    const uint64_t* __restrict__ threshold, int capacity, const int32_t* __restrict__ sel_offsets,
+    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
+    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
+  __shared__ int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks below are chains of dependent reads
+  __shared__ uint32_t s_bal[4];
+  const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  {
     const int b = cand_offsets[r], C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
     const int base = sel_offsets[r];
+    const uint64_t thr = *threshold;
+    {
+      const int j = tid;
+      const uint32_t mine = __ballot_sync(0xffffffffu, j < C && keys[b + j] < thr);
+      if (lane == 0) s_bal[warp] = mine;
+      if (j < C) {
+        const int pj = parent[b + j];
+        par[j] = pj >= j ? -1 : pj;
+      }
+    }
+    __syncthreads();
     uint32_t bal[4];
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      int j = w * 32 + lane;
-      bal[w] = __ballot_sync(0xffffffffu, !none && j < C && keys[b + j] <= T);
-    }
+    for (int w = 0; w < 4; ++w) bal[w] = s_bal[w];
     auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
       int l = 0;
 #pragma unroll
@@ -229,15 +296,14 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
       }
       return l;
     };
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      int j = w * 32 + lane;
-      if (!((bal[w] >> lane) & 1u)) continue;
+    {
+      const int w = warp;
+      const int j = tid;
+      if (!((bal[w] >> lane) & 1u)) return;
       const int l = local_of(j);
       const int k = base + l;
-      if (k >= capacity) continue;
-      int p = parent[b + j];
-      if (p >= j) p = -1;
+      if (k >= capacity) return;
+      const int p = par[j];
       uint32_t m[4] = {0u, 0u, 0u, 0u};
       m[l >> 5] |= 1u << (l & 31);
       int pl = -1;
@@ -247,8 +313,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
         int la = local_of(c);
         if (step == 0) pl = la;
         m[la >> 5] |= 1u << (la & 31);
-        int pc = parent[b + c];
-        c = (pc >= c) ? -1 : pc;
+        c = par[c];
       }
       sel_node[k] = j;
       sel_req[k] = r;
@@ -264,7 +329,9 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_pack(
 int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, cudaStream_t st) {
   const int R = t->num_requests, N = t->total_cand;
   uint64_t* keys = reinterpret_cast<uint64_t*>(ctx->workspace);
-  if ((size_t)N * sizeof(uint64_t) > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  const size_t keys_bytes = align_up((size_t)N * sizeof(uint64_t), 256);
+  if (keys_bytes + 256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  uint64_t* threshold = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(ctx->workspace) + keys_bytes);
   GateParams gp;
   gp.depth_mask = g->depth_mask;
   for (int d = 0; d < 32; ++d) gp.log_tau[d] = g->log_tau[d] + 0.0f;  // canonicalise -0 (R:G-13)
@@ -275,9 +342,12 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);
   }
   const int budget = g->static_k > 0 ? N : g->budget;
-  k_select_pack<<<1, SEL_THREADS, 0, st>>>(t->cand_offsets, t->parent, o->cand_depth, keys, R, N, budget,
-                                           o->capacity, o->n_selected, o->sel_offsets, o->sel_node, o->sel_req,
-                                           o->parent_local, o->sel_depth, o->anc_mask);
+  k_select<<<1, SEL_THREADS, 0, st>>>(t->cand_offsets, keys, R, N, budget, o->n_selected, o->sel_offsets, threshold);
+  if (R > 0) {
+    k_pack<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, o->cand_depth, keys, threshold, o->capacity,
+                                        o->sel_offsets, o->sel_node, o->sel_req, o->parent_local, o->sel_depth,
+                                        o->anc_mask);
+  }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;
 }
