@@ -142,14 +142,14 @@ def run_reference(args, rank, world):
 def run_gpu(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
-    from paper_2604_09603_b200 import build, echo, workloads as W
+    from paper_2604_09603_b200 import build, echo, sharding, workloads as W
 
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     build.build_library()
-    wl = W.make_config(args.config, seed=W.SEED_BASE + args.config + 1000 * rank)
+    wl = sharding.rank_workload(args.config, rank)
     g = wl.gate
     cap = wl.capacity()
     ctx = echo.EchoContext(local_rank, 0)
@@ -294,13 +294,9 @@ def main():
     r = run_gpu(args, rank, world, local_rank)
     torch, dist = r["torch"], r["dist"]
     e2e_dt, h2d, d2h = run_e2e(r, args)
-    stats = torch.tensor([r["ms"], e2e_dt, -float(r["n_sel"]), -float(r["accepted"])], dtype=torch.float64, device=r["dev"])
-    tot = torch.tensor([float(r["n_sel"]), float(r["accepted"])], dtype=torch.float64, device=r["dev"])
-    if world > 1:
-        dist.all_reduce(stats, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms, e2e_dt = float(stats[0]), float(stats[1])
-    n_sel_all, acc_all = float(tot[0]), float(tot[1])
+    from paper_2604_09603_b200 import sharding
+    (ms, e2e_dt), (n_sel_all, acc_all) = sharding.reduce_step_stats(
+        [r["ms"], e2e_dt], [r["n_sel"], r["accepted"]], world, r["dev"], dist)
     if rank == 0:
         peak, peak_src = peaks()
         achieved = r["bytes_alg"] / (r["t_attn"] * 1e-3) / 1e9
@@ -315,7 +311,7 @@ def main():
             while splits < 8 and units * splits < 2 * torch.cuda.get_device_properties(0).multi_processor_count:
                 splits *= 2
         launches = 3 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)  # gate 3, plan + attn, merge, accept, argmax
-        line = {"metric": "verified draft tokens/s", "value": n_sel_all * args.steps / (ms * 1e-3), "unit": "tokens/s",
+        line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "requests": wl.R, "verified_nodes_per_step": r["n_sel"],

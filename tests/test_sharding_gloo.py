@@ -1,0 +1,65 @@
+"""N > 1 path on CPU: two gloo processes run the host-side logic bench.py uses under torchrun:
+per-rank batches are disjoint, rank 0 reproduces the single-GPU workload, the step time is the max over ranks and the
+token counts are sums -- and each rank's selection (computed by the oracle here: no GPU) depends on its own batch only."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2604_09603_b200 import sharding
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import echo_oracle as orc
+        wl = sharding.rank_workload(0, rank)
+        g = wl.gate
+        sel = orc.gate_select(wl.cand_offsets, wl.parent, wl.logq, g.depth_mask, g.log_tau, g.w_max, g.budget, g.static_k)
+        n_sel = int(sel["n_selected"])
+        ms = 10.0 + 5.0 * rank            # rank 1 is the slow one
+        (t_max, e_max), (n_all, acc_all) = sharding.reduce_step_stats([ms, ms / 1e3], [n_sel, rank + 1], world,
+                                                                       torch.device("cpu"), dist)
+        gathered = [None] * world
+        dist.all_gather_object(gathered, (n_sel, float(wl.logq.sum()), wl.prefix_len.tolist()))
+        out[rank] = dict(t_max=t_max, e_max=e_max, n_all=n_all, acc_all=acc_all, gathered=gathered, n_sel=n_sel)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_reduction_and_disjoint_batches():
+    world = 2
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+        res = {k: dict(v) for k, v in out.items()}
+    assert set(res) == {0, 1}
+    for r in (0, 1):
+        assert res[r]["t_max"] == 15.0 and res[r]["e_max"] == pytest.approx(0.015)   # max over ranks
+        assert res[r]["acc_all"] == 3.0                                              # 1 + 2
+        assert res[r]["n_all"] == res[0]["n_sel"] + res[1]["n_sel"]                  # sum over ranks
+    g = res[0]["gathered"]
+    assert g[0][1] != g[1][1]                      # different draws per rank
+    assert g == res[1]["gathered"]                 # both ranks saw the same exchange
+    # whole-job value = all ranks' units / slowest rank's time
+    assert sharding.job_throughput(res[0]["n_all"], 4, res[0]["t_max"]) == pytest.approx(res[0]["n_all"] * 4 / 0.015)
+
+
+def test_rank0_is_the_single_gpu_workload():
+    from paper_2604_09603_b200 import workloads as W
+    a, b = sharding.rank_workload(0, 0), W.make_config(0)
+    assert np.array_equal(a.logq, b.logq) and np.array_equal(a.page_table, b.page_table)
+    assert sharding.rank_seed(2, 3) == W.SEED_BASE + 2 + 3000
+    t, c = sharding.reduce_step_stats([1.5], [7], 1, torch.device("cpu"))
+    assert t == [1.5] and c == [7.0]
