@@ -282,7 +282,8 @@ def main():
     ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
     ap.add_argument("--attn-path", type=int, default=0)
     ap.add_argument("--splits", type=int, default=0)
-    ap.add_argument("--ref-nodes", type=int, default=32)
+    ap.add_argument("--ref-nodes", type=int, default=32, help="--impl reference: packed nodes of oracle attention per step (~0.75 s)")
+    ap.add_argument("--baseline-nodes", type=int, default=512, help="cpu_baseline leg: packed nodes of oracle attention (~12 s once)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -328,7 +329,7 @@ def main():
                 "gpu_launches": launches * args.steps, "clocks": r["sampler"].summary()}
         if not args.no_cpu_baseline:
             try:
-                v, desc, cores = oracle_sample(wl, n_attn_nodes=args.ref_nodes)
+                v, desc, cores = oracle_sample(wl, n_attn_nodes=args.baseline_nodes)
                 line["cpu_baseline"] = {"value": v, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": desc}
             except Exception as e:  # the baseline leg must never take the GPU number down with it
                 line["cpu_baseline"] = {"value": None, "unit": "tokens/s", "cores": 1, "kind": "oracle", "sample": f"failed: {e}"}
