@@ -259,7 +259,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cta = blockIdx.x, grid = gridDim.x;
-  const int n_items = *p.n_items;
 
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();  // SW128 operand tiles need 1024-byte alignment
@@ -279,6 +278,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = *tmem_slot;
+  // Programmatic dependent launch: everything above (barrier init, TMEM allocation, descriptor prefetch) overlaps
+  // k_plan; the work list is read only after k_plan has completed.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const int n_items = *p.n_items;
 
   if (warp >= 12) tc::setmaxnreg_dec<REGS_AUX>();
   if (warp == W_PROD_K0 || warp == W_PROD_V0 || warp == W_PROD_K1 || warp == W_PROD_V1) {
@@ -648,6 +651,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
                                                        int32_t* __restrict__ n_items) {
   __shared__ int s_cnt[PLAN_BUCKETS];
   __shared__ int s_warp[32];
+  asm volatile("griddepcontrol.launch_dependents;");  // let k_verify_attn_tc set itself up meanwhile
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int b = tid; b < PLAN_BUCKETS; b += PLAN_THREADS) s_cnt[b] = 0;
   __syncthreads();
@@ -795,7 +799,19 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   p.part_o = part_o; p.part_lse = part_lse; p.n_rows_cap = n_rows; p.status = ctx->dev_status;
   int grid = ctx->opt_num_ctas > 0 ? (int)ctx->opt_num_ctas : ctx->num_sms;
   if ((size_t)grid > max_items) grid = (int)(max_items ? max_items : 1);
-  k_verify_attn_tc<<<grid, NTHREADS, SMEM_TOTAL, st>>>(tq, tk, tv, p);
+  {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = SMEM_TOTAL;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, tq, tk, tv, p));
+  }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;
 }
