@@ -44,6 +44,10 @@ template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile
 __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) __nanosleep(256);
 }
+// same with a short back-off, for producers that run a ring ahead of their consumers
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) __nanosleep(64);
+}
 
 // generic-proxy smem writes -> visible to the async proxy (TMA / tcgen05 operand reads)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }

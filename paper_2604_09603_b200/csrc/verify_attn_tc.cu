@@ -90,6 +90,7 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_ADD(slot) prof_[slot] += clock64() - prof_t0_
 #define PROF_WAIT(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait(b, ph); prof_[slot] += clock64() - t_; } while (0)
 #define PROF_WAIT_RELAXED(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait_relaxed(b, ph); prof_[slot] += clock64() - t_; } while (0)
+#define PROF_WAIT_BACKOFF(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait_backoff(b, ph); prof_[slot] += clock64() - t_; } while (0)
 #define PROF_DECL(n) unsigned long long prof_[n] = {}
 #define PROF_FLUSH(base, n) do { if (blockIdx.x < ECHO_PROF_CTAS) for (int q_ = 0; q_ < n; ++q_) g_wait_prof[blockIdx.x][(base) + q_] = prof_[q_]; } while (0)
 #define PROF_SPAN_BEGIN() const long long span_t_ = clock64()
@@ -99,6 +100,7 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_ADD(slot) do {} while (0)
 #define PROF_WAIT(slot, b, ph) tc::mbar_wait(b, ph)
 #define PROF_WAIT_RELAXED(slot, b, ph) tc::mbar_wait_relaxed(b, ph)
+#define PROF_WAIT_BACKOFF(slot, b, ph) tc::mbar_wait_backoff(b, ph)
 #define PROF_DECL(n) do {} while (0)
 #define PROF_FLUSH(base, n) do {} while (0)
 #define PROF_SPAN_BEGIN() do {} while (0)
@@ -310,7 +312,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         if (more) nx = load_item(p.items, item_index(k, cta, grid));
         const int total = it.P + it.Ki;
         if (loads_q) {
-          PROF_WAIT(2, bar(B_QEMPTY), (itc & 1) ^ 1);
+          PROF_WAIT_BACKOFF(2, bar(B_QEMPTY), (itc & 1) ^ 1);
           tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
           const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
           tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
@@ -338,7 +340,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           const int npv = max(0, min(4, npages - j * 8 - half * 4));  // my pages of this tile that hold tokens
           const uint32_t dst = s_dst + slot * TILE_BYTES + half * 4 * PAGE_BYTES;
           const uint32_t fb = bar(b_full + slot);
-          PROF_WAIT(1, bar(b_empty + slot), ph ^ 1);
+          PROF_WAIT_BACKOFF(1, bar(b_empty + slot), ph ^ 1);
           tc::mbar_expect_tx(fb, npv * PAGE_BYTES);
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
