@@ -36,6 +36,15 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def tensor_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        if "bf16_tflops" in d:
+            return float(d["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+    return 2250.0, "fallback (B200_PROFILING.md nominal dense bf16)"
+
+
 class ClockSampler(threading.Thread):
     """samples SM clock, power and throttle reasons during the timed region: NVML every 2 ms when pynvml is there
     (the default run lasts ~15 ms), else nvidia-smi every 100 ms"""
@@ -174,7 +183,7 @@ def run_gpu(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     build.build_library()
-    wl = sharding.rank_workload(args.config, rank)
+    wl = sharding.rank_workload(args.config, rank, static=args.static, gated=not args.static)
     g = wl.gate
     cap = wl.capacity()
     ctx = echo.EchoContext(local_rank, 0)
@@ -310,6 +319,7 @@ def main():
     ap.add_argument("--ref-nodes", type=int, default=32, help="--impl reference: packed nodes of oracle attention per step (~0.75 s)")
     ap.add_argument("--baseline-nodes", type=int, default=512, help="cpu_baseline leg: packed nodes of oracle attention (~12 s once)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
@@ -326,6 +336,10 @@ def main():
     if rank == 0:
         peak, peak_src = peaks()
         achieved = r["bytes_alg"] / (r["t_attn"] * 1e-3) / 1e9
+        tpeak, tpeak_src = tensor_peak()
+        # the static-60 run has ~400 FLOP per byte, above the ridge of the measured peaks: its roof is the tensor pipe
+        tensor_bound = r["flops_alg"] / r["bytes_alg"] > tpeak * 1e12 / (peak * 1e9)
+        tflops = r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
@@ -340,15 +354,17 @@ def main():
         line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": {"workload": WORKLOADS[args.config], "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
+                "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else ""), "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
                            "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],
                            "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12},
                 "accepted_tokens_per_s": acc_all * args.steps / (ms * 1e-3),
-                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                             "traffic": traffic, "peak_source": peak_src, "kernel": "echo_verify_attn (plan + k_verify_attn_tc"
-                             + (" + k_lse_merge)" if splits > 1 else ")"), "bytes_per_launch": r["bytes_alg"]},
+                "roofline": {"bound": "tensor" if tensor_bound else "hbm", "achieved": tflops if tensor_bound else achieved,
+                             "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",
+                             "frac": tflops / tpeak if tensor_bound else achieved / peak,
+                             "traffic": None if args.static else traffic, "peak_source": tpeak_src if tensor_bound else peak_src, "kernel": "echo_verify_attn (plan + k_verify_attn_tc"
+                             + (" + k_lse_merge)" if splits > 1 else ")"), "bytes_per_launch": r["bytes_alg"], "flops_per_launch": r["flops_alg"]},
                 "e2e": {"value": n_sel_all * args.steps / e2e_dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h},
                 "gpu_launches": launches * args.steps, "clocks": r["sampler"].summary()}

@@ -175,3 +175,22 @@ def test_attn_extreme_scores(path, regime):
     rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(48)] + [(0, 0), (n - 1, wl.Hq - 1)]
     _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
     assert ctx.device_status() == 0
+
+
+@pytest.mark.parametrize("cfg,static", [(2, False), (2, True), (3, False)])
+def test_attn_full_size_bench_configuration(cfg, static):
+    """BASELINE.json's full sizes (BS=128) in the launch configuration bench.py times (default path, default
+    splits): 130 sampled (node, head) rows -- first and last row of the batch, the rest uniform -- against the
+    oracle, which computes each row on its own."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(cfg, static=static, gated=not static)
+    ctx, sel, want_sel, q, k, v = _setup(wl)
+    ctx.set_option(echo.OPT_ATTN_PATH, 0)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 0)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    n = want_sel["n_selected"]
+    assert n == (wl.R * 60 if static else wl.gate.budget)
+    rng = np.random.default_rng(100 + cfg)
+    rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(128)] + [(0, 0), (n - 1, wl.Hq - 1)]
+    _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
+    assert ctx.device_status() == 0
