@@ -205,9 +205,9 @@ def run_gpu(args, rank, world, local_rank):
     out = torch.zeros_like(q)
     lse = torch.zeros(cap, wl.Hq, dtype=torch.float32, device=dev)
 
-    def gate(din):
+    def gate(din, sel_=None):
         return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
-                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel)
+                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel_ or sel)
 
     gate(d_in)
     sel_h = sel.to_host()
@@ -228,19 +228,20 @@ def run_gpu(args, rank, world, local_rank):
     attn_ev = [(ev(), ev()) for _ in range(args.steps)]
     gate_ev = [(ev(), ev()) for _ in range(args.steps)]
 
-    def step(din, i=None, qq=q):
+    def step(din, i=None, qq=q, bufs=None):
+        sel_, acc_, out_, lse_ = bufs or (sel, acc, out, lse)
         if i is not None:
             gate_ev[i][0].record()
-        gate(din)
+        gate(din, sel_)
         if i is not None:
             gate_ev[i][1].record(); attn_ev[i][0].record()
-        ctx.verify_attn(sel, kv, qq, SM_SCALE, out=out, lse=lse)
+        ctx.verify_attn(sel_, kv, qq, SM_SCALE, out=out_, lse=lse_)
         if i is not None:
             attn_ev[i][1].record()
         if logits is not None:
-            ctx.accept(sel, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc)
+            ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc_)
         else:
-            ctx.accept(sel, kv, din["draft"], din["prev"], target_token=din["target"], out=acc)
+            ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=din["target"], out=acc_)
 
     def barrier():
         if world > 1:
@@ -271,39 +272,58 @@ def run_gpu(args, rank, world, local_rank):
 
 def run_e2e(r, args):
     """Same step through the public API with HOST buffers: pinned H2D of the step's inputs (trees, logq, Q,
-    tokens) and D2H of its results (out, lse, acceptance) inside the timed region; the paged KV cache is
-    resident serving state and is not re-uploaded."""
-    torch, dev = r["torch"], r["dev"]
-    h_in, d_in = r["h_in"], r["d_in"]
+    tokens) and D2H of its results (out, lse, acceptance) inside the timed region, every step; the paged KV cache
+    is resident serving state and is not re-uploaded.  Three streams and two sets of device
+    buffers: the upload of step i+1 and the download of step i-1 overlap the kernels of step i (PCIe is full
+    duplex); each step still moves all of its own bytes."""
+    torch, dev, ctx, wl = r["torch"], r["dev"], r["ctx"], r["wl"]
+    h_in = r["h_in"]
     h_q = r["q"].cpu().pin_memory()
-    d_q = r["q"]
-    h_out = torch.empty_like(r["out"], device="cpu").pin_memory()
-    h_lse = torch.empty_like(r["lse"], device="cpu").pin_memory()
-    acc = r["acc"]
-    outs = [acc.accept_len, acc.accept_idx, acc.bonus_token, acc.new_len, r["sel"].n_selected]
-    h_outs = [torch.empty_like(t, device="cpu").pin_memory() for t in outs]
-    h2d = sum(t.numel() * t.element_size() for t in h_in.values()) + h_q.numel() * 2
-    d2h = h_out.numel() * 2 + h_lse.numel() * 4 + sum(t.numel() * t.element_size() for t in outs)
+    sets = []
+    for n in range(2):
+        d_in = {k_: t.to(dev) for k_, t in h_in.items()}
+        q = torch.empty_like(r["q"])
+        sel = ctx.alloc_selection(wl.R, wl.N, r["cap"])
+        acc = ctx.alloc_accept(wl.R, r["cap"])
+        out, lse = torch.zeros_like(r["out"]), torch.zeros_like(r["lse"])
+        outs = [out, lse, acc.accept_len, acc.accept_idx, acc.bonus_token, acc.new_len, sel.n_selected]
+        h_outs = [torch.empty_like(t, device="cpu").pin_memory() for t in outs]
+        ev = [torch.cuda.Event() for _ in range(3)]  # upload done, kernels done, download done
+        sets.append(dict(d_in=d_in, q=q, bufs=(sel, acc, out, lse), outs=outs, h_outs=h_outs, ev=ev))
+    h2d = sum(t.numel() * t.element_size() for t in h_in.values()) + h_q.numel() * h_q.element_size()
+    d2h = sum(t.numel() * t.element_size() for t in sets[0]["outs"])
+    s_up, s_run, s_down = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
 
-    def one():
-        for k_, t in h_in.items():
-            d_in[k_].copy_(t, non_blocking=True)
-        d_q.copy_(h_q, non_blocking=True)
-        r["step"](d_in, None, d_q)
-        h_out.copy_(r["out"], non_blocking=True)
-        h_lse.copy_(r["lse"], non_blocking=True)
-        for ht, t in zip(h_outs, outs):
-            ht.copy_(t, non_blocking=True)
-        torch.cuda.synchronize()
+    def one(i):
+        st = sets[i % 2]
+        up, run, down = st["ev"]
+        with torch.cuda.stream(s_up):
+            s_up.wait_event(run)          # the kernels of step i-2 have read this set's inputs
+            for k_, t in h_in.items():
+                st["d_in"][k_].copy_(t, non_blocking=True)
+            st["q"].copy_(h_q, non_blocking=True)
+            up.record(s_up)
+        with torch.cuda.stream(s_run):
+            s_run.wait_event(up)
+            s_run.wait_event(down)        # the results of step i-2 have left this set's output buffers
+            r["step"](st["d_in"], None, st["q"], st["bufs"])
+            run.record(s_run)
+        with torch.cuda.stream(s_down):
+            s_down.wait_event(run)
+            for ht, t in zip(st["h_outs"], st["outs"]):
+                ht.copy_(t, non_blocking=True)
+            down.record(s_down)
 
-    for _ in range(max(1, args.warmup // 2)):
-        one()
+    for i in range(max(2, args.warmup // 2)):
+        one(i)
     r["barrier"]()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
-        one()
+    for i in range(args.steps):
+        one(i)
     r["barrier"]()
     dt = time.perf_counter() - t0
+    n_dev = int(sets[(args.steps - 1) % 2]["h_outs"][6].item())
+    assert n_dev == r["n_sel"], (n_dev, r["n_sel"])  # the downloaded result is the step's
     return dt, int(h2d), int(d2h)
 
 
