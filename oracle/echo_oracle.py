@@ -95,6 +95,60 @@ def select(cand_offsets, S, depth, cut, budget, w_max, static_k=0):
     return sorted((i, j) for (_, _, i, j) in elig[:max(0, budget)])
 
 
+# ---------------------------------------------------------------- O3' (NEXT-1): Algorithm 1 as printed
+def select_alg1(cand_offsets, S, depth, depth_mask, log_tau, budget, w_max):
+    """Algorithm 1, followed line by line in the paper's order (readings R:L-1..L-4):
+    Phase 1 walks the depths; at each depth the active requests are visited in request order while budget is left;
+    a request whose gate passes (or whose depth is not gated) appends its level -- the candidate tree already holds
+    the W_topk drafted nodes of that level (S:G-9) -- and pays for it; one whose gate fails leaves active_set for
+    trunc_set.  Phase 2 visits trunc_set in insertion order and widens each by up to W_max nodes of its truncation
+    level.  The cap of Eq. 4 is never exceeded: a level (or a widening) that does not fit is granted best-first by
+    (S desc, node asc) as far as the budget goes (R:L-1).  Paper depth d = 1 is depth 0 here (S:G-1).
+    Returns (sorted list of (request, node), cut depth per request for the requests that were truncated)."""
+    R = len(cand_offsets) - 1
+    G = [[] for _ in range(R)]
+    budget = max(0, int(budget))
+    active = list(range(R))
+    trunc = []
+    cut = {}
+    d = -1
+    while budget > 0 and active:                       # l.5
+        d += 1                                         # l.6
+        if d >= 32:
+            break
+        for i in list(active):                         # l.7, request order
+            if budget <= 0:
+                break
+            b, e = int(cand_offsets[i]), int(cand_offsets[i + 1])
+            lvl = [j for j in range(e - b) if depth[b + j] == d]
+            if not lvl:                                # R:L-2: the drafted tree ends here; nothing to extend or widen
+                active.remove(i)
+                continue
+            if (depth_mask >> d) & 1:                  # l.8
+                m = max(S[b + j] for j in lvl)
+                is_pass = bool(np.float32(m) > np.float32(log_tau[d]))
+            else:
+                is_pass = True
+            if is_pass:                                # l.9-11
+                lvl.sort(key=lambda j: (-float(S[b + j]), j))
+                grant = lvl[:budget]
+                G[i] += grant
+                budget -= len(grant)
+            else:                                      # l.12-13
+                active.remove(i)
+                trunc.append(i)
+                cut[i] = d
+    for i in trunc:                                    # l.18-21 (garbled in the paper: R:L-4)
+        if budget <= 0:
+            break
+        b, e = int(cand_offsets[i]), int(cand_offsets[i + 1])
+        lvl = sorted([j for j in range(e - b) if depth[b + j] == cut[i]], key=lambda j: (-float(S[b + j]), j))
+        w = min(budget, max(0, int(w_max)), len(lvl))
+        G[i] += lvl[:w]
+        budget -= w
+    return sorted((i, j) for i in range(R) for j in G[i]), cut
+
+
 # ---------------------------------------------------------------- O4 + O5 (S4, S5)
 def pack(cand_offsets, parent, depth, selected, R):
     """Flatten & Pack, Fig. 3(3): request asc, node asc (S:P-1); CSR offsets,
@@ -127,15 +181,19 @@ def pack(cand_offsets, parent, depth, selected, R):
                 sel_depth=np.asarray(sel_depth, np.uint8), anc_mask=anc, masks=masks)
 
 
-def gate_select(cand_offsets, parent, logq, depth_mask, log_tau, w_max, budget, static_k=0):
-    """S1-S5 end to end (what `echo_gate_select` must reproduce bit-exactly)."""
+def gate_select(cand_offsets, parent, logq, depth_mask, log_tau, w_max, budget, static_k=0, schedule=0):
+    """S1-S5 end to end (what `echo_gate_select` must reproduce bit-exactly).  schedule 0 = global top-B
+    (north_star, S:G-10); 1 = Algorithm 1 as printed (NEXT-1); `cut_depth` is the gate's verdict in both."""
     R = len(cand_offsets) - 1
     S, depth = path_scores(cand_offsets, parent, logq)
     if static_k > 0:
         cut = np.full(R, INT32_MAX, np.int32)
     else:
         cut = gate_cut_depth(cand_offsets, S, depth, depth_mask, log_tau)
-    sel = select(cand_offsets, S, depth, cut, budget, w_max, static_k)
+    if schedule == 1 and static_k <= 0:
+        sel, _ = select_alg1(cand_offsets, S, depth, depth_mask, log_tau, budget, w_max)
+    else:
+        sel = select(cand_offsets, S, depth, cut, budget, w_max, static_k)
     out = pack(cand_offsets, parent, depth, sel, R)
     out.update(path_score=S, cand_depth=depth, cut_depth=cut)
     return out
