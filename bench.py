@@ -184,7 +184,10 @@ def run_gpu(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=dev)
     build.build_library()
     wl = sharding.rank_workload(args.config, rank, static=args.static, gated=not args.static)
+    if args.gating != "sparse" and not args.static:
+        wl.gate = wl.gate.ablation(args.gating)
     g = wl.gate
+    schedule = {"topb": echo.SCHED_TOPB, "alg1": echo.SCHED_ALG1}[args.schedule]
     cap = wl.capacity()
     ctx = echo.EchoContext(local_rank, 0)
     ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq)
@@ -207,7 +210,8 @@ def run_gpu(args, rank, world, local_rank):
 
     def gate(din, sel_=None):
         return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
-                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel_ or sel)
+                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel_ or sel,
+                               schedule=schedule)
 
     gate(d_in)
     sel_h = sel.to_host()
@@ -339,6 +343,10 @@ def main():
     ap.add_argument("--ref-nodes", type=int, default=32, help="--impl reference: packed nodes of oracle attention per step (~0.75 s)")
     ap.add_argument("--baseline-nodes", type=int, default=512, help="cpu_baseline leg: packed nodes of oracle attention (~12 s once)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--schedule", default="topb", choices=["topb", "alg1"],
+                    help="topb: global top-B (north_star); alg1: Algorithm 1 as printed (SURVEY 8(f) NEXT-1)")
+    ap.add_argument("--gating", default="sparse", choices=["sparse", "dense", "fixed"],
+                    help="the paper's ablation variants (PAPER.md:254-258): gate every depth / one threshold")
     ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -374,7 +382,9 @@ def main():
         line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else ""), "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
+                "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
+                           + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
+                           "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
                            "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],

@@ -91,6 +91,9 @@ typedef struct {
   const float* logq;           /* dev [N], natural log of the draft confidence q(x|h), <= 0 (R:G-2) */
 } EchoTrees;
 
+#define ECHO_SCHED_TOPB 0
+#define ECHO_SCHED_ALG1 1
+
 /* Gate and scheduler parameters: Alg. 1 inputs (K_max, D_sig, tau, W_max). */
 typedef struct {
   uint32_t depth_mask; /* bit d set <=> d in D_sig (Eq. 7) */
@@ -98,6 +101,10 @@ typedef struct {
   int32_t w_max;       /* Phase-2 width cap per truncated request; 0 = no widening */
   int32_t budget;      /* K_max >= 0 (Eq. 4) */
   int32_t static_k;    /* 0 = elastic global top-B; >0 = per-request top-static_k, gates off (R:G-15) */
+  int32_t schedule;    /* ECHO_SCHED_TOPB: global top-B by path score inside a tier (north_star, R:G-10);
+                          ECHO_SCHED_ALG1: Algorithm 1 as printed, P:127-160 -- Phase 1 depth by depth, request order
+                          inside a depth, a level best-first by (S desc, node asc); Phase 2 over the truncated
+                          requests in truncation order (R:L-1..L-4).  Ignored when static_k > 0. */
 } EchoGate;
 
 /* Packed ragged batch ("Flatten & Pack", Fig. 3(3)): request asc, node asc (R:P-1). */

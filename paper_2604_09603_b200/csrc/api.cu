@@ -108,6 +108,7 @@ int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSe
   if (!ctx || !t || !g || !o) return ECHO_ERR_INVALID_ARG;
   if (t->num_requests < 0 || t->total_cand < 0 || t->max_cand_per_req < 0) return ECHO_ERR_INVALID_ARG;
   if (g->budget < 0 || g->w_max < 0 || g->static_k < 0 || o->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->schedule != ECHO_SCHED_TOPB && g->schedule != ECHO_SCHED_ALG1) return ECHO_ERR_INVALID_ARG;
   if (t->max_cand_per_req > ECHO_MAX_CAND) return ECHO_ERR_UNSUPPORTED;
   if (!t->cand_offsets || !o->n_selected || !o->sel_offsets || !o->cut_depth) return ECHO_ERR_INVALID_ARG;
   if (t->total_cand > 0 && (!t->parent || !t->logq || !o->path_score || !o->cand_depth)) return ECHO_ERR_INVALID_ARG;

@@ -16,6 +16,7 @@ struct GateParams {
   float log_tau[32];
   int32_t w_max;
   int32_t static_k;
+  int32_t schedule;
 };
 
 __device__ __forceinline__ float f32_unordered(uint32_t o) {
@@ -29,6 +30,15 @@ constexpr uint64_t KEY_INELIGIBLE = ~0ull;
 // bits 31..62, global candidate index (monotone in (request, node)) in bits 0..30.
 __device__ __forceinline__ uint64_t make_key(int tier, float S, int g) {
   return ((uint64_t)tier << 63) | ((uint64_t)(~f32_ordered(S)) << 31) | (uint64_t)(uint32_t)g;
+}
+
+// ECHO_SCHED_ALG1 (Algorithm 1 as printed): the grants of Phase 1 (depth by depth,
+// request order inside a depth, a level best-first) and then Phase 2 (truncated requests in the order they were
+// truncated, the W_max best nodes of the truncation level) are, read as one sequence, the eligible nodes sorted by
+// (phase, depth, request, rank in level); taking the first K_max of that order is the algorithm, including the
+// level that only partly fits (readings R:L-1..L-4).
+__device__ __forceinline__ uint64_t make_key_alg1(int phase, int depth, int request, int rank) {
+  return ((uint64_t)phase << 63) | ((uint64_t)depth << 56) | ((uint64_t)(uint32_t)request << 16) | (uint64_t)rank;
 }
 
 __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
@@ -98,6 +108,13 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
       int rank = 0;  // per-request top-static_k by (S desc, node asc) (R:G-15)
       for (int t = 0; t < C; ++t) rank += (s_S[t] > S) || (s_S[t] == S && t < j);
       if (rank < gp.static_k) key = make_key(0, 0.0f, b + j);
+    } else if (gp.schedule == ECHO_SCHED_ALG1) {
+      if (d <= cut) {
+        int rank = 0;  // position in the level by (S desc, node asc)
+        for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
+        if (d < cut) key = make_key_alg1(0, d, i, rank);
+        else if (rank < gp.w_max) key = make_key_alg1(1, d, i, rank);
+      }
     } else if (d < cut) {
       key = make_key(0, S, b + j);  // tier 0: depth extension
     } else if (d == cut) {
@@ -337,6 +354,7 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
   for (int d = 0; d < 32; ++d) gp.log_tau[d] = g->log_tau[d] + 0.0f;  // canonicalise -0 (R:G-13)
   gp.w_max = g->w_max;
   gp.static_k = g->static_k;
+  gp.schedule = g->schedule;
   if (R > 0) {
     k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gp, o->path_score,
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libecho.so")
 ECHO_OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5
 OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS = 1, 2, 3
+SCHED_TOPB, SCHED_ALG1 = 0, 1  # EchoGate.schedule: global top-B (north_star) / Algorithm 1 as printed
 ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
 MAX_ACCEPT = 32
 CUT_NEVER = 0x7FFFFFFF
@@ -35,7 +36,7 @@ class EchoTrees(C.Structure):
 
 class EchoGate(C.Structure):
     _fields_ = [("depth_mask", C.c_uint32), ("log_tau", C.c_float * 32), ("w_max", C.c_int32),
-                ("budget", C.c_int32), ("static_k", C.c_int32)]
+                ("budget", C.c_int32), ("static_k", C.c_int32), ("schedule", C.c_int32)]
 
 
 class EchoSelection(C.Structure):
@@ -267,7 +268,7 @@ class EchoContext:
 
     def gate_select(self, cand_offsets, parent, logq, depth_mask: int, log_tau, w_max: int, budget: int,
                     static_k: int = 0, capacity: Optional[int] = None, max_cand: int = 128,
-                    out: Optional[Selection] = None) -> Selection:
+                    out: Optional[Selection] = None, schedule: int = 0) -> Selection:
         """echo_gate_select.  cand_offsets/parent int32 and logq float32 device tensors."""
         R = cand_offsets.numel() - 1
         N = parent.numel()
@@ -281,7 +282,7 @@ class EchoContext:
         lt = np.asarray(log_tau, np.float32)
         for d in range(32):
             g.log_tau[d] = float(lt[d])
-        g.w_max, g.budget, g.static_k = int(w_max), int(budget), int(static_k)
+        g.w_max, g.budget, g.static_k, g.schedule = int(w_max), int(budget), int(static_k), int(schedule)
         cs = sel.c_struct()
         self._check(self.lib.echo_gate_select(self._h, C.byref(trees), C.byref(g), C.byref(cs), self._stream()))
         return sel

@@ -49,6 +49,26 @@ class Gate:
             g.log_tau[d] = np.float32(np.log(np.float64(t))) if t > 0 else np.float32(-np.inf)
         return g
 
+    def taus(self) -> Dict[int, float]:
+        return {d: float(np.exp(np.float64(self.log_tau[d]))) for d in range(32) if (self.depth_mask >> d) & 1}
+
+    def ablation(self, variant: str, max_depth: int = 8) -> "Gate":
+        """The two simplified variants of the paper's ablation, which the paper does not
+        parametrise (readings R:L-5, L-6): "dense" gates every depth below `max_depth` with the calibrated
+        thresholds interpolated linearly over depth (held constant outside the calibrated range); "fixed" keeps the
+        sweet-spot depths and uses one threshold, the median of the calibrated ones."""
+        t = self.taus()
+        if variant == "sparse" or not t:
+            return self.replace()
+        ds = sorted(t)
+        if variant == "dense":
+            new = {d: float(np.interp(d, ds, [t[x] for x in ds])) for d in range(max_depth)}
+        elif variant == "fixed":
+            new = {d: float(np.median([t[x] for x in ds])) for d in ds}
+        else:
+            raise ValueError(variant)
+        return Gate.from_taus(new, self.w_max, self.budget, self.static_k)
+
     def replace(self, **kw) -> "Gate":
         g = Gate(self.depth_mask, self.log_tau.copy(), self.w_max, self.budget, self.static_k)
         for k, v in kw.items():

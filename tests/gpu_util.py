@@ -23,10 +23,10 @@ def get_ctx():
     return ctx
 
 
-def run_gate_select(ctx, wl, gate=None, capacity=None):
+def run_gate_select(ctx, wl, gate=None, capacity=None, schedule=0):
     g = gate or wl.gate
     return ctx.gate_select(dev(wl.cand_offsets), dev(wl.parent), dev(wl.logq), g.depth_mask, g.log_tau, g.w_max,
-                           g.budget, g.static_k, capacity=capacity, max_cand=max(1, wl.max_cand))
+                           g.budget, g.static_k, capacity=capacity, max_cand=max(1, wl.max_cand), schedule=schedule)
 
 
 def make_kv(wl, k, v):

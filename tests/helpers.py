@@ -18,10 +18,10 @@ def torch_bf16_to_bits(t):
     return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
 
 
-def oracle_gate_select(orc, wl, gate=None):
+def oracle_gate_select(orc, wl, gate=None, schedule=0):
     g = gate or wl.gate
     return orc.gate_select(wl.cand_offsets, wl.parent, wl.logq, g.depth_mask, g.log_tau, g.w_max,
-                           g.budget, g.static_k)
+                           g.budget, g.static_k, schedule=schedule)
 
 
 def packed_tokens(wl, sel):

@@ -220,3 +220,45 @@ def test_argmax_ties_lowest_index():
     want = orc.argmax_bf16(torch_bf16_to_bits(lg[:n]), V)
     np.testing.assert_array_equal(got, want)
     assert got[0] == 0 and got[1] == 300 and got[2] == 999 and got[3] < 1000 and got[4] == 5
+
+
+# ---------------------------------------------------------------- NEXT-1: Algorithm 1 as printed (schedule = ALG1)
+A1 = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "alg1.json")))
+
+
+@pytest.mark.parametrize("B", list(range(0, 11)))
+def test_alg1_hand_example_all_budgets(B):
+    from paper_2604_09603_b200 import echo
+    ctx = get_ctx()
+    offs = np.asarray(GOLD["cand_offsets"], np.int32)
+    parent = np.asarray(GOLD["parent"], np.int32)
+    logq = np.asarray(GOLD["logq"], np.float32)
+    lt = np.zeros(32, np.float32)
+    sel = ctx.gate_select(dev(offs), dev(parent), dev(logq), 0, lt, 0, B, capacity=16, schedule=echo.SCHED_ALG1)
+    got = sel.to_host()
+    want = orc.gate_select(offs, parent, logq, 0, lt, 0, B, schedule=1)
+    assert_selection_equal(got, want)
+    order = sorted(tuple(x) for x in A1["grant_order"][:B])
+    assert sorted(zip(got["sel_req"].tolist(), got["sel_node"].tolist())) == order
+
+
+@pytest.mark.parametrize("cfg,gated,R", [(0, True, None), (0, False, None), (1, True, None), (2, True, None),
+                                         (3, True, None), (4, True, None), (2, False, 7)])
+def test_alg1_configs(cfg, gated, R):
+    from paper_2604_09603_b200 import echo
+    ctx = get_ctx()
+    wl = W.make_config(cfg, gated=gated, R=R)
+    sel = run_gate_select(ctx, wl, schedule=echo.SCHED_ALG1)
+    want = oracle_gate_select(orc, wl, schedule=1)
+    assert_selection_equal(sel.to_host(), want)
+    assert ctx.device_status() == 0
+
+
+@pytest.mark.parametrize("budget", [0, 1, 7, 40, 95, 96, 500])
+def test_alg1_budget_edges_and_widening(budget):
+    from paper_2604_09603_b200 import echo
+    ctx = get_ctx()
+    wl = W.make_config(0, gated=True)
+    g = wl.gate.replace(budget=budget)
+    sel = run_gate_select(ctx, wl, g, capacity=max(budget, 1), schedule=echo.SCHED_ALG1)
+    assert_selection_equal(sel.to_host(), oracle_gate_select(orc, wl, g, schedule=1))
