@@ -194,3 +194,47 @@ def test_attn_full_size_bench_configuration(cfg, static):
     rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(128)] + [(0, 0), (n - 1, wl.Hq - 1)]
     _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
     assert ctx.device_status() == 0
+
+
+def test_step_is_cuda_graph_capturable():
+    """The three calls never synchronise or read device results on the host (include/echo.h): one verify step is
+    captured into a CUDA graph (the paper serves under CUDA graphs) and replayed on new Q; results equal the
+    eager run bit for bit."""
+    import torch
+    wl = W.make_config(1, R=4, gated=True)
+    ctx, sel, want_sel, q, k, v = _setup(wl)
+    from paper_2604_09603_b200 import echo
+    ctx.set_option(echo.OPT_ATTN_PATH, 0)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 0)
+    kv = make_kv(wl, k, v)
+    g = wl.gate
+    cap = sel.capacity
+    d_off, d_par, d_lq = dev(wl.cand_offsets), dev(wl.parent), dev(wl.logq)
+    out = torch.zeros_like(q)
+    lse = torch.zeros(cap, wl.Hq, dtype=torch.float32, device="cuda")
+
+    def step():
+        ctx.gate_select(d_off, d_par, d_lq, g.depth_mask, g.log_tau, g.w_max, g.budget, g.static_k, capacity=cap,
+                        max_cand=wl.max_cand, out=sel)
+        ctx.verify_attn(sel, kv, q, SM_SCALE, out=out, lse=lse)
+
+    step()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        step()  # warm-up on the capture stream
+        side.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+    torch.cuda.synchronize()
+    q.copy_(torch.randn_like(q))
+    out.zero_(); lse.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    out_g, lse_g = out.clone(), lse.clone()
+    out.zero_(); lse.zero_()
+    step()
+    torch.cuda.synchronize()
+    assert torch.equal(out_g, out) and torch.equal(lse_g, lse)
+    _compare(wl, want_sel, q, k, v, out_g, lse_g)
