@@ -334,3 +334,45 @@ def compact_kv(sel, acc, k_pool_bits, v_pool_bits, page_table, prefix_len, R):
             k_pool_bits[:, d // PAGE, :, d % PAGE, :] = tmp[t][0]
             v_pool_bits[:, d // PAGE, :, d % PAGE, :] = tmp[t][1]
     return dict(slot_src=slot_src, slot_dst=slot_dst, new_len=new_len)
+
+
+# ---------------------------------------------------------------- O11 (NEXT-3): warm-up calibration of the gates
+def calibrate(depth, conf, accepted, delta):
+    """Offline calibration, P:115 (and P:446): per depth d, the separability of the layer confidences c_{i,d} of
+    accepted versus rejected samples is the AUC (Hanley & McNeil 1982: the Wilcoxon / Mann-Whitney statistic,
+    AUC = (#{c_pos > c_neg} + 0.5 #{c_pos == c_neg}) / (n_pos n_neg)); sweet spots D_sig = {d : AUC_d > delta};
+    tau_d "maximises the separation between the two distributions": the observed value v that maximises
+    J(v) = #pos(c > v)/n_pos - #neg(c > v)/n_neg (Youden's J = the Kolmogorov-Smirnov distance of the two empirical
+    CDFs; the gate is c > tau, Eq. 7), the smallest such v on ties (readings R:K-1..K-3).  Plain
+    definitions on exact integers; a depth with no accepted or no rejected sample gets AUC 0.5 and tau 0 and is
+    never a sweet spot.  Returns dict(auc f64[32], tau f32[32], n_pos, n_neg i64[32], depth_mask)."""
+    depth = np.asarray(depth).astype(np.int64)
+    conf = np.asarray(conf, np.float32)
+    accepted = np.asarray(accepted).astype(bool)
+    auc = np.full(32, 0.5, np.float64)
+    tau = np.zeros(32, np.float32)
+    n_pos = np.zeros(32, np.int64)
+    n_neg = np.zeros(32, np.int64)
+    mask = 0
+    for d in range(32):
+        m = depth == d
+        pos = np.sort(conf[m & accepted])
+        neg = np.sort(conf[m & ~accepted])
+        n_pos[d], n_neg[d] = len(pos), len(neg)
+        if len(pos) == 0 or len(neg) == 0:
+            continue
+        less = np.searchsorted(neg, pos, side="left").astype(np.int64)      # negatives strictly below each positive
+        leq = np.searchsorted(neg, pos, side="right").astype(np.int64)
+        two_u = int((2 * less + (leq - less)).sum())                         # 2 x the Mann-Whitney U
+        auc[d] = float(two_u) / float(2 * len(pos) * len(neg))
+        best_v, best_num = None, None
+        for v in np.unique(np.concatenate([pos, neg])):                      # ascending: the first maximum is kept
+            p_gt = len(pos) - int(np.searchsorted(pos, v, side="right"))
+            n_gt = len(neg) - int(np.searchsorted(neg, v, side="right"))
+            num = p_gt * len(neg) - n_gt * len(pos)                          # J(v) n_pos n_neg, an integer
+            if best_num is None or num > best_num:
+                best_v, best_num = v, num
+        tau[d] = best_v
+        if auc[d] > delta:
+            mask |= 1 << d
+    return dict(auc=auc, tau=tau, n_pos=n_pos, n_neg=n_neg, depth_mask=mask)
