@@ -269,7 +269,22 @@ def run_gpu(args, rank, world, local_rank):
     t_attn = float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
     t_gate = float(np.mean([a.elapsed_time(b) for a, b in gate_ev]))
     accepted = int(acc.accept_len[:wl.R].sum().item())
-    return dict(torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
+    # the step before the path: warm-up calibration of the gates, timed outside the step
+    calib_us = None
+    if rank == 0 and args.calibrate_samples > 0:
+        tr = W.draw_calibration_traces(np.random.default_rng(W.SEED_BASE), args.calibrate_samples)
+        d_tr = [d(a) for a in tr]
+        for _ in range(3):
+            ctx.calibrate(*d_tr, 0.65)
+        c0, c1 = ev(), ev()
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(10):
+            ctx.calibrate(*d_tr, 0.65)
+        c1.record()
+        torch.cuda.synchronize()
+        calib_us = c0.elapsed_time(c1) * 100.0
+    return dict(calib_us=calib_us, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
                 accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
                 out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
 
@@ -347,6 +362,8 @@ def main():
                     help="topb: global top-B (north_star); alg1: Algorithm 1 as printed (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--gating", default="sparse", choices=["sparse", "dense", "fixed"],
                     help="the paper's ablation variants (PAPER.md:254-258): gate every depth / one threshold")
+    ap.add_argument("--calibrate-samples", type=int, default=160000,
+                    help="warm-up traces for echo_calibrate, timed outside the step (0 = skip)")
     ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -388,7 +405,8 @@ def main():
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
                            "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],
-                           "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12},
+                           "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12,
+                           "calibrate_us": r["calib_us"], "calibrate_samples": args.calibrate_samples},
                 "accepted_tokens_per_s": acc_all * args.steps / (ms * 1e-3),
                 "roofline": {"bound": "tensor" if tensor_bound else "hbm", "achieved": tflops if tensor_bound else achieved,
                              "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",

@@ -46,6 +46,8 @@ typedef enum {
 #define ECHO_DEV_BAD_LOGQ 2u     /* logq > 0 or NaN */
 #define ECHO_DEV_DEPTH_OVERFLOW 4u /* a candidate deeper than 31 */
 #define ECHO_DEV_PAGE_OVERFLOW 8u  /* P_i + K_i needs more than max_pages_per_req pages */
+#define ECHO_DEV_BAD_TRACE 16u     /* echo_calibrate: depth >= 32 or a confidence outside [0, 1] / NaN (sample skipped) */
+#define ECHO_DEV_CALIB_OVERFLOW 32u /* echo_calibrate: more than ECHO_CALIB_MAX_PER_DEPTH samples at one depth (rest dropped) */
 
 /* test / tuning hooks for echo_set_option */
 #define ECHO_OPT_FORCE_SPLITS 1   /* >0: split every KV stream into exactly this many parts (<= 16) */
@@ -54,6 +56,8 @@ typedef enum {
 
 #define ECHO_MAX_CAND 128   /* C_i <= 128 candidates per request (R:G-14) */
 #define ECHO_MAX_DEPTH 32   /* depth < 32 (R:G-14) */
+#define ECHO_CALIB_MAX_PER_DEPTH 24576 /* echo_calibrate sorts one depth's samples in shared memory */
+#define ECHO_CALIB_WORKSPACE_BYTES (256 + (size_t)ECHO_MAX_DEPTH * ECHO_CALIB_MAX_PER_DEPTH * 4)
 #define ECHO_MAX_ACCEPT 32  /* an accepted path has <= 32 nodes (one per depth) */
 #define ECHO_CUT_NEVER 0x7fffffff
 #define ECHO_PROF_CTAS 256  /* echo_debug_wait_prof: rows (persistent CTAs) ... */
@@ -180,6 +184,30 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
  * P_i .. P_i+L-1, every read before any write to the same slot column (R:C-6). */
 int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t num_requests,
                 EchoPagedKV* kv, EchoAccept* out, echo_stream_t stream);
+
+/* ---- warm-up calibration of the gates ------------------------------ */
+/* Traces collected during warm-up: one sample per (request, depth) with the layer confidence
+ * c_{i,d} (Eq. 6, a probability in [0, 1]) and whether the node the target then took at that depth was accepted. */
+typedef struct {
+  int64_t num_samples;     /* M >= 0 */
+  const uint8_t* depth;    /* dev [M], < 32 */
+  const float* conf;       /* dev [M], in [0, 1], no NaN */
+  const uint8_t* accepted; /* dev [M], 0 / 1 */
+} EchoTraces;
+typedef struct {
+  double* auc;          /* dev [32]: AUC_d, 0.5 where a class is missing */
+  float* tau;           /* dev [32]: tau_d (an observed confidence), 0 where a class is missing */
+  int32_t* n_pos;       /* dev [32]: accepted samples at depth d */
+  int32_t* n_neg;       /* dev [32]: rejected samples at depth d */
+  uint32_t* depth_mask; /* dev [1]: bit d <=> d in D_sig */
+} EchoCalibration;
+/* "Offline Calibration": per depth, AUC_d of the confidences of accepted vs rejected samples
+ * (Hanley & McNeil 1982: (#{c+ > c-} + 0.5 #{c+ == c-}) / (n+ n-), computed exactly on integers and divided once in
+ * fp64); D_sig = {d : both classes present and AUC_d > delta}; tau_d = the smallest observed confidence v that
+ * maximises J(v) = #{c+ > v}/n+ - #{c- > v}/n- (the gate is c > tau, Eq. 7; readings R:K-1..K-3).  The caller turns
+ * tau into EchoGate.log_tau on the host (R:G-2).  Needs a context workspace of ECHO_CALIB_WORKSPACE_BYTES; at most
+ * ECHO_CALIB_MAX_PER_DEPTH samples per depth (more: status bit, the excess is dropped).  Asynchronous on `stream`. */
+int echo_calibrate(EchoCtx* ctx, const EchoTraces* traces, double delta, EchoCalibration* out, echo_stream_t stream);
 
 #ifdef __cplusplus
 }

@@ -145,6 +145,15 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
   return launch_verify_attn(ctx, sel, kv, layer, Hq, R, q, out, lse, sm_scale, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int echo_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibration* o, echo_stream_t stream) {
+  if (!ctx || !t || !o) return ECHO_ERR_INVALID_ARG;
+  if (t->num_samples < 0 || !(delta == delta)) return ECHO_ERR_INVALID_ARG;
+  if (t->num_samples > 0 && (!t->depth || !t->conf || !t->accepted)) return ECHO_ERR_INVALID_ARG;
+  if (!o->auc || !o->tau || !o->n_pos || !o->n_neg || !o->depth_mask) return ECHO_ERR_INVALID_ARG;
+  if (misaligned(o->auc, 8) || misaligned(t->conf, 4)) return ECHO_ERR_INVALID_ARG;
+  return launch_calibrate(ctx, t, delta, o, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t R, EchoPagedKV* kv,
                 EchoAccept* out, echo_stream_t stream) {
   if (!ctx || !sel || !res || !out) return ECHO_ERR_INVALID_ARG;

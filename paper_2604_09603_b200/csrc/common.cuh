@@ -1,5 +1,6 @@
 // Shared internals of libecho.so (CUDA path only; the CPU oracle shares nothing with this).
 #pragma once
+#include <climits>
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <stdint.h>
@@ -34,6 +35,7 @@ static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; 
 
 // launchers implemented by the .cu files
 int launch_gate_select(EchoCtx*, const EchoTrees*, const EchoGate*, EchoSelection*, cudaStream_t);
+int launch_calibrate(EchoCtx*, const EchoTraces*, double delta, EchoCalibration*, cudaStream_t);
 int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
                        const void* q, void* out, float* lse, float sm_scale, cudaStream_t);
 int launch_accept(EchoCtx*, const EchoSelection*, const EchoVerifyResult*, int32_t R, EchoPagedKV*, EchoAccept*,

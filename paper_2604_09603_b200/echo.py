@@ -26,7 +26,8 @@ CUT_NEVER = 0x7FFFFFFF
 DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
-           "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept"]
+           "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept",
+           "echo_calibrate"]
 
 
 class EchoTrees(C.Structure):
@@ -64,6 +65,19 @@ class EchoAccept(C.Structure):
                 ("slot_dst", C.c_void_p), ("target_token_out", C.c_void_p)]
 
 
+class EchoTraces(C.Structure):
+    _fields_ = [("num_samples", C.c_int64), ("depth", C.c_void_p), ("conf", C.c_void_p), ("accepted", C.c_void_p)]
+
+
+class EchoCalibration(C.Structure):
+    _fields_ = [("auc", C.c_void_p), ("tau", C.c_void_p), ("n_pos", C.c_void_p), ("n_neg", C.c_void_p),
+                ("depth_mask", C.c_void_p)]
+
+
+CALIB_MAX_PER_DEPTH = 24576
+CALIB_WORKSPACE_BYTES = 256 + 32 * CALIB_MAX_PER_DEPTH * 4
+DEV_BAD_TRACE, DEV_CALIB_OVERFLOW = 16, 32
+
 _lib = None
 
 
@@ -93,6 +107,8 @@ def load_library():
     lib.echo_set_option.restype = C.c_int
     lib.echo_debug_wait_prof.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
     lib.echo_debug_wait_prof.restype = C.c_int
+    lib.echo_calibrate.argtypes = [C.c_void_p, P(EchoTraces), C.c_double, P(EchoCalibration), C.c_void_p]
+    lib.echo_calibrate.restype = C.c_int
     lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
     lib.echo_gate_select.restype = C.c_int
     lib.echo_verify_attn.argtypes = [C.c_void_p, P(EchoSelection), P(EchoPagedKV), C.c_int32, C.c_int32,
@@ -309,6 +325,29 @@ class EchoContext:
                           torch.zeros(r, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(r, MAX_ACCEPT, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(max(1, capacity), **i32))
+
+    def calibrate(self, depth, conf, accepted, delta: float):
+        """echo_calibrate.  depth / accepted uint8 and conf float32 device tensors of M warm-up samples ->
+        dict of device tensors auc f64[32], tau f32[32], n_pos / n_neg i32[32], depth_mask i32[1] (bits)."""
+        import torch
+        if self.workspace_bytes < CALIB_WORKSPACE_BYTES:
+            torch.cuda.synchronize(self.device)
+            opts = self.get_options()
+            self.lib.echo_destroy(self._h)
+            self._h = C.c_void_p()
+            self._check(self.lib.echo_create(C.byref(self._h), self.device.index, CALIB_WORKSPACE_BYTES))
+            self.workspace_bytes = CALIB_WORKSPACE_BYTES
+            for k_, v_ in opts.items():
+                self.set_option(k_, v_)
+        d = self.device
+        out = dict(auc=torch.zeros(32, dtype=torch.float64, device=d), tau=torch.zeros(32, dtype=torch.float32, device=d),
+                   n_pos=torch.zeros(32, dtype=torch.int32, device=d), n_neg=torch.zeros(32, dtype=torch.int32, device=d),
+                   depth_mask=torch.zeros(1, dtype=torch.int32, device=d))
+        tr = EchoTraces(int(conf.numel()), _ptr(depth), _ptr(conf), _ptr(accepted))
+        oc = EchoCalibration(_ptr(out["auc"]), _ptr(out["tau"]), _ptr(out["n_pos"]), _ptr(out["n_neg"]),
+                             _ptr(out["depth_mask"]))
+        self._check(self.lib.echo_calibrate(self._h, C.byref(tr), C.c_double(delta), C.byref(oc), self._stream()))
+        return out
 
     def accept(self, sel: Selection, kv: PagedKV, draft_token, prev_token, target_token=None,
                target_logits=None, vocab: int = 0, out: Optional[Acceptance] = None,

@@ -383,3 +383,17 @@ def draw_logits(wl: Workload, sel_cand: np.ndarray, device: str = "cpu", ld: Opt
     bumped = (logits[rows[hit], tgt[hit]].float() + 8.0).to(torch.bfloat16)
     logits[rows[hit], tgt[hit]] = bumped
     return logits
+
+
+def draw_calibration_traces(rng, M: int, ties: bool = False, separation=(0.7, 0.1, 0.1, 0.3, 0.1, 0.6, 0.05, 0.0)):
+    """Warm-up traces for echo_calibrate (stand-in for the paper's warm-up runs): M samples of
+    (depth < 8, layer confidence in (0, 1], accepted).  Accepted samples draw Beta(2,2) shifted up by half the
+    depth's `separation`, rejected ones down, so depths 0 and 5 ("root and target depth") separate
+    well and the others do not.  `ties` rounds confidences to 1/64.  No method arithmetic here."""
+    sep = np.asarray(separation, np.float64)
+    depth = rng.integers(0, len(sep), M).astype(np.uint8)
+    acc = rng.random(M) < 0.4
+    conf = np.clip(rng.beta(2, 2, M) + sep[depth] * (acc - 0.5), 1e-6, 1.0)
+    if ties:
+        conf = np.maximum(np.round(conf * 64) / 64, 1.0 / 64)
+    return depth, conf.astype(np.float32), acc.astype(np.uint8)
