@@ -238,3 +238,31 @@ def test_step_is_cuda_graph_capturable():
     torch.cuda.synchronize()
     assert torch.equal(out_g, out) and torch.equal(lse_g, lse)
     _compare(wl, want_sel, q, k, v, out_g, lse_g)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_attn_second_layer_of_a_two_layer_pool(path):
+    """pools [2 layers][pages][Hkv][16][128]: attention over layer 1 reads layer 1's pages only (4-D tensor map
+    coordinate = ((layer * pages + page) * Hkv + head) * 2)."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(1, R=3, gated=True)
+    ctx = get_ctx()
+    sel = run_gate_select(ctx, wl)
+    want_sel = oracle_gate_select(orc, wl)
+    q, k, v = W.draw_qkv(wl, max(1, sel.capacity), device="cuda", num_layers=2)
+    ctx.set_option(echo.OPT_ATTN_PATH, path)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 0)
+    kv = make_kv(wl, k, v)
+    n = want_sel["n_selected"]
+    rng = np.random.default_rng(9)
+    rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(40)] + [(0, 0), (n - 1, wl.Hq - 1)]
+    qb, kb, vb = torch_bf16_to_bits(q), torch_bf16_to_bits(k), torch_bf16_to_bits(v)
+    for layer in (1, 0):
+        out, lse = ctx.verify_attn(sel, kv, q, SM_SCALE, layer=layer)
+        res = orc.verify_attn(want_sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, layer=layer,
+                              rows=rows)
+        o_gpu = bf16_bits_to_f32(torch_bf16_to_bits(out)).astype(np.float64)
+        l_gpu = lse.cpu().numpy().astype(np.float64)
+        assert max(np.abs(o_gpu[k_, h] - res[(k_, h)][0]).max() for (k_, h) in rows) <= TOL_O
+        assert max(abs(l_gpu[k_, h] - res[(k_, h)][1]) for (k_, h) in rows) <= TOL_LSE
+    assert ctx.device_status() == 0
