@@ -386,9 +386,12 @@ def main():
         tensor_bound = r["flops_alg"] / r["bytes_alg"] > tpeak * 1e12 / (peak * 1e9)
         tflops = r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")  # measured DRAM bytes per launch from the ncu --set full capture
         if os.path.exists(tp):
-            traffic = json.load(open(tp)).get(f"cfg{args.config}")
+            for ln in open(tp).read().splitlines()[1:]:
+                f = ln.split(",")
+                if f and f[0] == f"cfg{args.config}":
+                    traffic = int(f[1])
         wl = r["wl"]
         units = wl.R * wl.Hkv
         splits = args.splits or 1
