@@ -397,8 +397,8 @@ def main():
         splits = args.splits or 1
         if not args.splits:  # the library's split policy (csrc/verify_attn.cu), to count launches
             sms = torch.cuda.get_device_properties(0).multi_processor_count
-            cost = {s_: -(-units * s_ // sms) / s_ + 0.05 * s_ + (0.1 if s_ > 1 else 0.0) for s_ in (1, 2, 4, 8)}
-            splits = min(cost, key=lambda s_: (cost[s_], s_))
+            while splits < 8 and units * splits < sms:
+                splits *= 2
         launches = 3 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)  # gate 3, plan + attn, merge, accept, argmax
         line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,

@@ -93,6 +93,7 @@ __global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
     int32_t* __restrict__ accept_idx, int32_t* __restrict__ slot_src, int32_t* __restrict__ slot_dst) {
   __shared__ int s_L;
   __shared__ int s_src[ECHO_MAX_ACCEPT], s_dst[ECHO_MAX_ACCEPT];
+  pdl_wait();  // the attention kernel before this one reads the pools this kernel compacts in place
   const int i = blockIdx.x;
   const int b = sel_offsets[i], Ki = min(sel_offsets[i + 1] - b, ECHO_MAX_CAND);
   const int P = prefix_len[i];
@@ -205,12 +206,12 @@ int launch_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult
   }
   if (R > 0) {
     const bool have_pools = kv->k_pool && kv->v_pool;  // NULL pools: slot maps only, no copy
-    k_accept_compact<<<R, AC_THREADS, 0, st>>>(
+    ECHO_CUDA_TRY(ctx, launch_pdl(k_accept_compact, dim3(R), dim3(AC_THREADS), 0, st,
         sel->sel_offsets, sel->parent_local, sel->sel_depth, sel->anc_mask, res->draft_token, res->prev_token, tt,
         kv->page_table, kv->prefix_len, kv->max_pages_per_req, kv->num_kv_heads, kv->num_pages, kv->num_layers,
-        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->k_pool) : nullptr,
-        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->v_pool) : nullptr, out->accept_len, out->last_node,
-        out->bonus_token, out->new_len, out->accept_idx, out->slot_src, out->slot_dst);
+        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->k_pool) : (__nv_bfloat16*)nullptr,
+        have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->v_pool) : (__nv_bfloat16*)nullptr, out->accept_len, out->last_node,
+        out->bonus_token, out->new_len, out->accept_idx, out->slot_src, out->slot_dst));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

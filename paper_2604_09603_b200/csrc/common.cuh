@@ -34,6 +34,28 @@ struct EchoCtx {
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // launchers implemented by the .cu files
+// Programmatic dependent launch: the kernel may start while its predecessor on the stream is still running; it
+// must call pdl_wait() before touching anything the predecessor writes (or reads and this kernel overwrites).
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+#endif
+
 int launch_gate_select(EchoCtx*, const EchoTrees*, const EchoGate*, EchoSelection*, cudaStream_t);
 int launch_calibrate(EchoCtx*, const EchoTraces*, double delta, EchoCalibration*, cudaStream_t);
 int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,

@@ -52,6 +52,7 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
   __shared__ uint32_t s_lvlmax[ECHO_MAX_DEPTH];
   __shared__ int s_cut;
 
+  pdl_launch_dependents();
   const int i = blockIdx.x;
   const int b = cand_offsets[i];
   const int C = min(cand_offsets[i + 1] - b, ECHO_MAX_CAND);
@@ -148,6 +149,8 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(
   __shared__ int s_eligible;
   __shared__ int s_done;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_launch_dependents();
+  pdl_wait();  // keys come from k_score_gate
 
   // ---- S3: threshold T = budget-th smallest key (keys are unique => no ties to break) ----
   // Keys stay in registers across the passes when N <= SEL_THREADS * SEL_KPT (every config of BASELINE.json),
@@ -287,6 +290,8 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
   __shared__ int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks below are chains of dependent reads
   __shared__ uint32_t s_bal[4];
   const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_launch_dependents();
+  pdl_wait();  // threshold and offsets come from k_select
   {
     const int b = cand_offsets[r], C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
     const int base = sel_offsets[r];
@@ -360,11 +365,12 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);
   }
   const int budget = g->static_k > 0 ? N : g->budget;
-  k_select<<<1, SEL_THREADS, 0, st>>>(t->cand_offsets, keys, R, N, budget, o->n_selected, o->sel_offsets, threshold);
+  ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, N, budget,
+                                o->n_selected, o->sel_offsets, threshold));
   if (R > 0) {
-    k_pack<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, o->cand_depth, keys, threshold, o->capacity,
+    ECHO_CUDA_TRY(ctx, launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent, o->cand_depth, keys, threshold, o->capacity,
                                         o->sel_offsets, o->sel_node, o->sel_req, o->parent_local, o->sel_depth,
-                                        o->anc_mask);
+                                        o->anc_mask));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

@@ -161,20 +161,15 @@ int launch_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV
   const __nv_bfloat16* kp = reinterpret_cast<const __nv_bfloat16*>(kv->k_pool) + (size_t)layer * layer_elems;
   const __nv_bfloat16* vp = reinterpret_cast<const __nv_bfloat16*>(kv->v_pool) + (size_t)layer * layer_elems;
 
-  // split policy: the host knows only capacities (P_i, K_i are device-side).  With `units` = (request, KV head)
-  // streams and s splits the makespan is about ceil(units s / SMs) / s stream lengths; every split level costs
-  // per-item set-up and, beyond one, the partials and the merge launch.  Measured at cfg1 (256 units): one split
-  // 0.068 ms, two 0.107 ms, four 0.104 ms.  Long-tail balancing is the planner's job.
+  // split policy: the host knows only capacities (P_i, K_i are device-side).  Split the KV range only when there
+  // are fewer (request, KV head) streams than SMs, and then just enough to give every SM one: every split level
+  // costs per-item set-up, the fp32 partials and the merge launch, and the planner already balances whole items.
+  // Measured: cfg1 (256 streams) one split 0.068 ms, two 0.107 ms; cfg3 (512 streams) one 0.256 ms, two 0.312 ms.
   int splits = 1;
   if (ctx->opt_force_splits > 0) splits = (int)ctx->opt_force_splits;
   else {
     const long units = (long)R * Hkv;
-    double best = 1e30;
-    for (int s = 1; s <= 8; s *= 2) {
-      const long waves = (units * s + ctx->num_sms - 1) / ctx->num_sms;
-      const double cost = (double)waves / s + 0.05 * s + (s > 1 ? 0.1 : 0.0);
-      if (cost < best) { best = cost; splits = s; }
-    }
+    while (splits < 8 && units * splits < (long)ctx->num_sms) splits *= 2;
   }
   if (splits > 16) splits = 16;
   const size_t n_rows = (size_t)cap * Hq;

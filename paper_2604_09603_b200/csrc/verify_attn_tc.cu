@@ -261,6 +261,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cta = blockIdx.x, grid = gridDim.x;
+  pdl_launch_dependents();  // echo_accept's kernel may queue behind this one (it waits for our completion itself)
 
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();  // SW128 operand tiles need 1024-byte alignment
@@ -653,7 +654,8 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
                                                        int32_t* __restrict__ n_items) {
   __shared__ int s_cnt[PLAN_BUCKETS];
   __shared__ int s_warp[32];
-  asm volatile("griddepcontrol.launch_dependents;");  // let k_verify_attn_tc set itself up meanwhile
+  pdl_launch_dependents();  // let k_verify_attn_tc set itself up meanwhile
+  pdl_wait();               // sel_offsets come from echo_gate_select's kernels
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int b = tid; b < PLAN_BUCKETS; b += PLAN_THREADS) s_cnt[b] = 0;
   __syncthreads();
@@ -785,7 +787,8 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   uint8_t* plan = reinterpret_cast<uint8_t*>(ctx->workspace) + part_bytes;
   int32_t* n_items = reinterpret_cast<int32_t*>(plan);
   int4* items = reinterpret_cast<int4*>(plan + 256);
-  k_plan<<<1, PLAN_THREADS, 0, st>>>(sel->sel_offsets, kv->prefix_len, R, Hkv, G, splits, (int)max_items, items, n_items);
+  ECHO_CUDA_TRY(ctx, launch_pdl(k_plan, dim3(1), dim3(PLAN_THREADS), 0, st, sel->sel_offsets, kv->prefix_len, R, Hkv, G,
+                                splits, (int)max_items, items, n_items));
 
   static bool attr_set = false;
   if (!attr_set) {
