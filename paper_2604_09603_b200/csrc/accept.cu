@@ -180,12 +180,20 @@ __global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
     const int layer = col / (32 * Hkv);
     __nv_bfloat16* pool = kvsel ? v_pool : k_pool;
     uint4* base = reinterpret_cast<uint4*>(pool + (size_t)layer * num_pages * Hkv * PAGE * D);
-    for (int t = 0; t < L; ++t) {
-      const int s = s_src[t], d = s_dst[t];
-      if (s == d) continue;
-      const size_t so = (((size_t)(s / PAGE) * Hkv + head) * PAGE + (s % PAGE)) * (D * 2 / 16) + chunk;
-      const size_t dofs = (((size_t)(d / PAGE) * Hkv + head) * PAGE + (d % PAGE)) * (D * 2 / 16) + chunk;
-      base[dofs] = base[so];
+    // No destination of an earlier move is the source of a later one (src position P + a_t with a_t >= t, dst
+    // position P + t' with t' < t), so the loads of a batch of moves are issued together, then its stores: one
+    // memory round trip per 8 moves instead of one per move.
+    auto row_ofs = [&](int slot) -> size_t {
+      return (((size_t)(slot / PAGE) * Hkv + head) * PAGE + (slot % PAGE)) * (D * 2 / 16) + chunk;
+    };
+    for (int t0 = 0; t0 < L; t0 += 8) {
+      uint4 v[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e)
+        if (t0 + e < L && s_src[t0 + e] != s_dst[t0 + e]) v[e] = base[row_ofs(s_src[t0 + e])];
+#pragma unroll
+      for (int e = 0; e < 8; ++e)
+        if (t0 + e < L && s_src[t0 + e] != s_dst[t0 + e]) base[row_ofs(s_dst[t0 + e])] = v[e];
     }
   }
 }
