@@ -183,7 +183,10 @@ def run_gpu(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     build.build_library()
-    wl = sharding.rank_workload(args.config, rank, static=args.static, gated=not args.static)
+    heads = args.shard == "heads" and world > 1
+    # requests: every rank its own batch (weak scaling); heads: every rank the KV heads [r Hkv/W, (r+1) Hkv/W) of
+    # the same batch (strong scaling, no collective either: attention is independent per KV head)
+    wl = sharding.rank_workload(args.config, 0 if heads else rank, static=args.static, gated=not args.static)
     if args.gating != "sparse" and not args.static:
         wl.gate = wl.gate.ablation(args.gating)
     g = wl.gate
@@ -202,11 +205,13 @@ def run_gpu(args, rank, world, local_rank):
             "prev": pin(wl.prev_token)}
     d_in = {k: v.to(dev) for k, v in h_in.items()}
     q, k, v = W.draw_qkv(wl, cap, device=str(dev))
+    if heads:
+        q, k, v = sharding.shard_attention_inputs(q, k, v, rank, world)
     kv = echo.PagedKV(k, v, d(wl.page_table), d(wl.prefix_len))
     sel = ctx.alloc_selection(wl.R, wl.N, cap)
     acc = ctx.alloc_accept(wl.R, cap)
     out = torch.zeros_like(q)
-    lse = torch.zeros(cap, wl.Hq, dtype=torch.float32, device=dev)
+    lse = torch.zeros(cap, q.shape[1], dtype=torch.float32, device=dev)
 
     def gate(din, sel_=None):
         return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
@@ -227,6 +232,8 @@ def run_gpu(args, rank, world, local_rank):
         if logits.shape[0] < cap:
             logits = torch.cat([logits, torch.zeros(cap - logits.shape[0], logits.shape[1], dtype=logits.dtype, device=dev)])
     bytes_alg, flops_alg = algorithmic_bytes(wl, sel_h)
+    if heads:
+        bytes_alg, flops_alg = bytes_alg // world, flops_alg // world
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
     attn_ev = [(ev(), ev()) for _ in range(args.steps)]
@@ -284,7 +291,7 @@ def run_gpu(args, rank, world, local_rank):
         c1.record()
         torch.cuda.synchronize()
         calib_us = c0.elapsed_time(c1) * 100.0
-    return dict(calib_us=calib_us, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
+    return dict(calib_us=calib_us, heads=heads, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
                 accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
                 out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
 
@@ -364,6 +371,8 @@ def main():
                     help="the paper's ablation variants (PAPER.md:254-258): gate every depth / one threshold")
     ap.add_argument("--calibrate-samples", type=int, default=160000,
                     help="warm-up traces for echo_calibrate, timed outside the step (0 = skip)")
+    ap.add_argument("--shard", default="requests", choices=["requests", "heads"],
+                    help="N > 1: requests = each rank its own batch (weak); heads = KV-head shards of one batch (strong)")
     ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -377,7 +386,8 @@ def main():
     e2e_dt, h2d, d2h = run_e2e(r, args)
     from paper_2604_09603_b200 import sharding
     (ms, e2e_dt), (n_sel_all, acc_all) = sharding.reduce_step_stats(
-        [r["ms"], e2e_dt], [r["n_sel"], r["accepted"]], world, r["dev"], dist)
+        [r["ms"], e2e_dt], [r["n_sel"] / (world if r["heads"] else 1), r["accepted"] / (world if r["heads"] else 1)],
+        world, r["dev"], dist)
     if rank == 0:
         peak, peak_src = peaks()
         achieved = r["bytes_alg"] / (r["t_attn"] * 1e-3) / 1e9
@@ -402,7 +412,7 @@ def main():
         launches = 3 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)  # gate 3, plan + attn, merge, accept, argmax
         line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
-                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "higher_is_better": True, "scaling": "strong" if r["heads"] else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
                            + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
                            "requests": wl.R, "verified_nodes_per_step": r["n_sel"],

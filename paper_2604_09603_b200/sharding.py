@@ -36,3 +36,21 @@ def reduce_step_stats(times_ms, counts, world: int, device, dist=None):
 def job_throughput(total_units: float, steps: int, max_ms: float) -> float:
     """Whole-job units per second: units all ranks processed per step x steps / slowest rank's time."""
     return total_units * steps / (max_ms * 1e-3)
+
+
+def head_shard(rank: int, world: int, Hq: int, Hkv: int):
+    """Head-sharded (tensor-parallel style) split of the verify attention: rank r owns the KV
+    heads [r Hkv/W, (r+1) Hkv/W) of every page and the query heads of those groups.  Attention is independent per
+    KV head, so S6-S7 need no collective; S1-S5 and S9 are replicated (kilobytes); S10 compacts each rank's heads.
+    Returns (slice over query heads, slice over KV heads)."""
+    if world < 1 or not (0 <= rank < world) or Hkv % world or Hq % Hkv:
+        raise ValueError(f"cannot shard Hq={Hq} Hkv={Hkv} over {world} ranks")
+    per = Hkv // world
+    G = Hq // Hkv
+    return slice(rank * per * G, (rank + 1) * per * G), slice(rank * per, (rank + 1) * per)
+
+
+def shard_attention_inputs(q, k_pool, v_pool, rank: int, world: int):
+    """q [cap][Hq][128], pools [layers][pages][Hkv][16][128] (torch tensors) -> this rank's contiguous shards."""
+    hq, hkv = head_shard(rank, world, q.shape[1], k_pool.shape[2])
+    return q[:, hq].contiguous(), k_pool[:, :, hkv].contiguous(), v_pool[:, :, hkv].contiguous()

@@ -266,3 +266,24 @@ def test_attn_second_layer_of_a_two_layer_pool(path):
         assert max(np.abs(o_gpu[k_, h] - res[(k_, h)][0]).max() for (k_, h) in rows) <= TOL_O
         assert max(abs(l_gpu[k_, h] - res[(k_, h)][1]) for (k_, h) in rows) <= TOL_LSE
     assert ctx.device_status() == 0
+
+
+@pytest.mark.parametrize("world", [2, 4])
+def test_attn_head_sharded_equals_unsharded(world):
+    """NEXT-4 / SURVEY 8(e): rank r runs the same call on its KV heads' shard of Q and the pools; the concatenation
+    of the ranks' outputs is the unsharded output bit for bit (one GPU, the shards run one after the other: they
+    share nothing and wait on nothing)."""
+    import torch
+    from paper_2604_09603_b200 import echo, sharding
+    wl = W.make_config(1, R=5, gated=True)
+    ctx, sel, want_sel, q, k, v = _setup(wl)
+    ctx.set_option(echo.OPT_ATTN_PATH, 0)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 1)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    outs, lses = [], []
+    for r in range(world):
+        qs, ks, vs = sharding.shard_attention_inputs(q, k, v, r, world)
+        o_r, l_r = ctx.verify_attn(sel, make_kv(wl, ks, vs), qs, SM_SCALE)
+        outs.append(o_r.clone()); lses.append(l_r.clone())
+    n = want_sel["n_selected"]
+    assert torch.equal(torch.cat(outs, dim=1)[:n], out[:n]) and torch.equal(torch.cat(lses, dim=1)[:n], lse[:n])

@@ -63,3 +63,22 @@ def test_rank0_is_the_single_gpu_workload():
     assert sharding.rank_seed(2, 3) == W.SEED_BASE + 2 + 3000
     t, c = sharding.reduce_step_stats([1.5], [7], 1, torch.device("cpu"))
     assert t == [1.5] and c == [7.0]
+
+
+def test_head_shards_partition_the_heads():
+    for Hq, Hkv, W_ in [(64, 8, 1), (64, 8, 2), (64, 8, 8), (32, 8, 4), (64, 4, 4)]:
+        q_seen, kv_seen = [], []
+        for r in range(W_):
+            hq, hkv = sharding.head_shard(r, W_, Hq, Hkv)
+            q_seen += list(range(Hq))[hq]
+            kv_seen += list(range(Hkv))[hkv]
+            G = Hq // Hkv
+            assert [h // G for h in list(range(Hq))[hq]] == sorted(list(range(Hkv))[hkv] * G)   # groups stay whole
+        assert q_seen == list(range(Hq)) and kv_seen == list(range(Hkv))
+    with pytest.raises(ValueError):
+        sharding.head_shard(0, 3, 64, 8)
+    q = torch.arange(2 * 8 * 4).reshape(2, 8, 4)
+    kp = torch.arange(1 * 3 * 2 * 16 * 4).reshape(1, 3, 2, 16, 4)
+    qs, ks, vs = sharding.shard_attention_inputs(q, kp, kp + 1, 1, 2)
+    assert qs.shape == (2, 4, 4) and ks.shape == (1, 3, 1, 16, 4) and qs.is_contiguous()
+    assert torch.equal(qs, q[:, 4:]) and torch.equal(vs, kp[:, :, 1:] + 1)
