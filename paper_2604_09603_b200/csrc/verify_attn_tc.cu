@@ -1,15 +1,20 @@
-// S6 on the 5th-gen tensor cores: persistent, warp-specialised split-KV verify attention.
+// S6 on the 5th-gen tensor cores: persistent, warp-specialised split-KV verify attention (DESIGN.md section 6).
 //
-//   work item  = (request i, KV head, 128-row tile of (node, head-in-group) rows, KV split)
-//   warp 0     = TMA producer: Q tile (3-D tensor map over [node][head][d]) and, per 128-token KV tile,
-//                one 16x64 box per (page, d-half) for K and V (pages are looked up in the page table)
-//   warp 1     = MMA issuer (one lane): S = Q K^T (SS, K-major x K-major) into TMEM, O += P V (TS: P read
-//                from TMEM, V as the MN-major B operand) -- accumulators never leave TMEM
-//   warps 2-5  = softmax: thread = row; tcgen05.ld S, tree mask only in tiles that touch positions >= P_i,
-//                lazy rescale of O (only when the running max grows by > 2^8), P written back to TMEM as
-//                bf16 over S, epilogue normalises and stores out/lse (or the fp32 split partial)
-// Each KV page is read once per (KV head, row tile) and serves all rows of the tile; K/V rings and the S
-// double buffer keep TMA, tensor pipe and MUFU busy at the same time.
+//   work item   = (request i, KV head, 128-row tile of (node, head-in-group) rows, KV split); KV tile = 128 tokens
+//   warps 12,16 = K producers, warps 14,17 = V producers (one lane each): one 4-D TMA box per page (16 tokens x 128 d
+//                 of one KV head), pages looked up in the page table; warp 12 also loads the Q tile (3-D tensor map
+//                 over [node][head][d]).  Two issuing threads per ring because one cp.async.bulk.tensor costs its
+//                 thread 110-170 cycles whatever the box size.
+//   warp 13     = issuer of S = Q K^T (SS, K-major x K-major) into one of three S buffers in TMEM
+//   warp 15     = issuer of O += P V (TS: P read from TMEM where the softmax wrote it over S, V as the MN-major B
+//                 operand straight from its TMA layout); accumulators never leave TMEM
+//   warps 0-7   = softmax, two warpgroups, thread = half a row (64 columns): weights against a running reference
+//                 without a row maximum first, two-pass fallback on a vote of the two warps of a row quarter; tree
+//                 mask only in tiles that touch positions >= P_i; a quarter of the prefix-tile weights take 2^x on
+//                 the FMA pipe; P written back to TMEM as bf16 over the first 32 columns of the thread's S half
+//   warps 8-11  = epilogue: O / l -> bf16 out + lse (or the fp32 split partial) while the softmax is on the next item
+//   setmaxnreg  : softmax 160, epilogue 80, single-lane warps 40 registers
+// Each KV page is read once per (KV head, row tile) and serves all rows of the tile.
 // Operator definition: include/echo.h (paper: P:39, P:85 names it only; readings R:A-1..A-8).
 #include <cuda.h>
 
@@ -36,7 +41,8 @@ constexpr int SMEM_BAR = SMEM_XCHG + 2 * TILE_M * 4;
 constexpr int SMEM_TOTAL = SMEM_BAR + 256;  // dynamic smem is declared 1024-byte aligned: no slack
 // warpgroups 0 and 1 (warps 0-3, 4-7) softmax: warpgroup w takes columns [64 w, 64 w + 64) of every S row, so each
 // SM sub-partition has two softmax warps to issue from; warpgroup 2 (warps 8-11) epilogue; warpgroup 3: warp 12 Q+K
-// producer, 13 QK^T MMA issuer, 14 V producer, 15 PV MMA issuer
+// producer, 13 QK^T MMA issuer, 14 V producer, 15 PV MMA issuer; warpgroup 4: warps 16 / 17 second K / V producer,
+// 18-19 idle (they pad the warpgroup so that setmaxnreg applies)
 constexpr int NTHREADS = 640;
 constexpr int W_EPI = 8, W_PROD_K0 = 12, W_MMA_QK = 13, W_PROD_V0 = 14, W_MMA_PV = 15, W_PROD_K1 = 16, W_PROD_V1 = 17;
 constexpr int REGS_SOFTMAX = 160, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 160 + 80 + 2 * 40) = 640 * 96, the launch allocation
