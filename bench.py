@@ -213,7 +213,14 @@ def run_gpu(args, rank, world, local_rank):
     out = torch.zeros_like(q)
     lse = torch.zeros(cap, q.shape[1], dtype=torch.float32, device=dev)
 
+    g_global, gb_bufs = g.replace(budget=g.budget * world), {}
+    all_sizes = sharding.exchange_sizes(wl.N, wl.R, world, dist) if args.global_budget else None
+
     def gate(din, sel_=None):
+        if args.global_budget and not heads:  # one budget of world x B over the ranks' requests: the one exchange of the path
+            return sharding.global_budget_gate_select(ctx, rank, world, din["cand_offsets"], din["parent"], din["logq"],
+                                                      g_global, sel_ or sel, max_cand=wl.max_cand, schedule=schedule,
+                                                      dist=dist, all_sizes=all_sizes, bufs=gb_bufs)
         return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
                                g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel_ or sel,
                                schedule=schedule)
@@ -373,6 +380,8 @@ def main():
                     help="warm-up traces for echo_calibrate, timed outside the step (0 = skip)")
     ap.add_argument("--shard", default="requests", choices=["requests", "heads"],
                     help="N > 1: requests = each rank its own batch (weak); heads = KV-head shards of one batch (strong)")
+    ap.add_argument("--global-budget", action="store_true",
+                    help="request-sharded ranks share ONE budget of N x B: keys are all-gathered before the select")
     ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -414,7 +423,7 @@ def main():
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "strong" if r["heads"] else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
-                           + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
+                           + (" global-budget" if args.global_budget else "") + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
                            "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",

@@ -109,6 +109,10 @@ typedef struct {
                           ECHO_SCHED_ALG1: Algorithm 1 as printed, P:127-160 -- Phase 1 depth by depth, request order
                           inside a depth, a level best-first by (S desc, node asc); Phase 2 over the truncated
                           requests in truncation order (R:L-1..L-4).  Ignored when static_k > 0. */
+  int32_t cand_index_base; /* 0, or -- when several ranks share one budget (echo_gate_keys / echo_gate_select_keys) --
+                              the number of candidates of the ranks before this one: keys carry the global candidate
+                              index, so ties break by (rank, request, node) and keys stay unique across ranks */
+  int32_t request_base;    /* likewise the number of requests of the ranks before this one (ECHO_SCHED_ALG1 keys) */
 } EchoGate;
 
 /* Packed ragged batch ("Flatten & Pack", Fig. 3(3)): request asc, node asc (R:P-1). */
@@ -184,6 +188,19 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
  * P_i .. P_i+L-1, every read before any write to the same slot column (R:C-6). */
 int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t num_requests,
                 EchoPagedKV* kv, EchoAccept* out, echo_stream_t stream);
+
+/* ---- one budget shared by several ranks (request-sharded multi-GPU) ---------- */
+/* echo_gate_select in two halves around the one exchange the path has: every rank computes S1-S2 and the 64-bit
+ * selection keys of its own candidates (echo_gate_keys; keys[total_cand] device, caller-owned; ~0 = not eligible),
+ * the ranks all-gather their keys (N x 8 B each, e.g. ncclAllGather; ranks with fewer candidates pad with ~0), and
+ * every rank selects against the whole population and packs its own requests (echo_gate_select_keys: the budget-th
+ * smallest of all_keys[n_all] is the threshold; local_keys are this rank's, indexed like cand_offsets).  With
+ * all_keys == local_keys the pair equals echo_gate_select.  gate->cand_index_base / request_base must be the exclusive
+ * prefix sums of total_cand / num_requests over the ranks, and gate->budget the global K_max on every rank. */
+int echo_gate_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, EchoSelection* out, uint64_t* keys,
+                   echo_stream_t stream);
+int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, const uint64_t* local_keys,
+                          const uint64_t* all_keys, int64_t n_all, EchoSelection* out, echo_stream_t stream);
 
 /* ---- warm-up calibration of the gates ------------------------------ */
 /* Traces collected during warm-up: one sample per (request, depth) with the layer confidence

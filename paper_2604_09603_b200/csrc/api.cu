@@ -104,21 +104,47 @@ int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas) {
   return debug_wait_prof(reinterpret_cast<unsigned long long*>(host_out), n_ctas);
 }
 
-int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, echo_stream_t stream) {
+static int check_gate(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, bool need_packed) {
   if (!ctx || !t || !g || !o) return ECHO_ERR_INVALID_ARG;
   if (t->num_requests < 0 || t->total_cand < 0 || t->max_cand_per_req < 0) return ECHO_ERR_INVALID_ARG;
   if (g->budget < 0 || g->w_max < 0 || g->static_k < 0 || o->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->cand_index_base < 0 || g->request_base < 0) return ECHO_ERR_INVALID_ARG;
   if (g->schedule != ECHO_SCHED_TOPB && g->schedule != ECHO_SCHED_ALG1) return ECHO_ERR_INVALID_ARG;
   if (t->max_cand_per_req > ECHO_MAX_CAND) return ECHO_ERR_UNSUPPORTED;
-  if (!t->cand_offsets || !o->n_selected || !o->sel_offsets || !o->cut_depth) return ECHO_ERR_INVALID_ARG;
+  if (!t->cand_offsets || !o->cut_depth) return ECHO_ERR_INVALID_ARG;
   if (t->total_cand > 0 && (!t->parent || !t->logq || !o->path_score || !o->cand_depth)) return ECHO_ERR_INVALID_ARG;
+  if (!need_packed) return ECHO_OK;
+  if (!o->n_selected || !o->sel_offsets) return ECHO_ERR_INVALID_ARG;
   long need = g->static_k > 0 ? (long)t->num_requests * g->static_k : (long)g->budget;
   if (need > t->total_cand) need = t->total_cand;
   if (o->capacity < need) return ECHO_ERR_INVALID_ARG;
   if (o->capacity > 0 && (!o->sel_node || !o->sel_req || !o->parent_local || !o->sel_depth || !o->anc_mask))
     return ECHO_ERR_INVALID_ARG;
   if (misaligned(o->anc_mask, 16)) return ECHO_ERR_INVALID_ARG;
+  return ECHO_OK;
+}
+
+int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, echo_stream_t stream) {
+  const int rc = check_gate(ctx, t, g, o, true);
+  if (rc != ECHO_OK) return rc;
   return launch_gate_select(ctx, t, g, o, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int echo_gate_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, uint64_t* keys,
+                   echo_stream_t stream) {
+  const int rc = check_gate(ctx, t, g, o, false);
+  if (rc != ECHO_OK) return rc;
+  if (t->total_cand > 0 && (!keys || misaligned(keys, 8))) return ECHO_ERR_INVALID_ARG;
+  return launch_gate_keys(ctx, t, g, o, keys, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, const uint64_t* local_keys,
+                          const uint64_t* all_keys, int64_t n_all, EchoSelection* o, echo_stream_t stream) {
+  const int rc = check_gate(ctx, t, g, o, true);
+  if (rc != ECHO_OK) return rc;
+  if (n_all < 0 || (n_all > 0 && !all_keys) || (t->total_cand > 0 && !local_keys)) return ECHO_ERR_INVALID_ARG;
+  if (misaligned(all_keys, 8) || misaligned(local_keys, 8)) return ECHO_ERR_INVALID_ARG;
+  return launch_gate_select_keys(ctx, t, g, local_keys, all_keys, n_all, o, reinterpret_cast<cudaStream_t>(stream));
 }
 
 static int check_kv(const EchoPagedKV* kv, bool need_pools) {

@@ -17,6 +17,8 @@ struct GateParams {
   int32_t w_max;
   int32_t static_k;
   int32_t schedule;
+  int32_t cand_base;  // global index of this call's first candidate / request (> 0 only when several ranks share
+  int32_t req_base;   // one budget)
 };
 
 __device__ __forceinline__ float f32_unordered(uint32_t o) {
@@ -108,20 +110,20 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
     if (gp.static_k > 0) {
       int rank = 0;  // per-request top-static_k by (S desc, node asc) (R:G-15)
       for (int t = 0; t < C; ++t) rank += (s_S[t] > S) || (s_S[t] == S && t < j);
-      if (rank < gp.static_k) key = make_key(0, 0.0f, b + j);
+      if (rank < gp.static_k) key = make_key(0, 0.0f, gp.cand_base + b + j);
     } else if (gp.schedule == ECHO_SCHED_ALG1) {
       if (d <= cut) {
         int rank = 0;  // position in the level by (S desc, node asc)
         for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
-        if (d < cut) key = make_key_alg1(0, d, i, rank);
-        else if (rank < gp.w_max) key = make_key_alg1(1, d, i, rank);
+        if (d < cut) key = make_key_alg1(0, d, gp.req_base + i, rank);
+        else if (rank < gp.w_max) key = make_key_alg1(1, d, gp.req_base + i, rank);
       }
     } else if (d < cut) {
-      key = make_key(0, S, b + j);  // tier 0: depth extension
+      key = make_key(0, S, gp.cand_base + b + j);  // tier 0: depth extension
     } else if (d == cut) {
       int rank = 0;  // tier 1: the w_max best nodes of the truncation level (R:G-7, G-8)
       for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
-      if (rank < gp.w_max) key = make_key(1, S, b + j);
+      if (rank < gp.w_max) key = make_key(1, S, gp.cand_base + b + j);
     }
     keys[b + j] = key;
   }
@@ -140,8 +142,11 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 }
 
 __global__ void __launch_bounds__(SEL_THREADS) k_select(
-    const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ keys, int R, int N, int budget,
-    int32_t* __restrict__ n_selected, int32_t* __restrict__ sel_offsets, uint64_t* __restrict__ threshold) {
+    const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ local_keys, int R,
+    const uint64_t* __restrict__ keys, int N, int budget, int32_t* __restrict__ n_selected,
+    int32_t* __restrict__ sel_offsets, uint64_t* __restrict__ threshold) {
+  // `keys` [N] is the whole key population the budget is drawn from (this call's own keys, or the keys of every rank
+  // that shares the budget); `local_keys` are this call's candidates, indexed like cand_offsets.
   __shared__ int s_hist[256];
   __shared__ int s_warp[32];
   __shared__ uint64_t s_prefix;
@@ -256,7 +261,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
       int j = w * 32 + lane;
-      bool s = !none && j < C && keys[b + j] <= T;
+      bool s = !none && j < C && local_keys[b + j] <= T;
       cnt += __popc(__ballot_sync(0xffffffffu, s));
     }
     if (lane == 0) sel_offsets[r + 1] = cnt;
@@ -348,24 +353,59 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
 
 }  // namespace
 
-int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, cudaStream_t st) {
-  const int R = t->num_requests, N = t->total_cand;
-  uint64_t* keys = reinterpret_cast<uint64_t*>(ctx->workspace);
-  const size_t keys_bytes = align_up((size_t)N * sizeof(uint64_t), 256);
-  if (keys_bytes + 256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
-  uint64_t* threshold = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(ctx->workspace) + keys_bytes);
+static GateParams gate_params(const EchoGate* g) {
   GateParams gp;
   gp.depth_mask = g->depth_mask;
   for (int d = 0; d < 32; ++d) gp.log_tau[d] = g->log_tau[d] + 0.0f;  // canonicalise -0 (R:G-13)
   gp.w_max = g->w_max;
   gp.static_k = g->static_k;
   gp.schedule = g->schedule;
+  gp.cand_base = g->cand_index_base;
+  gp.req_base = g->request_base;
+  return gp;
+}
+
+int launch_gate_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, uint64_t* keys,
+                     cudaStream_t st) {
+  if (t->num_requests > 0) {
+    k_score_gate<<<t->num_requests, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g),
+                                                            o->path_score, o->cand_depth, o->cut_depth, keys,
+                                                            ctx->dev_status);
+  }
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}
+
+int launch_gate_select_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, const uint64_t* local_keys,
+                            const uint64_t* all_keys, int64_t n_all, EchoSelection* o, cudaStream_t st) {
+  const int R = t->num_requests;
+  if (n_all > 0x7fffffffll) return ECHO_ERR_UNSUPPORTED;
+  if (256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  uint64_t* threshold = reinterpret_cast<uint64_t*>(ctx->workspace);
+  const int budget = g->static_k > 0 ? (int)n_all : g->budget;
+  ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, local_keys, R, all_keys,
+                                (int)n_all, budget, o->n_selected, o->sel_offsets, threshold));
   if (R > 0) {
-    k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gp, o->path_score,
+    ECHO_CUDA_TRY(ctx, launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent,
+                                  o->cand_depth, local_keys, threshold, o->capacity, o->sel_offsets, o->sel_node,
+                                  o->sel_req, o->parent_local, o->sel_depth, o->anc_mask));
+  }
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}
+
+int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, cudaStream_t st) {
+  const int R = t->num_requests, N = t->total_cand;
+  uint64_t* keys = reinterpret_cast<uint64_t*>(ctx->workspace);
+  const size_t keys_bytes = align_up((size_t)N * sizeof(uint64_t), 256);
+  if (keys_bytes + 256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
+  uint64_t* threshold = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(ctx->workspace) + keys_bytes);
+  if (R > 0) {
+    k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g), o->path_score,
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);
   }
   const int budget = g->static_k > 0 ? N : g->budget;
-  ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, N, budget,
+  ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, keys, N, budget,
                                 o->n_selected, o->sel_offsets, threshold));
   if (R > 0) {
     ECHO_CUDA_TRY(ctx, launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent, o->cand_depth, keys, threshold, o->capacity,

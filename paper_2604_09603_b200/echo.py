@@ -27,7 +27,7 @@ DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
            "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept",
-           "echo_calibrate"]
+           "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys"]
 
 
 class EchoTrees(C.Structure):
@@ -37,7 +37,8 @@ class EchoTrees(C.Structure):
 
 class EchoGate(C.Structure):
     _fields_ = [("depth_mask", C.c_uint32), ("log_tau", C.c_float * 32), ("w_max", C.c_int32),
-                ("budget", C.c_int32), ("static_k", C.c_int32), ("schedule", C.c_int32)]
+                ("budget", C.c_int32), ("static_k", C.c_int32), ("schedule", C.c_int32),
+                ("cand_index_base", C.c_int32), ("request_base", C.c_int32)]
 
 
 class EchoSelection(C.Structure):
@@ -107,6 +108,11 @@ def load_library():
     lib.echo_set_option.restype = C.c_int
     lib.echo_debug_wait_prof.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
     lib.echo_debug_wait_prof.restype = C.c_int
+    lib.echo_gate_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p, C.c_void_p]
+    lib.echo_gate_keys.restype = C.c_int
+    lib.echo_gate_select_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), C.c_void_p, C.c_void_p, C.c_int64,
+                                          P(EchoSelection), C.c_void_p]
+    lib.echo_gate_select_keys.restype = C.c_int
     lib.echo_calibrate.argtypes = [C.c_void_p, P(EchoTraces), C.c_double, P(EchoCalibration), C.c_void_p]
     lib.echo_calibrate.restype = C.c_int
     lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
@@ -301,6 +307,47 @@ class EchoContext:
         g.w_max, g.budget, g.static_k, g.schedule = int(w_max), int(budget), int(static_k), int(schedule)
         cs = sel.c_struct()
         self._check(self.lib.echo_gate_select(self._h, C.byref(trees), C.byref(g), C.byref(cs), self._stream()))
+        return sel
+
+    @staticmethod
+    def _gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, cand_index_base, request_base):
+        g = EchoGate()
+        g.depth_mask = int(depth_mask) & 0xFFFFFFFF
+        lt = np.asarray(log_tau, np.float32)
+        for d in range(32):
+            g.log_tau[d] = float(lt[d])
+        g.w_max, g.budget, g.static_k, g.schedule = int(w_max), int(budget), int(static_k), int(schedule)
+        g.cand_index_base, g.request_base = int(cand_index_base), int(request_base)
+        return g
+
+    def gate_keys(self, cand_offsets, parent, logq, depth_mask: int, log_tau, w_max: int, budget: int, sel: Selection,
+                  static_k: int = 0, schedule: int = 0, cand_index_base: int = 0, request_base: int = 0,
+                  max_cand: int = 128):
+        """echo_gate_keys: S1-S2 and the selection keys of this rank's candidates -> int64 device tensor [N]
+        (the bits of the uint64 keys; -1 = not eligible), to be all-gathered across the ranks sharing the budget.
+        The tensor is a buffer this context reuses on the next call."""
+        import torch
+        R, N = cand_offsets.numel() - 1, parent.numel()
+        if getattr(self, "_keys_buf", None) is None or self._keys_buf.numel() < max(1, N):
+            self._keys_buf = torch.empty(max(1, N), dtype=torch.int64, device=self.device)
+        keys = self._keys_buf
+        trees = EchoTrees(R, N, max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
+        g = self._gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, cand_index_base, request_base)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_gate_keys(self._h, C.byref(trees), C.byref(g), C.byref(cs), _ptr(keys), self._stream()))
+        return keys[:N]
+
+    def gate_select_keys(self, cand_offsets, parent, logq, depth_mask: int, log_tau, w_max: int, budget: int,
+                         local_keys, all_keys, sel: Selection, static_k: int = 0, schedule: int = 0,
+                         max_cand: int = 128) -> Selection:
+        """echo_gate_select_keys: threshold over `all_keys` (every rank's keys), packing of this rank's requests."""
+        R, N = cand_offsets.numel() - 1, parent.numel()
+        self.ensure_workspace(R, N, sel.capacity, 0)
+        trees = EchoTrees(R, N, max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
+        g = self._gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, 0, 0)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_gate_select_keys(self._h, C.byref(trees), C.byref(g), _ptr(local_keys), _ptr(all_keys),
+                                                   int(all_keys.numel()), C.byref(cs), self._stream()))
         return sel
 
     def verify_attn(self, sel: Selection, kv: PagedKV, q, sm_scale: float, layer: int = 0, out=None, lse=None):

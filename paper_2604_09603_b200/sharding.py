@@ -54,3 +54,53 @@ def shard_attention_inputs(q, k_pool, v_pool, rank: int, world: int):
     """q [cap][Hq][128], pools [layers][pages][Hkv][16][128] (torch tensors) -> this rank's contiguous shards."""
     hq, hkv = head_shard(rank, world, q.shape[1], k_pool.shape[2])
     return q[:, hq].contiguous(), k_pool[:, :, hkv].contiguous(), v_pool[:, :, hkv].contiguous()
+
+
+def rank_bases(sizes, rank: int):
+    """Exclusive prefix sum of per-rank sizes (candidates or requests): the base this rank's keys carry."""
+    return int(sum(int(x) for x in sizes[:rank]))
+
+
+def exchange_sizes(N: int, R: int, world: int, dist=None):
+    """[(N_r, R_r)] of every rank, exchanged once at set-up (host integers: batch shapes are known on the host)."""
+    if world == 1:
+        return [(int(N), int(R))]
+    if dist is None:
+        import torch.distributed as dist  # noqa: PLC0415
+    out = [None] * world
+    dist.all_gather_object(out, (int(N), int(R)))
+    return [tuple(x) for x in out]
+
+
+def global_budget_gate_select(ctx, rank: int, world: int, cand_offsets, parent, logq, gate, sel, max_cand=128,
+                              schedule=0, dist=None, all_sizes=None, bufs=None):
+    """Request-sharded ranks that share ONE verification budget (the paper's batch-wide K_max, Eq. 4, over the whole
+    data-parallel group): the only exchange of the path.  Every rank computes its keys, the ranks
+    all-gather them (N x 8 B, padded with "not eligible" to the largest N), and each selects against all keys and
+    packs its own requests.  `gate.budget` is the global budget.  `all_sizes` = exchange_sizes(...) (taken here if not
+    given); `bufs` = a dict the call keeps its padded / gathered key buffers in between steps.  No host
+    synchronisation: sizes are host integers, everything else stays on the stream."""
+    import torch
+    if dist is None and world > 1:
+        import torch.distributed as dist  # noqa: PLC0415
+    R, N = cand_offsets.numel() - 1, parent.numel()
+    if all_sizes is None:
+        all_sizes = exchange_sizes(N, R, world, dist)
+    Ns = [n for n, _ in all_sizes]
+    Rs = [r for _, r in all_sizes]
+    keys = ctx.gate_keys(cand_offsets, parent, logq, gate.depth_mask, gate.log_tau, gate.w_max, gate.budget, sel,
+                         static_k=gate.static_k, schedule=schedule, cand_index_base=rank_bases(Ns, rank),
+                         request_base=rank_bases(Rs, rank), max_cand=max_cand)
+    n_max = max(1, max(Ns))
+    bufs = bufs if bufs is not None else {}
+    if "padded" not in bufs or bufs["padded"].numel() != n_max or bufs["gathered"].numel() != world * n_max:
+        bufs["padded"] = torch.full((n_max,), -1, dtype=torch.int64, device=keys.device)
+        bufs["gathered"] = torch.empty(world * n_max, dtype=torch.int64, device=keys.device)
+    padded, gathered = bufs["padded"], bufs["gathered"]
+    padded[:N].copy_(keys)
+    if world > 1:
+        dist.all_gather_into_tensor(gathered, padded)
+    else:
+        gathered.copy_(padded)
+    return ctx.gate_select_keys(cand_offsets, parent, logq, gate.depth_mask, gate.log_tau, gate.w_max, gate.budget,
+                                keys, gathered, sel, static_k=gate.static_k, schedule=schedule, max_cand=max_cand)

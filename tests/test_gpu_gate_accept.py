@@ -262,3 +262,53 @@ def test_alg1_budget_edges_and_widening(budget):
     g = wl.gate.replace(budget=budget)
     sel = run_gate_select(ctx, wl, g, capacity=max(budget, 1), schedule=echo.SCHED_ALG1)
     assert_selection_equal(sel.to_host(), oracle_gate_select(orc, wl, g, schedule=1))
+
+
+# ---------------------------------------------------------------- one budget shared by several ranks
+def _slice_oracle(want, r0, r1):
+    """the packed arrays of requests [r0, r1) of a selection over the merged batch, rebased to a rank-local view"""
+    offs = want["sel_offsets"]
+    a, b = int(offs[r0]), int(offs[r1])
+    return dict(n_selected=b - a, sel_offsets=(offs[r0:r1 + 1] - offs[r0]).astype(np.int32),
+                sel_node=want["sel_node"][a:b], sel_req=(want["sel_req"][a:b] - r0).astype(np.int32),
+                parent_local=want["parent_local"][a:b], sel_depth=want["sel_depth"][a:b],
+                anc_mask=want["anc_mask"][a:b], path_score=None, cand_depth=None, cut_depth=want["cut_depth"][r0:r1])
+
+
+@pytest.mark.parametrize("cfgs,schedule", [((2, 2), 0), ((1, 3, 0), 0), ((2, 2), 1), ((0, 4, 1), 1)])
+def test_global_budget_across_ranks_equals_merged_batch(cfgs, schedule):
+    """Ranks with their own requests share ONE budget: keys of all ranks, one threshold, each rank packs its own.
+    The ranks run one after the other on this GPU and torch.cat stands in for the all-gather (they share nothing
+    else); the oracle selects on the merged batch."""
+    import torch
+    ctx = get_ctx()
+    wls = [W.make_config(c, R=5 + 3 * i, seed=777 + i) for i, c in enumerate(cfgs)]
+    g0 = wls[0].gate
+    budget = sum(w.N for w in wls) // 3
+    offs = np.concatenate([[0]] + [w.cand_offsets[1:] + sum(x.N for x in wls[:i]) for i, w in enumerate(wls)]).astype(np.int32)
+    parent = np.concatenate([w.parent for w in wls])
+    logq = np.concatenate([w.logq for w in wls])
+    want = orc.gate_select(offs, parent, logq, g0.depth_mask, g0.log_tau, g0.w_max, budget, 0, schedule=schedule)
+    sels, keys, dts = [], [], []
+    for i, w in enumerate(wls):
+        dt = (dev(w.cand_offsets), dev(w.parent), dev(w.logq))
+        sel = ctx.alloc_selection(w.R, w.N, min(budget, w.N))
+        k = ctx.gate_keys(*dt, g0.depth_mask, g0.log_tau, g0.w_max, budget, sel, schedule=schedule,
+                          cand_index_base=sum(x.N for x in wls[:i]), request_base=sum(x.R for x in wls[:i]),
+                          max_cand=max(1, w.max_cand))
+        sels.append(sel); keys.append(k.clone()); dts.append(dt)   # one context plays all ranks: its key buffer is reused
+    n_max = max(k.numel() for k in keys)
+    gathered = torch.cat([torch.cat([k, torch.full((n_max - k.numel(),), -1, dtype=torch.int64, device=k.device)]) for k in keys])
+    total = 0
+    for i, w in enumerate(wls):
+        ctx.gate_select_keys(*dts[i], g0.depth_mask, g0.log_tau, g0.w_max, budget, keys[i], gathered, sels[i],
+                             schedule=schedule, max_cand=max(1, w.max_cand))
+        got = sels[i].to_host()
+        r0 = sum(x.R for x in wls[:i])
+        exp = _slice_oracle(want, r0, r0 + w.R)
+        assert got["n_selected"] == exp["n_selected"]
+        for key in ("sel_offsets", "sel_node", "sel_req", "parent_local", "sel_depth", "anc_mask", "cut_depth"):
+            np.testing.assert_array_equal(np.asarray(got[key])[:len(exp[key])], exp[key], err_msg=f"rank {i} {key}")
+        total += got["n_selected"]
+    assert total == want["n_selected"] <= budget
+    assert ctx.device_status() == 0

@@ -82,3 +82,45 @@ def test_head_shards_partition_the_heads():
     qs, ks, vs = sharding.shard_attention_inputs(q, kp, kp + 1, 1, 2)
     assert qs.shape == (2, 4, 4) and ks.shape == (1, 3, 1, 16, 4) and qs.is_contiguous()
     assert torch.equal(qs, q[:, 4:]) and torch.equal(vs, kp[:, :, 1:] + 1)
+
+
+class _FakeCtx:
+    """records what sharding.global_budget_gate_select passes to the two halves of the gate (no GPU here)"""
+    device = torch.device("cpu")
+
+    def gate_keys(self, cand_offsets, parent, logq, depth_mask, log_tau, w_max, budget, sel, static_k=0, schedule=0,
+                  cand_index_base=0, request_base=0, max_cand=128):
+        self.bases = (cand_index_base, request_base)
+        return torch.arange(parent.numel(), dtype=torch.int64) + 1000 * cand_index_base
+
+    def gate_select_keys(self, cand_offsets, parent, logq, depth_mask, log_tau, w_max, budget, local_keys, all_keys,
+                         sel, static_k=0, schedule=0, max_cand=128):
+        return dict(local=local_keys.clone(), all=all_keys.clone(), bases=self.bases, budget=budget)
+
+
+def _worker_global(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2604_09603_b200 import workloads as W
+        N, R = (7, 2) if rank == 0 else (4, 3)                      # ranks of different sizes: padding is exercised
+        offs = torch.tensor([0, 3, N] if rank == 0 else [0, 1, 2, N], dtype=torch.int32)
+        gate = W.Gate(budget=5)
+        res = sharding.global_budget_gate_select(_FakeCtx(), rank, world, offs, torch.zeros(N, dtype=torch.int32),
+                                                 torch.zeros(N), gate, None, dist=dist)
+        out[rank] = {k: (v.tolist() if hasattr(v, "tolist") else v) for k, v in res.items()}
+    finally:
+        dist.destroy_process_group()
+
+
+def test_global_budget_exchange_under_gloo():
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker_global, args=(2, _free_port(), out), nprocs=2, join=True)
+        res = {k: dict(v) for k, v in out.items()}
+    assert res[0]["bases"] == (0, 0) and res[1]["bases"] == (7, 2)          # exclusive prefix sums of (N, R)
+    want_all = list(range(7)) + [7000 + i for i in range(4)] + [-1] * 3     # rank 1 padded to the largest N
+    assert res[0]["all"] == want_all and res[1]["all"] == want_all
+    assert res[0]["local"] == list(range(7)) and res[1]["local"] == [7000 + i for i in range(4)]
+    assert res[0]["budget"] == res[1]["budget"] == 5
+    assert sharding.rank_bases([3, 4, 5], 2) == 7 and sharding.rank_bases([3, 4, 5], 0) == 0
