@@ -652,8 +652,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 
 // Device-side planner: P_i and K_i exist only on the device, so the work list is built there.
 // Items are bucketed by KV-tile count (descending) so that the snake assignment balances CTAs.
-constexpr int PLAN_THREADS = 1024;
-constexpr int PLAN_BUCKETS = 4096;
+constexpr int PLAN_THREADS = 256;   // one request per thread and pass at the batch sizes of BASELINE.json; a small CTA syncs faster
+constexpr int PLAN_BUCKETS = 1024;  // tile counts above 1023 (131 k tokens) share the last bucket
 __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict__ sel_offsets,
                                                        const int32_t* __restrict__ prefix_len, int R, int Hkv, int G,
                                                        int splits, int max_items, int4* __restrict__ items,
@@ -664,6 +664,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
   pdl_wait();               // sel_offsets come from echo_gate_select's kernels
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int b = tid; b < PLAN_BUCKETS; b += PLAN_THREADS) s_cnt[b] = 0;
+  if (tid < 32) s_warp[tid] = 0;
   __syncthreads();
   auto for_items = [&](auto&& fn) {
     for (int r = tid; r < R; r += PLAN_THREADS) {
