@@ -376,3 +376,37 @@ def calibrate(depth, conf, accepted, delta):
         if auc[d] > delta:
             mask |= 1 << d
     return dict(auc=auc, tau=tau, n_pos=n_pos, n_neg=n_neg, depth_mask=mask)
+
+
+# ---------------------------------------------------------------- O12 (NEXT-4): draft-side level expansion
+def draft_expand(level, k, parent_score, child_logq, child_token):
+    """One level of the draft tree built from the draft model's top-k outputs (EAGLE-style dynamic expansion, the step
+    the paper takes from its base system, "topk tokens"; readings R:D-1..D-3).  Per request:
+    the k_prev nodes of the previous level (k_prev = 1 virtual root with score 0 at level 0, else k) each propose k
+    children with draft log-probabilities; the cumulative score of a candidate is fl32(S_parent + logq) (Eq. 5), and
+    the level keeps the k best by (score desc, parent slot asc, child rank asc), in that order.
+    parent_score f32 [R][k_prev]; child_logq f32 / child_token i32 [R][k_prev][k].
+    Returns dict(sel_parent i32 [R][k] (slot in the previous level, -1 at level 0), logq f32 [R][k], token i32 [R][k],
+    score f32 [R][k])."""
+    parent_score = np.asarray(parent_score, np.float32)
+    child_logq = np.asarray(child_logq, np.float32)
+    child_token = np.asarray(child_token, np.int32)
+    R, k_prev, kk = child_logq.shape
+    assert kk == k and (k_prev == 1 if level == 0 else k_prev == k)
+    sel_parent = np.zeros((R, k), np.int32)
+    logq = np.zeros((R, k), np.float32)
+    token = np.zeros((R, k), np.int32)
+    score = np.zeros((R, k), np.float32)
+    for i in range(R):
+        cands = []
+        for p in range(k_prev):
+            for c in range(k):
+                s = np.float32(np.float32(parent_score[i, p]) + child_logq[i, p, c])
+                cands.append((-float(s), p, c, s))
+        cands.sort(key=lambda t: (t[0], t[1], t[2]))
+        for slot, (_, p, c, s) in enumerate(cands[:k]):
+            sel_parent[i, slot] = -1 if level == 0 else p
+            logq[i, slot] = child_logq[i, p, c]
+            token[i, slot] = child_token[i, p, c]
+            score[i, slot] = s
+    return dict(sel_parent=sel_parent, logq=logq, token=token, score=score)
