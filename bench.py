@@ -298,7 +298,35 @@ def run_gpu(args, rank, world, local_rank):
         c1.record()
         torch.cuda.synchronize()
         calib_us = c0.elapsed_time(c1) * 100.0
-    return dict(calib_us=calib_us, heads=heads, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
+    # the step on the other side of the path (NEXT-4): the candidate trees built on the device, level by level
+    draft_us = None
+    if rank == 0 and args.calibrate_samples > 0:
+        rng = np.random.default_rng(W.SEED_BASE + 1)
+        Ld, kd = 8, 10
+        lv = [W.draw_draft_level(rng, wl.R, 1 if l_ == 0 else kd, kd) for l_ in range(Ld)]
+        d_lv = [(d(a), d(b)) for a, b in lv]
+        t_off = d((np.arange(wl.R + 1) * Ld * kd).astype(np.int32))
+        t_par = torch.zeros(wl.R * Ld * kd, dtype=torch.int32, device=dev)
+        t_lq = torch.zeros(wl.R * Ld * kd, dtype=torch.float32, device=dev)
+        t_tok = torch.zeros_like(t_par)
+        sc = [torch.zeros(wl.R, kd, dtype=torch.float32, device=dev) for _ in range(Ld + 1)]
+        ps0 = torch.zeros(wl.R, 1, dtype=torch.float32, device=dev)
+
+        def build_tree():
+            for l_ in range(Ld):
+                ctx.draft_expand(l_, kd, ps0 if l_ == 0 else sc[l_], d_lv[l_][0], d_lv[l_][1], t_off, t_par, t_lq, t_tok,
+                                 sc[l_ + 1], max_cand=Ld * kd)
+        for _ in range(3):
+            build_tree()
+        c0, c1 = ev(), ev()
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(10):
+            build_tree()
+        c1.record()
+        torch.cuda.synchronize()
+        draft_us = c0.elapsed_time(c1) * 100.0
+    return dict(calib_us=calib_us, draft_us=draft_us, heads=heads, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
                 accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
                 out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
 
@@ -429,7 +457,8 @@ def main():
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
                            "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],
                            "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12,
-                           "calibrate_us": r["calib_us"], "calibrate_samples": args.calibrate_samples},
+                           "calibrate_us": r["calib_us"], "calibrate_samples": args.calibrate_samples,
+                           "draft_tree_8x10_us": r["draft_us"]},
                 "accepted_tokens_per_s": acc_all * args.steps / (ms * 1e-3),
                 "roofline": {"bound": "tensor" if tensor_bound else "hbm", "achieved": tflops if tensor_bound else achieved,
                              "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",

@@ -47,6 +47,7 @@ typedef enum {
 #define ECHO_DEV_DEPTH_OVERFLOW 4u /* a candidate deeper than 31 */
 #define ECHO_DEV_PAGE_OVERFLOW 8u  /* P_i + K_i needs more than max_pages_per_req pages */
 #define ECHO_DEV_BAD_TRACE 16u     /* echo_calibrate: depth >= 32 or a confidence outside [0, 1] / NaN (sample skipped) */
+#define ECHO_DEV_TREE_OVERFLOW 64u  /* echo_draft_expand: level * topk nodes do not fit the request's candidate range */
 #define ECHO_DEV_CALIB_OVERFLOW 32u /* echo_calibrate: more than ECHO_CALIB_MAX_PER_DEPTH samples at one depth (rest dropped) */
 
 /* test / tuning hooks for echo_set_option */
@@ -56,6 +57,7 @@ typedef enum {
 
 #define ECHO_MAX_CAND 128   /* C_i <= 128 candidates per request (R:G-14) */
 #define ECHO_MAX_DEPTH 32   /* depth < 32 (R:G-14) */
+#define ECHO_MAX_TOPK 16    /* echo_draft_expand: draft top-k per node (the configs use 8, 10, 16) */
 #define ECHO_CALIB_MAX_PER_DEPTH 24576 /* echo_calibrate sorts one depth's samples in shared memory */
 #define ECHO_CALIB_WORKSPACE_BYTES (256 + (size_t)ECHO_MAX_DEPTH * ECHO_CALIB_MAX_PER_DEPTH * 4)
 #define ECHO_MAX_ACCEPT 32  /* an accepted path has <= 32 nodes (one per depth) */
@@ -201,6 +203,24 @@ int echo_gate_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, E
                    echo_stream_t stream);
 int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, const uint64_t* local_keys,
                           const uint64_t* all_keys, int64_t n_all, EchoSelection* out, echo_stream_t stream);
+
+/* ---- draft-side tree construction ------------------------------------ */
+/* The draft model's outputs for one level: every node of the previous level (one virtual root with score 0 at level 0,
+ * else topk nodes in their slot order) proposes its topk most likely next tokens with their log-probabilities. */
+typedef struct {
+  int32_t level, topk;        /* 0 <= level < 32, 1 <= topk <= ECHO_MAX_TOPK */
+  const float* parent_score;  /* dev [R][k_prev]: cumulative scores of the previous level (zeros at level 0) */
+  const float* child_logq;    /* dev [R][k_prev][topk], natural log, <= 0 */
+  const int32_t* child_token; /* dev [R][k_prev][topk] */
+} EchoDraftLevel;
+/* Appends level `level` to every request's candidate tree in place ("G_i.append(topk tokens)", Alg. 1 l.10):
+ * the topk candidates with the best cumulative score fl32(S_parent + logq) (Eq. 5), ties by (parent slot, child rank),
+ * become nodes cand_offsets[i] + level*topk + slot with parent (level-1)*topk + parent slot (-1 at level 0), their logq
+ * and token; score_out [R][topk] is the next call's parent_score.  trees->parent / logq (written here, hence not
+ * const in effect) and token [total_cand] are caller-owned device arrays with room for (level+1)*topk nodes per request
+ * (status bit otherwise).  Readings R:D-1..D-3. */
+int echo_draft_expand(EchoCtx* ctx, const EchoDraftLevel* draft, EchoTrees* trees, int32_t* token, float* score_out,
+                      echo_stream_t stream);
 
 /* ---- warm-up calibration of the gates ------------------------------ */
 /* Traces collected during warm-up: one sample per (request, depth) with the layer confidence

@@ -171,6 +171,17 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
   return launch_verify_attn(ctx, sel, kv, layer, Hq, R, q, out, lse, sm_scale, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int echo_draft_expand(EchoCtx* ctx, const EchoDraftLevel* l, EchoTrees* t, int32_t* token, float* score_out,
+                      echo_stream_t stream) {
+  if (!ctx || !l || !t) return ECHO_ERR_INVALID_ARG;
+  if (t->num_requests < 0 || l->level < 0 || l->topk < 1) return ECHO_ERR_INVALID_ARG;
+  if (l->level >= ECHO_MAX_DEPTH || l->topk > ECHO_MAX_TOPK) return ECHO_ERR_UNSUPPORTED;
+  if (t->num_requests > 0 && (!t->cand_offsets || !t->parent || !t->logq || !token || !score_out || !l->parent_score ||
+                              !l->child_logq || !l->child_token))
+    return ECHO_ERR_INVALID_ARG;
+  return launch_draft_expand(ctx, l, t, token, score_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int echo_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibration* o, echo_stream_t stream) {
   if (!ctx || !t || !o) return ECHO_ERR_INVALID_ARG;
   if (t->num_samples < 0 || !(delta == delta)) return ECHO_ERR_INVALID_ARG;

@@ -27,7 +27,7 @@ DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
            "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept",
-           "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys"]
+           "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand"]
 
 
 class EchoTrees(C.Structure):
@@ -75,6 +75,13 @@ class EchoCalibration(C.Structure):
                 ("depth_mask", C.c_void_p)]
 
 
+class EchoDraftLevel(C.Structure):
+    _fields_ = [("level", C.c_int32), ("topk", C.c_int32), ("parent_score", C.c_void_p), ("child_logq", C.c_void_p),
+                ("child_token", C.c_void_p)]
+
+
+MAX_TOPK = 16
+DEV_TREE_OVERFLOW = 64
 CALIB_MAX_PER_DEPTH = 24576
 CALIB_WORKSPACE_BYTES = 256 + 32 * CALIB_MAX_PER_DEPTH * 4
 DEV_BAD_TRACE, DEV_CALIB_OVERFLOW = 16, 32
@@ -113,6 +120,8 @@ def load_library():
     lib.echo_gate_select_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), C.c_void_p, C.c_void_p, C.c_int64,
                                           P(EchoSelection), C.c_void_p]
     lib.echo_gate_select_keys.restype = C.c_int
+    lib.echo_draft_expand.argtypes = [C.c_void_p, P(EchoDraftLevel), P(EchoTrees), C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.echo_draft_expand.restype = C.c_int
     lib.echo_calibrate.argtypes = [C.c_void_p, P(EchoTraces), C.c_double, P(EchoCalibration), C.c_void_p]
     lib.echo_calibrate.restype = C.c_int
     lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
@@ -372,6 +381,18 @@ class EchoContext:
                           torch.zeros(r, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(r, MAX_ACCEPT, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(max(1, capacity), **i32))
+
+    def draft_expand(self, level: int, topk: int, parent_score, child_logq, child_token, cand_offsets, parent, logq,
+                     token, score_out, max_cand: int = 128):
+        """echo_draft_expand: appends level `level` (topk nodes per request) to the candidate trees in place.
+        parent_score f32 [R][k_prev], child_logq f32 / child_token i32 [R][k_prev][topk]; cand_offsets / parent / logq
+        are the EchoTrees arrays, token i32 [N], score_out f32 [R][topk] (the next level's parent_score)."""
+        R = cand_offsets.numel() - 1
+        lv = EchoDraftLevel(int(level), int(topk), _ptr(parent_score), _ptr(child_logq), _ptr(child_token))
+        trees = EchoTrees(R, parent.numel(), max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
+        self._check(self.lib.echo_draft_expand(self._h, C.byref(lv), C.byref(trees), _ptr(token), _ptr(score_out),
+                                               self._stream()))
+        return score_out
 
     def calibrate(self, depth, conf, accepted, delta: float):
         """echo_calibrate.  depth / accepted uint8 and conf float32 device tensors of M warm-up samples ->

@@ -397,3 +397,13 @@ def draw_calibration_traces(rng, M: int, ties: bool = False, separation=(0.7, 0.
     if ties:
         conf = np.maximum(np.round(conf * 64) / 64, 1.0 / 64)
     return depth, conf.astype(np.float32), acc.astype(np.uint8)
+
+
+def draw_draft_level(rng, R: int, k_prev: int, k: int, vocab: int = 32000, alpha: float = 0.3):
+    """Stand-in for the draft model's output at one level: each of the k_prev parents proposes its k most likely next
+    tokens, probabilities Dirichlet(alpha) sorted descending (as a top-k would return them), tokens distinct among
+    siblings.  logq = (float) log(probability) taken here on the host (SURVEY G-2).  No method arithmetic."""
+    pr = -np.sort(-rng.dirichlet(np.full(k, alpha), size=(R, k_prev)), axis=-1)
+    logq = np.log(np.maximum(pr, 1e-30)).astype(np.float32)
+    tok = np.stack([[rng.choice(vocab, k, replace=False) for _ in range(k_prev)] for _ in range(R)]).astype(np.int32)
+    return logq, tok
