@@ -410,3 +410,68 @@ def draft_expand(level, k, parent_score, child_logq, child_token):
             token[i, slot] = child_token[i, p, c]
             score[i, slot] = s
     return dict(sel_parent=sel_parent, logq=logq, token=token, score=score)
+
+
+# ---------------------------------------------------------------- O13 (NEXT-2): stochastic tree acceptance
+def softmax_bits(row_bits, vocab, temperature):
+    """softmax(logits / T) of one bf16 row in fp64 (plain definition)."""
+    x = bf16_bits_to_f64(np.asarray(row_bits)[:vocab]) / float(np.float32(temperature))
+    x = x - x.max()
+    e = np.exp(x)
+    return e / e.sum()
+
+
+def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vocab, temperature, u_accept, u_bonus, R):
+    """Tree acceptance at temperature > 0 under the speculative-sampling conditions the paper cites,
+    in the multi-round form tree drafters use when the draft proposes its top-k deterministically (so q = 1 on a
+    proposed token; readings R:T-1..T-4).  Per request, starting from the distribution p after the last
+    committed token (root_logits) with nothing removed: the children of the current node are tried in packed order;
+    child c with token x is accepted iff u_accept[c] < p'(x), p' = p with the tokens rejected so far at this node
+    removed and renormalised; a rejected token is removed; an accepted child becomes the current node and p becomes
+    softmax(target_logits[c] / T).  When no child is accepted the bonus token is drawn from the residual p' by
+    inverse CDF in vocabulary order with u_bonus[i] (smallest v whose cumulative residual mass exceeds u (1 - m)).
+    Emits exactly p at every position (checked in the pins).  Returns accept_len / accept_idx / last_node /
+    bonus_token like `accept`, plus for the tests: final_p_removed (the residual distribution's removed tokens)."""
+    offs = sel["sel_offsets"]
+    accept_len = np.zeros(R, np.int32)
+    last_node = np.full(R, -1, np.int32)
+    bonus = np.full(R, -1, np.int32)
+    accept_idx = np.full((R, 32), -1, np.int32)
+    margins = []  # |u - p'| of every decision and the CDF gap around the bonus draw: the GPU tests skip knife edges
+    for i in range(R):
+        b, e = int(offs[i]), int(offs[i + 1])
+        pl = [int(x) for x in sel["parent_local"][b:e]]
+        p = softmax_bits(root_logits_bits[i], vocab, temperature)
+        cur, path = -1, []
+        while True:
+            removed, m, nxt = [], 0.0, None
+            for c in [l for l in range(e - b) if pl[l] == cur]:
+                x = int(draft_token[b + c])
+                px = 0.0 if x in removed else float(p[x])
+                pr = px / (1.0 - m) if (1.0 - m) > 0.0 else 0.0
+                u = float(np.float32(u_accept[b + c]))
+                margins.append(abs(u - pr))
+                if u < pr:
+                    nxt = c
+                    break
+                if x not in removed:
+                    removed.append(x)
+                    m += float(p[x])
+            if nxt is None or len(path) >= 32:
+                break
+            path.append(nxt)
+            cur = nxt
+            p = softmax_bits(target_logits_bits[b + nxt], vocab, temperature)
+        r = p.copy()
+        r[removed] = 0.0
+        cdf = np.cumsum(r)
+        target = float(np.float32(u_bonus[i])) * cdf[-1]
+        v = int(np.searchsorted(cdf, target, side="right"))
+        v = min(v, int(np.flatnonzero(r)[-1]))
+        margins.append(min(abs(target - (cdf[v - 1] if v > 0 else 0.0)), abs(cdf[v] - target)) / cdf[-1])
+        bonus[i] = v
+        accept_len[i] = len(path)
+        accept_idx[i, :len(path)] = [b + a for a in path]
+        last_node[i] = b + cur if cur >= 0 else -1
+    return dict(accept_len=accept_len, accept_idx=accept_idx, last_node=last_node, bonus_token=bonus,
+                min_margin=min(margins) if margins else 1.0)
