@@ -204,6 +204,29 @@ int echo_gate_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, E
 int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, const uint64_t* local_keys,
                           const uint64_t* all_keys, int64_t n_all, EchoSelection* out, echo_stream_t stream);
 
+/* ---- acceptance at temperature > 0 ----------------------------------- */
+typedef struct {
+  const int32_t* draft_token; /* dev [capacity], packed order */
+  const void* target_logits;  /* dev bf16 [capacity][ld]: the target's logits after each packed node */
+  const void* root_logits;    /* dev bf16 [R][ld]: the target's logits after the last committed token of each request */
+  int32_t vocab;
+  int64_t ld;                 /* row pitch in elements, multiple of 8; rows 16-byte aligned */
+  float temperature;          /* > 0 */
+  const float* u_accept;      /* dev [capacity]: uniform [0,1) draws, one per packed node (used when the node is tried) */
+  const float* u_bonus;       /* dev [R]: uniform [0,1) draws for the bonus tokens */
+} EchoSampleInputs;
+/* Tree acceptance under the speculative-sampling conditions in the multi-round form of tree drafters
+ * whose proposals are their deterministic top-k (q = 1 on a proposed token; readings R:T-1..T-4): from the
+ * distribution p = softmax(root_logits / T) of a request, the children of the current node are tried in packed order;
+ * child c with token x is accepted iff u_accept[c] < p'(x), where p' is p with the tokens already rejected at this
+ * node removed and renormalised; an accepted child becomes the current node (p = softmax(target_logits[c] / T)); when
+ * none is accepted, bonus_token is drawn from p' by inverse CDF in vocabulary order with u_bonus.  Every emitted token
+ * is distributed exactly as the target's p.  Probabilities are fp32 (ex2.approx), so a draw within ~1e-5 of its
+ * threshold may fall either way.  Outputs and KV compaction as echo_accept (target_token_out unused).  Needs
+ * (capacity + R) * 8 bytes of context workspace. */
+int echo_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoSampleInputs* in, int32_t num_requests,
+                           EchoPagedKV* kv, EchoAccept* out, echo_stream_t stream);
+
 /* ---- draft-side tree construction ------------------------------------ */
 /* The draft model's outputs for one level: every node of the previous level (one virtual root with score 0 at level 0,
  * else topk nodes in their slot order) proposes its topk most likely next tokens with their log-probabilities. */

@@ -431,13 +431,16 @@ def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vo
     softmax(target_logits[c] / T).  When no child is accepted the bonus token is drawn from the residual p' by
     inverse CDF in vocabulary order with u_bonus[i] (smallest v whose cumulative residual mass exceeds u (1 - m)).
     Emits exactly p at every position (checked in the pins).  Returns accept_len / accept_idx / last_node /
-    bonus_token like `accept`, plus for the tests: final_p_removed (the residual distribution's removed tokens)."""
+    bonus_token like `accept`, plus for the tests: min_margin (smallest |u - p'| over the decisions) and, per request,
+    the normalised residual CDF and the bonus draw (a token t is a valid draw within eps iff
+    cdf[t-1] - eps <= u <= cdf[t] + eps and its residual mass is positive)."""
     offs = sel["sel_offsets"]
     accept_len = np.zeros(R, np.int32)
     last_node = np.full(R, -1, np.int32)
     bonus = np.full(R, -1, np.int32)
     accept_idx = np.full((R, 32), -1, np.int32)
-    margins = []  # |u - p'| of every decision and the CDF gap around the bonus draw: the GPU tests skip knife edges
+    margins = []  # |u - p'| of every accept / reject decision: the GPU tests redraw uniforms that sit on a knife edge
+    cdfs, targets = [], []  # residual CDF and u (1 - m) of the bonus draw: neighbouring tokens are a rounding apart
     for i in range(R):
         b, e = int(offs[i]), int(offs[i + 1])
         pl = [int(x) for x in sel["parent_local"][b:e]]
@@ -468,10 +471,11 @@ def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vo
         target = float(np.float32(u_bonus[i])) * cdf[-1]
         v = int(np.searchsorted(cdf, target, side="right"))
         v = min(v, int(np.flatnonzero(r)[-1]))
-        margins.append(min(abs(target - (cdf[v - 1] if v > 0 else 0.0)), abs(cdf[v] - target)) / cdf[-1])
+        cdfs.append(cdf / cdf[-1])
+        targets.append(target / cdf[-1])
         bonus[i] = v
         accept_len[i] = len(path)
         accept_idx[i, :len(path)] = [b + a for a in path]
         last_node[i] = b + cur if cur >= 0 else -1
     return dict(accept_len=accept_len, accept_idx=accept_idx, last_node=last_node, bonus_token=bonus,
-                min_margin=min(margins) if margins else 1.0)
+                min_margin=min(margins) if margins else 1.0, bonus_cdf=cdfs, bonus_u=targets)

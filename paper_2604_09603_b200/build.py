@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libecho.so")
-SOURCES = ["api.cu", "gate_select.cu", "verify_attn.cu", "verify_attn_tc.cu", "accept.cu", "calibrate.cu", "draft_expand.cu"]
+SOURCES = ["api.cu", "gate_select.cu", "verify_attn.cu", "verify_attn_tc.cu", "accept.cu", "calibrate.cu", "draft_expand.cu", "accept_stochastic.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

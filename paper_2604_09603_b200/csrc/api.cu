@@ -171,6 +171,23 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
   return launch_verify_attn(ctx, sel, kv, layer, Hq, R, q, out, lse, sm_scale, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int echo_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoSampleInputs* in, int32_t R, EchoPagedKV* kv,
+                           EchoAccept* out, echo_stream_t stream) {
+  if (!ctx || !sel || !in || !out) return ECHO_ERR_INVALID_ARG;
+  int rc = check_kv(kv, false);
+  if (rc != ECHO_OK) return rc;
+  if (R < 0 || sel->capacity < 0 || in->vocab <= 0 || in->ld < in->vocab || !(in->temperature > 0.f)) return ECHO_ERR_INVALID_ARG;
+  if (in->ld % 8 != 0) return ECHO_ERR_UNSUPPORTED;
+  if (!sel->sel_offsets || !sel->n_selected || !in->root_logits || !in->u_bonus) return ECHO_ERR_INVALID_ARG;
+  if (sel->capacity > 0 && (!sel->parent_local || !in->draft_token || !in->target_logits || !in->u_accept))
+    return ECHO_ERR_INVALID_ARG;
+  if (misaligned(in->target_logits, 16) || misaligned(in->root_logits, 16)) return ECHO_ERR_INVALID_ARG;
+  if (!out->accept_len || !out->last_node || !out->bonus_token || !out->new_len || !out->accept_idx || !out->slot_src ||
+      !out->slot_dst)
+    return ECHO_ERR_INVALID_ARG;
+  return launch_accept_stochastic(ctx, sel, in, R, kv, out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int echo_draft_expand(EchoCtx* ctx, const EchoDraftLevel* l, EchoTrees* t, int32_t* token, float* score_out,
                       echo_stream_t stream) {
   if (!ctx || !l || !t) return ECHO_ERR_INVALID_ARG;

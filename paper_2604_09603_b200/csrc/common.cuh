@@ -61,6 +61,8 @@ int launch_gate_keys(EchoCtx*, const EchoTrees*, const EchoGate*, EchoSelection*
 int launch_gate_select_keys(EchoCtx*, const EchoTrees*, const EchoGate*, const uint64_t* local_keys,
                             const uint64_t* all_keys, int64_t n_all, EchoSelection*, cudaStream_t);
 int launch_draft_expand(EchoCtx*, const EchoDraftLevel*, EchoTrees*, int32_t* token, float* score_out, cudaStream_t);
+int launch_accept_stochastic(EchoCtx*, const EchoSelection*, const EchoSampleInputs*, int32_t R, EchoPagedKV*, EchoAccept*,
+                             cudaStream_t);
 int launch_calibrate(EchoCtx*, const EchoTraces*, double delta, EchoCalibration*, cudaStream_t);
 int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
                        const void* q, void* out, float* lse, float sm_scale, cudaStream_t);

@@ -27,7 +27,8 @@ DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
            "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept",
-           "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand"]
+           "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand",
+           "echo_accept_stochastic"]
 
 
 class EchoTrees(C.Structure):
@@ -75,6 +76,12 @@ class EchoCalibration(C.Structure):
                 ("depth_mask", C.c_void_p)]
 
 
+class EchoSampleInputs(C.Structure):
+    _fields_ = [("draft_token", C.c_void_p), ("target_logits", C.c_void_p), ("root_logits", C.c_void_p),
+                ("vocab", C.c_int32), ("ld", C.c_int64), ("temperature", C.c_float), ("u_accept", C.c_void_p),
+                ("u_bonus", C.c_void_p)]
+
+
 class EchoDraftLevel(C.Structure):
     _fields_ = [("level", C.c_int32), ("topk", C.c_int32), ("parent_score", C.c_void_p), ("child_logq", C.c_void_p),
                 ("child_token", C.c_void_p)]
@@ -120,6 +127,9 @@ def load_library():
     lib.echo_gate_select_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), C.c_void_p, C.c_void_p, C.c_int64,
                                           P(EchoSelection), C.c_void_p]
     lib.echo_gate_select_keys.restype = C.c_int
+    lib.echo_accept_stochastic.argtypes = [C.c_void_p, P(EchoSelection), P(EchoSampleInputs), C.c_int32, P(EchoPagedKV),
+                                           P(EchoAccept), C.c_void_p]
+    lib.echo_accept_stochastic.restype = C.c_int
     lib.echo_draft_expand.argtypes = [C.c_void_p, P(EchoDraftLevel), P(EchoTrees), C.c_void_p, C.c_void_p, C.c_void_p]
     lib.echo_draft_expand.restype = C.c_int
     lib.echo_calibrate.argtypes = [C.c_void_p, P(EchoTraces), C.c_double, P(EchoCalibration), C.c_void_p]
@@ -381,6 +391,27 @@ class EchoContext:
                           torch.zeros(r, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(r, MAX_ACCEPT, **i32), torch.zeros(r, MAX_ACCEPT, **i32),
                           torch.zeros(max(1, capacity), **i32))
+
+    def accept_stochastic(self, sel: Selection, kv: PagedKV, draft_token, target_logits, root_logits, vocab: int,
+                          temperature: float, u_accept, u_bonus, out: Optional[Acceptance] = None,
+                          compact: bool = True) -> Acceptance:
+        """echo_accept_stochastic.  target_logits bf16 [capacity][ld], root_logits bf16 [R][ld] (same pitch),
+        u_accept f32 [capacity], u_bonus f32 [R]."""
+        acc = out if out is not None else self.alloc_accept(sel.R, sel.capacity)
+        self.ensure_workspace(sel.R, 0, sel.capacity, 0)
+        assert target_logits.stride(0) == root_logits.stride(0)
+        inp = EchoSampleInputs(_ptr(draft_token), _ptr(target_logits), _ptr(root_logits), int(vocab),
+                               int(root_logits.stride(0)), float(temperature), _ptr(u_accept), _ptr(u_bonus))
+        ck = kv.c_struct()
+        if not compact:
+            ck.k_pool = None
+            ck.v_pool = None
+        oa = EchoAccept(_ptr(acc.accept_len), _ptr(acc.last_node), _ptr(acc.bonus_token), _ptr(acc.new_len),
+                        _ptr(acc.accept_idx), _ptr(acc.slot_src), _ptr(acc.slot_dst), None)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_accept_stochastic(self._h, C.byref(cs), C.byref(inp), sel.R, C.byref(ck), C.byref(oa),
+                                                    self._stream()))
+        return acc
 
     def draft_expand(self, level: int, topk: int, parent_score, child_logq, child_token, cand_offsets, parent, logq,
                      token, score_out, max_cand: int = 128):
