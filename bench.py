@@ -238,6 +238,13 @@ def run_gpu(args, rank, world, local_rank):
         logits = W.draw_logits(wl, glob, device=str(dev))
         if logits.shape[0] < cap:
             logits = torch.cat([logits, torch.zeros(cap - logits.shape[0], logits.shape[1], dtype=logits.dtype, device=dev)])
+    root_logits = u_acc = u_bon = None
+    if logits is not None and args.temperature > 0:  # acceptance at temperature > 0 (NEXT-2) instead of the argmax
+        gen = torch.Generator(device=dev).manual_seed(W.SEED_BASE + 7)
+        root_logits = torch.randn(wl.R, logits.shape[1], generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
+        root_logits[torch.arange(wl.R, device=dev), d(wl.prev_token).long()] += 8.0
+        u_acc = torch.rand(cap, generator=gen, device=dev)
+        u_bon = torch.rand(wl.R, generator=gen, device=dev)
     bytes_alg, flops_alg = algorithmic_bytes(wl, sel_h)
     if heads:
         bytes_alg, flops_alg = bytes_alg // world, flops_alg // world
@@ -256,7 +263,10 @@ def run_gpu(args, rank, world, local_rank):
         ctx.verify_attn(sel_, kv, qq, SM_SCALE, out=out_, lse=lse_)
         if i is not None:
             attn_ev[i][1].record()
-        if logits is not None:
+        if logits is not None and args.temperature > 0:
+            ctx.accept_stochastic(sel_, kv, din["draft"], logits, root_logits, wl.vocab, args.temperature, u_acc, u_bon,
+                                  out=acc_)
+        elif logits is not None:
             ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc_)
         else:
             ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=din["target"], out=acc_)
@@ -410,6 +420,8 @@ def main():
                     help="N > 1: requests = each rank its own batch (weak); heads = KV-head shards of one batch (strong)")
     ap.add_argument("--global-budget", action="store_true",
                     help="request-sharded ranks share ONE budget of N x B: keys are all-gathered before the select")
+    ap.add_argument("--temperature", type=float, default=0.0,
+                    help="config 4: > 0 accepts by speculative sampling at this temperature instead of greedy argmax")
     ap.add_argument("--static", action="store_true", help="cfg2's static-tree comparison run: 60 fixed nodes per request, gates off")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
@@ -451,7 +463,8 @@ def main():
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "strong" if r["heads"] else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
-                           + (" global-budget" if args.global_budget else "") + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
+                           + (" global-budget" if args.global_budget else "")
+                           + (f" temperature={args.temperature}" if args.temperature > 0 and args.config == 4 else "") + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
                            "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",

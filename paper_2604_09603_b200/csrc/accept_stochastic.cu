@@ -18,6 +18,8 @@ constexpr int PAGE = 16;
 constexpr int ST_THREADS = 256;
 constexpr int ST_UNROLL = 4;
 constexpr int WS_THREADS = 256;
+constexpr int SEG = 256;        // tokens per CDF segment: one coalesced warp load
+constexpr int MAX_SEGS = 1024;  // vocabulary <= 262 144
 
 __device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
   uint4 r;
@@ -102,7 +104,7 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
   __shared__ float s_removed_w[ECHO_MAX_CAND];
   __shared__ int s_L, s_cur, s_nrem, s_pick_seg;
   __shared__ float s_remw, s_prefix;
-  __shared__ float s_seg[WS_THREADS];
+  __shared__ float s_seg[MAX_SEGS];
   pdl_wait();  // statistics come from k_softmax_stats; the attention kernel before it reads the pools compacted below
   const int i = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
   const int b = sel_offsets[i], Ki = min(sel_offsets[i + 1] - b, ECHO_MAX_CAND);
@@ -112,25 +114,39 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
     // ---- the walk (R:T-1..T-3): every lane runs the same control flow, lane = child for the gathers ----
     int cur = -1, L = 0, nrem = 0;
     float remw = 0.f;
+    int pl[4], tok[4];  // this lane's four packed nodes: loaded once, so that a level costs one gather round trip
+    float ua[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int l = w * 32 + lane;
+      pl[w] = l < Ki ? parent_local[b + l] : -2;
+      tok[w] = l < Ki ? draft_token[b + l] : -1;
+      ua[w] = l < Ki ? u_accept[b + l] : 2.f;
+    }
     while (true) {
       const float2 mz = cur < 0 ? stats[cap + i] : stats[b + cur];
       const __nv_bfloat16* rowp = cur < 0 ? root_logits + (size_t)i * ld : target_logits + (size_t)(b + cur) * ld;
       nrem = 0;
       remw = 0.f;
       int accepted = -1;
-      for (int w = 0; w < 4 && accepted < 0; ++w) {
-        const int l = w * 32 + lane;
-        const bool is_child = l < Ki && parent_local[b + l] == cur;
-        const int x = is_child ? draft_token[b + l] : -1;
-        const bool tok_ok = is_child && x >= 0 && x < vocab;
-        const float wgt = tok_ok ? ex2f((__bfloat162float(rowp[x]) - mz.x) * c) : 0.f;
-        const float u = is_child ? u_accept[b + l] : 2.f;
+      float wgt[4];
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        const bool tok_ok = pl[w] == cur && tok[w] >= 0 && tok[w] < vocab;
+        wgt[w] = tok_ok ? ex2f((__bfloat162float(rowp[tok[w]]) - mz.x) * c) : 0.f;
+      }
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        if (accepted >= 0) break;
+        const bool is_child = pl[w] == cur;
+        const int x = is_child ? tok[w] : -1;
+        const float u = is_child ? ua[w] : 2.f;
         unsigned cm = __ballot_sync(0xffffffffu, is_child);
         while (cm) {
           const int j = __ffs(cm) - 1;
           cm &= cm - 1;
           const int xj = __shfl_sync(0xffffffffu, x, j);
-          const float wj = __shfl_sync(0xffffffffu, wgt, j), uj = __shfl_sync(0xffffffffu, u, j);
+          const float wj = __shfl_sync(0xffffffffu, wgt[w], j), uj = __shfl_sync(0xffffffffu, u, j);
           bool dup = false;
           for (int r = 0; r < nrem; ++r) dup |= s_removed[r] == xj;
           const float px = dup ? 0.f : wj;
@@ -173,44 +189,105 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
   __syncthreads();
 
   // ---- bonus token from the residual distribution of the last node, inverse CDF in vocabulary order (R:T-4) ----
+  // Segments of 256 consecutive tokens: a warp loads one with 32 coalesced 16-byte loads and reduces it to one sum;
+  // thread 0 walks the <= 1024 segment sums to the segment that holds the draw; warp 0 resolves it inside.
   {
-    const int cur = s_cur, nrem = s_nrem;
+    const int cur = s_cur, nrem = s_nrem, warp = tid >> 5;
     const float2 mz = cur < 0 ? stats[cap + i] : stats[b + cur];
     const __nv_bfloat16* rowp = cur < 0 ? root_logits + (size_t)i * ld : target_logits + (size_t)(b + cur) * ld;
-    const int seg = (vocab + WS_THREADS - 1) / WS_THREADS;
-    const int lo = min(vocab, tid * seg), hi = min(vocab, lo + seg);
-    float sum = 0.f;
-    for (int v = lo; v < hi; ++v) sum += ex2f((__bfloat162float(rowp[v]) - mz.x) * c);
-    s_seg[tid] = sum;
+    const int nseg = (vocab + SEG - 1) / SEG;
+    auto load8 = [&](int base, float (&w)[8]) {  // weights of tokens base .. base+7 (0 past the vocabulary)
+      if (base + 8 <= vocab) {
+        const uint4 u = ldg_stream(reinterpret_cast<const uint4*>(rowp + base));
+        const uint32_t q[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          w[2 * e] = ex2f((bf16_lo(q[e]) - mz.x) * c);
+          w[2 * e + 1] = ex2f((bf16_hi(q[e]) - mz.x) * c);
+        }
+      } else {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) w[e] = base + e < vocab ? ex2f((__bfloat162float(rowp[base + e]) - mz.x) * c) : 0.f;
+      }
+    };
+    constexpr int NW = WS_THREADS / 32, UNR = 4;
+    for (int s0 = warp; s0 < nseg; s0 += UNR * NW) {  // four segments' loads in flight per warp
+      uint4 u[UNR];
+#pragma unroll
+      for (int t = 0; t < UNR; ++t) {
+        const int base = (s0 + t * NW) * SEG + lane * 8;
+        u[t] = make_uint4(0u, 0u, 0u, 0u);
+        if (base + 8 <= vocab) u[t] = ldg_stream(reinterpret_cast<const uint4*>(rowp + base));
+      }
+#pragma unroll
+      for (int t = 0; t < UNR; ++t) {
+        const int sgm = s0 + t * NW, base = sgm * SEG + lane * 8;
+        if (sgm >= nseg) break;  // warp-uniform
+        float w[8];
+        if (base + 8 <= vocab) {
+          const uint32_t q[4] = {u[t].x, u[t].y, u[t].z, u[t].w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            w[2 * e] = ex2f((bf16_lo(q[e]) - mz.x) * c);
+            w[2 * e + 1] = ex2f((bf16_hi(q[e]) - mz.x) * c);
+          }
+        } else {
+          load8(base, w);
+        }
+        float sum = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+#pragma unroll
+        for (int ofs = 16; ofs; ofs >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, ofs);
+        if (lane == 0) s_seg[sgm] = sum;
+      }
+    }
     __syncthreads();
-    if (tid < nrem) atomicAdd(&s_seg[s_removed[tid] / seg], -s_removed_w[tid]);
+    if (tid < nrem) atomicAdd(&s_seg[s_removed[tid] / SEG], -s_removed_w[tid]);
     __syncthreads();
     const float target = u_bonus[i] * (mz.y - s_remw);
     if (tid == 0) {
       float run = 0.f;
       int pick = -1, last_pos = 0;
-      for (int s = 0; s < WS_THREADS; ++s) {
-        const float w = s_seg[s];
-        if (w > 0.f) last_pos = s;
-        if (pick < 0 && run + w > target) { pick = s; s_prefix = run; }
-        if (pick < 0) run += w;
+      for (int sgm = 0; sgm < nseg; ++sgm) {
+        const float w = s_seg[sgm];
+        if (w > 0.f) last_pos = sgm;
+        if (run + w > target) { pick = sgm; break; }
+        run += w;
       }
-      if (pick < 0) { pick = last_pos; s_prefix = -INFINITY; }  // rounding left the target past the end: last token
+      s_prefix = run;
+      if (pick < 0) { pick = last_pos; s_prefix = -INFINITY; }  // rounding left the draw past the end: last token
       s_pick_seg = pick;
     }
     __syncthreads();
-    if (tid == s_pick_seg) {
-      float acc = s_prefix;
-      int pick = -1, last_nz = lo;
-      for (int v = lo; v < hi; ++v) {
-        bool rem = false;
-        for (int r = 0; r < nrem; ++r) rem |= s_removed[r] == v;
-        const float w = rem ? 0.f : ex2f((__bfloat162float(rowp[v]) - mz.x) * c);
-        if (w > 0.f) last_nz = v;
-        acc += w;
-        if (acc > target) { pick = v; break; }
+    if (tid < 32) {
+      const int base = s_pick_seg * SEG + lane * 8;
+      float w[8];
+      load8(base, w);
+#pragma unroll
+      for (int e = 0; e < 8; ++e)
+        for (int r = 0; r < nrem; ++r)
+          if (s_removed[r] == base + e) w[e] = 0.f;
+      const float mine = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+      float incl = mine;
+#pragma unroll
+      for (int ofs = 1; ofs < 32; ofs <<= 1) {
+        const float t = __shfl_up_sync(0xffffffffu, incl, ofs);
+        if (lane >= ofs) incl += t;
       }
-      bonus_token[i] = pick >= 0 ? pick : last_nz;
+      const float before = s_prefix + (incl - mine);
+      int pick = -1, last_nz = -1;
+      float acc = before;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        if (w[e] > 0.f) last_nz = base + e;
+        acc += w[e];
+        if (pick < 0 && w[e] > 0.f && acc > target) pick = base + e;
+      }
+      const unsigned found = __ballot_sync(0xffffffffu, pick >= 0);
+      const unsigned nz = __ballot_sync(0xffffffffu, last_nz >= 0);
+      int out_tok;
+      if (found) out_tok = __shfl_sync(0xffffffffu, pick, __ffs(found) - 1);
+      else out_tok = nz ? __shfl_sync(0xffffffffu, last_nz, 31 - __clz(nz)) : 0;
+      if (lane == 0) bonus_token[i] = out_tok;
     }
   }
 

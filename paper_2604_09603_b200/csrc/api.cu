@@ -177,7 +177,7 @@ int echo_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoSam
   int rc = check_kv(kv, false);
   if (rc != ECHO_OK) return rc;
   if (R < 0 || sel->capacity < 0 || in->vocab <= 0 || in->ld < in->vocab || !(in->temperature > 0.f)) return ECHO_ERR_INVALID_ARG;
-  if (in->ld % 8 != 0) return ECHO_ERR_UNSUPPORTED;
+  if (in->ld % 8 != 0 || in->vocab > 262144) return ECHO_ERR_UNSUPPORTED;
   if (!sel->sel_offsets || !sel->n_selected || !in->root_logits || !in->u_bonus) return ECHO_ERR_INVALID_ARG;
   if (sel->capacity > 0 && (!sel->parent_local || !in->draft_token || !in->target_logits || !in->u_accept))
     return ECHO_ERR_INVALID_ARG;
