@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
 
   // ---- bonus token from the residual distribution of the last node, inverse CDF in vocabulary order (R:T-4) ----
   // Segments of 256 consecutive tokens: a warp loads one with 32 coalesced 16-byte loads and reduces it to one sum;
-  // thread 0 walks the <= 1024 segment sums to the segment that holds the draw; warp 0 resolves it inside.
+  // warp 0 scans the <= 1024 segment sums to the segment that holds the draw and resolves it inside.
   {
     const int cur = s_cur, nrem = s_nrem, warp = tid >> 5;
     const float2 mz = cur < 0 ? stats[cap + i] : stats[b + cur];
@@ -210,8 +210,8 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
         for (int e = 0; e < 8; ++e) w[e] = base + e < vocab ? ex2f((__bfloat162float(rowp[base + e]) - mz.x) * c) : 0.f;
       }
     };
-    constexpr int NW = WS_THREADS / 32, UNR = 4;
-    for (int s0 = warp; s0 < nseg; s0 += UNR * NW) {  // four segments' loads in flight per warp
+    constexpr int NW = WS_THREADS / 32, UNR = 8;
+    for (int s0 = warp; s0 < nseg; s0 += UNR * NW) {  // eight segments' loads in flight per warp
       uint4 u[UNR];
 #pragma unroll
       for (int t = 0; t < UNR; ++t) {
@@ -244,18 +244,32 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
     if (tid < nrem) atomicAdd(&s_seg[s_removed[tid] / SEG], -s_removed_w[tid]);
     __syncthreads();
     const float target = u_bonus[i] * (mz.y - s_remw);
-    if (tid == 0) {
-      float run = 0.f;
-      int pick = -1, last_pos = 0;
-      for (int sgm = 0; sgm < nseg; ++sgm) {
-        const float w = s_seg[sgm];
-        if (w > 0.f) last_pos = sgm;
-        if (run + w > target) { pick = sgm; break; }
-        run += w;
+    if (tid < 32) {  // lane = a run of consecutive segments; warp scan of the runs, then the owning lane walks its run
+      const int per = (nseg + 31) / 32, l0 = min(nseg, lane * per), l1 = min(nseg, l0 + per);
+      float mine = 0.f;
+      for (int sgm = l0; sgm < l1; ++sgm) mine += s_seg[sgm];
+      float incl = mine;
+#pragma unroll
+      for (int ofs = 1; ofs < 32; ofs <<= 1) {
+        const float t = __shfl_up_sync(0xffffffffu, incl, ofs);
+        if (lane >= ofs) incl += t;
       }
-      s_prefix = run;
-      if (pick < 0) { pick = last_pos; s_prefix = -INFINITY; }  // rounding left the draw past the end: last token
-      s_pick_seg = pick;
+      const float before = incl - mine;
+      const unsigned hit = __ballot_sync(0xffffffffu, mine > 0.f && before + mine > target);
+      const unsigned pos = __ballot_sync(0xffffffffu, mine > 0.f);
+      const int owner = hit ? __ffs(hit) - 1 : (pos ? 31 - __clz(pos) : 0);  // past the end by rounding: last mass
+      if (lane == owner) {
+        float run = before;
+        int pick = -1, last_pos = l0;
+        for (int sgm = l0; sgm < l1; ++sgm) {
+          const float w = s_seg[sgm];
+          if (w > 0.f) last_pos = sgm;
+          if (run + w > target) { pick = sgm; break; }
+          run += w;
+        }
+        s_prefix = pick >= 0 ? run : -INFINITY;
+        s_pick_seg = pick >= 0 ? pick : last_pos;
+      }
     }
     __syncthreads();
     if (tid < 32) {
