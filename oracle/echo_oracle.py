@@ -12,6 +12,14 @@ Pins (tests/test_oracle_pins.py, `-m "not gpu"`): worked example W1
 (tests/golden/w1.json), exactly-representable chain scores, Q=0 closed form,
 chain == dense causal attention, single node == decode attention, brute-force
 dense masked softmax, Python `sorted()` selection, exhaustive path enumeration.
+Functions beyond the hot path and their pins: `select_alg1`
+(tests/test_oracle_alg1_pins.py: hand-run example tests/golden/alg1.json,
+invariants, ample budget = global top-B, order brute force), `calibrate`
+(tests/test_oracle_calibrate_pins.py: closed forms, brute force over pairs,
+scikit-learn roc_auc_score / roc_curve), `draft_expand`
+(tests/test_oracle_draft_pins.py: hand example, brute-force top-k, Eq. 5 scores of
+the built tree), `accept_stochastic` (tests/test_oracle_stochastic_pins.py: hand
+example, emitted-token distribution on a grid of uniforms, T -> 0 = `accept`).
 The paper prints no numeric example of this path, so parity with
 "the paper's values" is unpinned; every function below is pinned by the
 mathematics listed above.
