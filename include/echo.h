@@ -8,9 +8,12 @@
  *   - Every pointer marked "dev" is DEVICE memory owned by the caller; it must stay valid
  *     until the work queued on `stream` has finished.  Structs themselves are HOST memory,
  *     read during the call only.
- *   - All three compute calls are asynchronous on `stream`, never synchronise, never read a
- *     device result on the host (CUDA-graph capturable).  Data-dependent sizes
- *     (n_selected, K_i, P_i) live on the device only.
+ *   - The hot path is three calls -- echo_gate_select, echo_verify_attn, echo_accept; beside them
+ *     echo_gate_keys / echo_gate_select_keys (one budget shared by several ranks),
+ *     echo_accept_stochastic (temperature > 0), echo_calibrate (warm-up calibration of the gates)
+ *     and echo_draft_expand (draft-side tree construction).  Every compute call is asynchronous
+ *     on `stream`, never synchronises, never reads a device result on the host (CUDA-graph
+ *     capturable).  Data-dependent sizes (n_selected, K_i, P_i) live on the device only.
  *   - Return value: ECHO_OK (0) or a negative EchoStatus.  Data-dependent precondition
  *     violations cannot be seen by the host; they set bits in the device status word
  *     (echo_device_status) and leave outputs unspecified.  Nothing traps.

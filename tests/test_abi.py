@@ -45,6 +45,11 @@ def test_null_arguments_rejected(lib):
     assert lib.echo_gate_select(None, None, None, None, None) == -1
     assert lib.echo_verify_attn(None, None, None, 0, 8, 1, None, None, None, C.c_float(1.0), None) == -1
     assert lib.echo_accept(None, None, None, 0, None, None, None) == -1
+    assert lib.echo_gate_keys(None, None, None, None, None, None) == -1
+    assert lib.echo_gate_select_keys(None, None, None, None, None, 0, None, None) == -1
+    assert lib.echo_accept_stochastic(None, None, None, 0, None, None, None) == -1
+    assert lib.echo_calibrate(None, None, C.c_double(0.5), None, None) == -1
+    assert lib.echo_draft_expand(None, None, None, None, None, None) == -1
     assert lib.echo_destroy(None) == -1
     assert lib.echo_set_option(None, 1, 1) == -1
 
