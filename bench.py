@@ -252,6 +252,7 @@ def run_gpu(args, rank, world, local_rank):
     ev = lambda: torch.cuda.Event(enable_timing=True)
     attn_ev = [(ev(), ev()) for _ in range(args.steps)]
     gate_ev = [(ev(), ev()) for _ in range(args.steps)]
+    acc_ev = [ev() for _ in range(args.steps)]
 
     def step(din, i=None, qq=q, bufs=None):
         sel_, acc_, out_, lse_ = bufs or (sel, acc, out, lse)
@@ -270,6 +271,8 @@ def run_gpu(args, rank, world, local_rank):
             ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc_)
         else:
             ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=din["target"], out=acc_)
+        if i is not None:
+            acc_ev[i].record()
 
     def barrier():
         if world > 1:
@@ -292,6 +295,8 @@ def run_gpu(args, rank, world, local_rank):
     sampler.stop_flag = True
     t_attn = float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
     t_gate = float(np.mean([a.elapsed_time(b) for a, b in gate_ev]))
+    t_acc = float(np.mean([attn_ev[i][1].elapsed_time(acc_ev[i]) for i in range(args.steps)]))
+    t_attn_min = float(np.min([a.elapsed_time(b) for a, b in attn_ev]))
     accepted = int(acc.accept_len[:wl.R].sum().item())
     # the step before the path: warm-up calibration of the gates, timed outside the step
     calib_us = None
@@ -336,7 +341,7 @@ def run_gpu(args, rank, world, local_rank):
         c1.record()
         torch.cuda.synchronize()
         draft_us = c0.elapsed_time(c1) * 100.0
-    return dict(calib_us=calib_us, draft_us=draft_us, heads=heads, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
+    return dict(calib_us=calib_us, draft_us=draft_us, heads=heads, t_acc=t_acc, t_attn_min=t_attn_min, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
                 accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
                 out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
 
@@ -468,7 +473,8 @@ def main():
                            "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
                            "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
                            if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
-                           "attn_ms": r["t_attn"], "gate_ms": r["t_gate"], "attn_flops": r["flops_alg"],
+                           "attn_ms": r["t_attn"], "attn_ms_min": r["t_attn_min"], "gate_ms": r["t_gate"], "accept_ms": r["t_acc"],
+                           "yield": r["accepted"] / max(1, r["n_sel"]), "attn_flops": r["flops_alg"],
                            "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12,
                            "calibrate_us": r["calib_us"], "calibrate_samples": args.calibrate_samples,
                            "draft_tree_8x10_us": r["draft_us"]},
