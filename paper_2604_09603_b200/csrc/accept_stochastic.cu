@@ -7,8 +7,8 @@
 //                     ballot, their target probabilities gathered in parallel (lane = child), the accept / reject
 //                     sequence run in packed order with the rejected mass removed and renormalised.  Then the whole
 //                     CTA draws the bonus token from the residual distribution of the last node by inverse CDF in
-//                     vocabulary order (thread = contiguous segment, block scan of the segment sums, the owning
-//                     thread rescans its segment), and compacts the accepted KV rows like echo_accept.
+//                     vocabulary order (segments of 256 tokens reduced by coalesced warp loads, warp 0 scans the
+//                     segment sums and resolves the segment), and compacts the accepted KV rows like echo_accept.
 #include "common.cuh"
 
 namespace {
