@@ -441,13 +441,15 @@ def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vo
     Emits exactly p at every position (checked in the pins).  Returns accept_len / accept_idx / last_node /
     bonus_token like `accept`, plus for the tests: min_margin (smallest |u - p'| over the decisions) and, per request,
     the normalised residual CDF and the bonus draw (a token t is a valid draw within eps iff
-    cdf[t-1] - eps <= u <= cdf[t] + eps and its residual mass is positive)."""
+    cdf[t-1] - eps <= u <= cdf[t] + eps and its residual mass is positive), and `decisions` = (packed node, p') of
+    every accept / reject test in the order they were taken."""
     offs = sel["sel_offsets"]
     accept_len = np.zeros(R, np.int32)
     last_node = np.full(R, -1, np.int32)
     bonus = np.full(R, -1, np.int32)
     accept_idx = np.full((R, 32), -1, np.int32)
     margins = []  # |u - p'| of every accept / reject decision: the GPU tests redraw uniforms that sit on a knife edge
+    decisions = []  # (packed node, p') of every decision, so that a test can redraw just the knife-edge uniforms
     cdfs, targets = [], []  # residual CDF and u (1 - m) of the bonus draw: neighbouring tokens are a rounding apart
     for i in range(R):
         b, e = int(offs[i]), int(offs[i + 1])
@@ -462,6 +464,7 @@ def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vo
                 pr = px / (1.0 - m) if (1.0 - m) > 0.0 else 0.0
                 u = float(np.float32(u_accept[b + c]))
                 margins.append(abs(u - pr))
+                decisions.append((b + c, pr))
                 if u < pr:
                     nxt = c
                     break
@@ -486,4 +489,4 @@ def accept_stochastic(sel, draft_token, root_logits_bits, target_logits_bits, vo
         accept_idx[i, :len(path)] = [b + a for a in path]
         last_node[i] = b + cur if cur >= 0 else -1
     return dict(accept_len=accept_len, accept_idx=accept_idx, last_node=last_node, bonus_token=bonus,
-                min_margin=min(margins) if margins else 1.0, bonus_cdf=cdfs, bonus_u=targets)
+                min_margin=min(margins) if margins else 1.0, bonus_cdf=cdfs, bonus_u=targets, decisions=decisions)

@@ -37,8 +37,11 @@ __device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w 
 __device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
 
 // (m, z) <- merge with (om, oz): z counts 2^((l - m) c)
+// A side whose maximum is -inf (every logit masked, e.g. banned tokens) holds no mass: without the early return
+// (-inf) - (-inf) = NaN would reach ex2 and poison Z.
 __device__ __forceinline__ void mz_merge(float& m, float& z, float om, float oz, float c) {
-  if (om > m) { z = z * ex2f((m - om) * c) + oz; m = om; }
+  if (om == -INFINITY) return;
+  if (om > m) { z = (m == -INFINITY ? 0.f : z * ex2f((m - om) * c)) + oz; m = om; }
   else if (oz > 0.f) z += oz * ex2f((om - m) * c);
 }
 __device__ __forceinline__ void mz_chunk(float& m, float& z, const uint4 u, float c) {
@@ -48,7 +51,8 @@ __device__ __forceinline__ void mz_chunk(float& m, float& z, const uint4 u, floa
   for (int q = 0; q < 4; ++q) { x[2 * q] = bf16_lo(w[q]); x[2 * q + 1] = bf16_hi(w[q]); }
 #pragma unroll
   for (int q = 0; q < 8; ++q) cm = fmaxf(cm, x[q]);
-  if (cm > m) { z *= ex2f((m - cm) * c); m = cm; }  // m = -inf: z is 0 and stays 0 (ex2(-inf) = 0)
+  if (cm == -INFINITY) return;  // eight masked logits add nothing (and (-inf) - (-inf) would be NaN below)
+  if (cm > m) { z = m == -INFINITY ? 0.f : z * ex2f((m - cm) * c); m = cm; }
 #pragma unroll
   for (int q = 0; q < 8; ++q) z += ex2f((x[q] - m) * c);
 }
@@ -92,7 +96,7 @@ __global__ void __launch_bounds__(ST_THREADS) k_softmax_stats(const int32_t* __r
 __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
     const int32_t* __restrict__ sel_offsets, const int32_t* __restrict__ parent_local,
     const int32_t* __restrict__ draft_token, const __nv_bfloat16* __restrict__ target_logits,
-    const __nv_bfloat16* __restrict__ root_logits, int64_t ld, int vocab, int cap, float c,
+    const __nv_bfloat16* __restrict__ root_logits, int64_t ld, int vocab, int cap, float c, float c_lo,
     const float2* __restrict__ stats, const float* __restrict__ u_accept, const float* __restrict__ u_bonus,
     const int32_t* __restrict__ page_table, const int32_t* __restrict__ prefix_len, int max_pages, int Hkv,
     int num_pages, int num_layers, __nv_bfloat16* __restrict__ k_pool, __nv_bfloat16* __restrict__ v_pool,
@@ -101,9 +105,8 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
     int32_t* __restrict__ slot_dst) {
   __shared__ int s_path[ECHO_MAX_ACCEPT], s_src[ECHO_MAX_ACCEPT], s_dst[ECHO_MAX_ACCEPT];
   __shared__ int s_removed[ECHO_MAX_CAND];
-  __shared__ float s_removed_w[ECHO_MAX_CAND];
   __shared__ int s_L, s_cur, s_nrem, s_pick_seg;
-  __shared__ float s_remw, s_prefix;
+  __shared__ double s_prefix, s_target;
   __shared__ float s_seg[MAX_SEGS];
   pdl_wait();  // statistics come from k_softmax_stats; the attention kernel before it reads the pools compacted below
   const int i = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
@@ -154,7 +157,7 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
           const float pr = denom > 0.f ? px / denom : 0.f;
           if (uj < pr) { accepted = w * 32 + j; break; }
           if (!dup && xj >= 0 && xj < vocab) {  // a token outside the vocabulary is never accepted and removes nothing
-            if (lane == 0) { s_removed[nrem] = xj; s_removed_w[nrem] = wj; }
+            if (lane == 0) s_removed[nrem] = xj;
             ++nrem;
             remw += wj;
             __syncwarp();
@@ -166,7 +169,7 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
       ++L;
       cur = accepted;
     }
-    if (lane == 0) { s_L = L; s_cur = cur; s_nrem = nrem; s_remw = remw; }
+    if (lane == 0) { s_L = L; s_cur = cur; s_nrem = nrem; }
     __syncwarp();
     // slot maps, as echo_accept writes them: path node t moves from position P + a_t to P + t (R:C-6)
     if (lane < ECHO_MAX_ACCEPT) {
@@ -190,24 +193,28 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
 
   // ---- bonus token from the residual distribution of the last node, inverse CDF in vocabulary order (R:T-4) ----
   // Segments of 256 consecutive tokens: a warp loads one with 32 coalesced 16-byte loads and reduces it to one sum;
-  // warp 0 scans the <= 1024 segment sums to the segment that holds the draw and resolves it inside.
+  // warp 0 scans the <= 1024 segment sums to the segment that holds the draw and resolves it inside.  The draw is
+  // compared with the kernel's OWN total of the residual weights (not with Z of k_softmax_stats, which is summed in
+  // another order), the scans run in fp64 and the exponent argument uses c split in two floats, so that the CDF the
+  // draw is inverted on is within ~3e-7 of the exact one (ex2.approx: 2^-22 per weight, pseudo-random in sign).
   {
     const int cur = s_cur, nrem = s_nrem, warp = tid >> 5;
     const float2 mz = cur < 0 ? stats[cap + i] : stats[b + cur];
     const __nv_bfloat16* rowp = cur < 0 ? root_logits + (size_t)i * ld : target_logits + (size_t)(b + cur) * ld;
     const int nseg = (vocab + SEG - 1) / SEG;
+    auto wgt = [&](float x) { const float d = x - mz.x; return ex2f(fmaf(d, c, d * c_lo)); };
     auto load8 = [&](int base, float (&w)[8]) {  // weights of tokens base .. base+7 (0 past the vocabulary)
       if (base + 8 <= vocab) {
         const uint4 u = ldg_stream(reinterpret_cast<const uint4*>(rowp + base));
         const uint32_t q[4] = {u.x, u.y, u.z, u.w};
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-          w[2 * e] = ex2f((bf16_lo(q[e]) - mz.x) * c);
-          w[2 * e + 1] = ex2f((bf16_hi(q[e]) - mz.x) * c);
+          w[2 * e] = wgt(bf16_lo(q[e]));
+          w[2 * e + 1] = wgt(bf16_hi(q[e]));
         }
       } else {
 #pragma unroll
-        for (int e = 0; e < 8; ++e) w[e] = base + e < vocab ? ex2f((__bfloat162float(rowp[base + e]) - mz.x) * c) : 0.f;
+        for (int e = 0; e < 8; ++e) w[e] = base + e < vocab ? wgt(__bfloat162float(rowp[base + e])) : 0.f;
       }
     };
     constexpr int NW = WS_THREADS / 32, UNR = 8;
@@ -228,8 +235,8 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
           const uint32_t q[4] = {u[t].x, u[t].y, u[t].z, u[t].w};
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            w[2 * e] = ex2f((bf16_lo(q[e]) - mz.x) * c);
-            w[2 * e + 1] = ex2f((bf16_hi(q[e]) - mz.x) * c);
+            w[2 * e] = wgt(bf16_lo(q[e]));
+            w[2 * e + 1] = wgt(bf16_hi(q[e]));
           }
         } else {
           load8(base, w);
@@ -241,59 +248,62 @@ __global__ void __launch_bounds__(WS_THREADS) k_walk_sample(
       }
     }
     __syncthreads();
-    if (tid < nrem) atomicAdd(&s_seg[s_removed[tid] / SEG], -s_removed_w[tid]);
+    if (tid < nrem) atomicAdd(&s_seg[s_removed[tid] / SEG], -wgt(__bfloat162float(rowp[s_removed[tid]])));
     __syncthreads();
-    const float target = u_bonus[i] * (mz.y - s_remw);
     if (tid < 32) {  // lane = a run of consecutive segments; warp scan of the runs, then the owning lane walks its run
       const int per = (nseg + 31) / 32, l0 = min(nseg, lane * per), l1 = min(nseg, l0 + per);
-      float mine = 0.f;
-      for (int sgm = l0; sgm < l1; ++sgm) mine += s_seg[sgm];
-      float incl = mine;
+      double mine = 0.0;
+      for (int sgm = l0; sgm < l1; ++sgm) mine += (double)fmaxf(s_seg[sgm], 0.f);
+      double incl = mine;
 #pragma unroll
       for (int ofs = 1; ofs < 32; ofs <<= 1) {
-        const float t = __shfl_up_sync(0xffffffffu, incl, ofs);
+        const double t = __shfl_up_sync(0xffffffffu, incl, ofs);
         if (lane >= ofs) incl += t;
       }
-      const float before = incl - mine;
-      const unsigned hit = __ballot_sync(0xffffffffu, mine > 0.f && before + mine > target);
-      const unsigned pos = __ballot_sync(0xffffffffu, mine > 0.f);
+      const double total = __shfl_sync(0xffffffffu, incl, 31);
+      const double target = (double)u_bonus[i] * total;
+      const double before = incl - mine;
+      const unsigned hit = __ballot_sync(0xffffffffu, mine > 0.0 && before + mine > target);
+      const unsigned pos = __ballot_sync(0xffffffffu, mine > 0.0);
       const int owner = hit ? __ffs(hit) - 1 : (pos ? 31 - __clz(pos) : 0);  // past the end by rounding: last mass
       if (lane == owner) {
-        float run = before;
+        double run = before;
         int pick = -1, last_pos = l0;
         for (int sgm = l0; sgm < l1; ++sgm) {
-          const float w = s_seg[sgm];
-          if (w > 0.f) last_pos = sgm;
+          const double w = (double)fmaxf(s_seg[sgm], 0.f);
+          if (w > 0.0) last_pos = sgm;
           if (run + w > target) { pick = sgm; break; }
           run += w;
         }
         s_prefix = pick >= 0 ? run : -INFINITY;
         s_pick_seg = pick >= 0 ? pick : last_pos;
+        s_target = target;
       }
     }
     __syncthreads();
     if (tid < 32) {
       const int base = s_pick_seg * SEG + lane * 8;
+      const double target = s_target;
       float w[8];
       load8(base, w);
 #pragma unroll
       for (int e = 0; e < 8; ++e)
         for (int r = 0; r < nrem; ++r)
           if (s_removed[r] == base + e) w[e] = 0.f;
-      const float mine = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
-      float incl = mine;
+      const double mine = (double)(((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7])));
+      double incl = mine;
 #pragma unroll
       for (int ofs = 1; ofs < 32; ofs <<= 1) {
-        const float t = __shfl_up_sync(0xffffffffu, incl, ofs);
+        const double t = __shfl_up_sync(0xffffffffu, incl, ofs);
         if (lane >= ofs) incl += t;
       }
-      const float before = s_prefix + (incl - mine);
+      const double before = s_prefix + (incl - mine);
       int pick = -1, last_nz = -1;
-      float acc = before;
+      double acc = before;
 #pragma unroll
       for (int e = 0; e < 8; ++e) {
         if (w[e] > 0.f) last_nz = base + e;
-        acc += w[e];
+        acc += (double)w[e];
         if (pick < 0 && w[e] > 0.f && acc > target) pick = base + e;
       }
       const unsigned found = __ballot_sync(0xffffffffu, pick >= 0);
@@ -339,7 +349,8 @@ int launch_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoS
   const size_t need = (size_t)(cap + R) * sizeof(float2);
   if (need > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
   float2* stats = reinterpret_cast<float2*>(ctx->workspace);
-  const float c = 1.4426950408889634f / in->temperature;
+  const double c_exact = 1.4426950408889634 / (double)in->temperature;
+  const float c = (float)c_exact, c_lo = (float)(c_exact - (double)c);  // log2(e) / T in two floats (bonus-draw CDF)
   if (cap + R > 0) {
     ECHO_CUDA_TRY(ctx, launch_pdl(k_softmax_stats, dim3(cap + R), dim3(ST_THREADS), 0, st, sel->n_selected, cap, R,
                                   reinterpret_cast<const __nv_bfloat16*>(in->target_logits),
@@ -349,7 +360,7 @@ int launch_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoS
     const bool have_pools = kv->k_pool && kv->v_pool;
     ECHO_CUDA_TRY(ctx, launch_pdl(k_walk_sample, dim3(R), dim3(WS_THREADS), 0, st, sel->sel_offsets, sel->parent_local,
                                   in->draft_token, reinterpret_cast<const __nv_bfloat16*>(in->target_logits),
-                                  reinterpret_cast<const __nv_bfloat16*>(in->root_logits), in->ld, in->vocab, cap, c,
+                                  reinterpret_cast<const __nv_bfloat16*>(in->root_logits), in->ld, in->vocab, cap, c, c_lo,
                                   stats, in->u_accept, in->u_bonus, kv->page_table, kv->prefix_len,
                                   kv->max_pages_per_req, kv->num_kv_heads, kv->num_pages, kv->num_layers,
                                   have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->k_pool) : (__nv_bfloat16*)nullptr,

@@ -6,7 +6,7 @@ import pytest
 from oracle import echo_oracle as orc
 from paper_2604_09603_b200 import workloads as W
 from helpers import oracle_gate_select, torch_bf16_to_bits, bf16_bits_to_f32
-from gpu_util import dev, get_ctx, run_gate_select, make_kv
+from gpu_util import dev, get_ctx, run_gate_select, make_kv, assert_selection_equal
 
 pytestmark = pytest.mark.gpu
 TOL_O, TOL_LSE = 1e-2, 1e-3
@@ -17,6 +17,7 @@ def _setup(wl, gate=None, poison=False, q_zero=False):
     ctx = get_ctx()
     sel = run_gate_select(ctx, wl, gate)
     want_sel = oracle_gate_select(orc, wl, gate)
+    assert_selection_equal(sel.to_host(), want_sel)   # the attention below runs on the GPU's own selection
     cap = max(1, sel.capacity)
     q, k, v = W.draw_qkv(wl, cap, device="cuda")
     if q_zero:
