@@ -193,7 +193,7 @@ def run_gpu(args, rank, world, local_rank):
     schedule = {"topb": echo.SCHED_TOPB, "alg1": echo.SCHED_ALG1}[args.schedule]
     cap = wl.capacity()
     ctx = echo.EchoContext(local_rank, 0)
-    ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq)
+    ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq, wl.Hkv)
     if args.attn_path:
         ctx.set_option(echo.OPT_ATTN_PATH, args.attn_path)
     if args.splits:

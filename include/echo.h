@@ -17,6 +17,8 @@
  *   - Return value: ECHO_OK (0) or a negative EchoStatus.  Data-dependent precondition
  *     violations cannot be seen by the host; they set bits in the device status word
  *     (echo_device_status) and leave outputs unspecified.  Nothing traps.
+ *   - A context belongs to one device; every call makes that device current for its duration and restores
+ *     the caller's.
  *   - There is no CPU fallback and no dispatch on architecture: echo_create fails with
  *     ECHO_ERR_ARCH unless the device has compute capability 10.0.
  *   - R = number of requests (the paper's batch size B); the paper's budget K_max
@@ -32,7 +34,7 @@
 extern "C" {
 #endif
 
-typedef struct EchoCtx EchoCtx;  /* opaque; owns the workspace */
+typedef struct EchoCtx EchoCtx;  /* opaque; owns the workspace and the TMA tensor maps it has encoded */
 typedef void* echo_stream_t;     /* a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
 
 typedef enum {
@@ -52,11 +54,14 @@ typedef enum {
 #define ECHO_DEV_BAD_TRACE 16u     /* echo_calibrate: depth >= 32 or a confidence outside [0, 1] / NaN (sample skipped) */
 #define ECHO_DEV_TREE_OVERFLOW 64u  /* echo_draft_expand: level * topk nodes do not fit the request's candidate range */
 #define ECHO_DEV_CALIB_OVERFLOW 32u /* echo_calibrate: more than ECHO_CALIB_MAX_PER_DEPTH samples at one depth (rest dropped) */
+#define ECHO_DEV_CAND_OVERFLOW 128u /* a request with more than ECHO_MAX_CAND candidates / packed nodes (the rest is ignored) */
+#define ECHO_DEV_INTERNAL 256u      /* a kernel found its own set-up violated (e.g. misaligned shared memory); outputs unspecified */
 
 /* test / tuning hooks for echo_set_option */
 #define ECHO_OPT_FORCE_SPLITS 1   /* >0: split every KV stream into exactly this many parts (<= 16) */
 #define ECHO_OPT_ATTN_PATH 2      /* 0 = auto, 1 = CUDA-core small-row kernel, 2 = tcgen05 kernel */
 #define ECHO_OPT_NUM_CTAS 3       /* >0: persistent grid size of the tcgen05 kernel (default: #SMs) */
+#define ECHO_OPT_ATTN_SAFE 4      /* 1: the tcgen05 kernel takes every item in its safe form (running row maximum) */
 
 #define ECHO_MAX_CAND 128   /* C_i <= 128 candidates per request (R:G-14) */
 #define ECHO_MAX_DEPTH 32   /* depth < 32 (R:G-14) */
@@ -65,29 +70,26 @@ typedef enum {
 #define ECHO_CALIB_WORKSPACE_BYTES (256 + (size_t)ECHO_MAX_DEPTH * ECHO_CALIB_MAX_PER_DEPTH * 4)
 #define ECHO_MAX_ACCEPT 32  /* an accepted path has <= 32 nodes (one per depth) */
 #define ECHO_CUT_NEVER 0x7fffffff
-#define ECHO_PROF_CTAS 256  /* echo_debug_wait_prof: rows (persistent CTAs) ... */
-#define ECHO_PROF_SLOTS 32  /* ... x counters per CTA */
 
 /* ---- lifetime ------------------------------------------------------------------------ */
 /* Creates a context on `device` with a workspace of `workspace_bytes` (device memory, owned by
  * the context, freed by echo_destroy).  ECHO_ERR_ARCH unless compute capability is 10.0. */
 int echo_create(EchoCtx** out, int device, size_t workspace_bytes);
 int echo_destroy(EchoCtx* ctx);
-/* Workspace needed by any call with at most these sizes: select keys [total_cand], split-KV
- * partials for 16 splits [capacity][num_q_heads] x (128+2) fp32, plan arrays. */
-size_t echo_workspace_bytes(int32_t num_requests, int32_t total_cand, int32_t capacity, int32_t num_q_heads);
+/* Workspace needed by any call with at most these sizes: select keys [total_cand]; split-KV partials
+ * [max_splits][capacity][num_q_heads] x (128+1) fp32 (max_splits = the largest split count echo_verify_attn may
+ * use: 1 when num_requests * num_kv_heads >= #SMs, else up to 8, or the ECHO_OPT_FORCE_SPLITS value; <= 0 means 16,
+ * the upper limit); the work list; (capacity + num_requests) x 8 bytes of echo_accept_stochastic statistics. */
+size_t echo_workspace_bytes(int32_t num_requests, int32_t total_cand, int32_t capacity, int32_t num_q_heads,
+                            int32_t max_splits);
+/* The number of KV splits echo_verify_attn uses for a batch of num_requests requests x num_kv_heads KV heads on this
+ * context (its device's SM count and ECHO_OPT_FORCE_SPLITS): the max_splits to size the workspace with. */
+int echo_attn_splits(EchoCtx* ctx, int32_t num_requests, int32_t num_kv_heads);
 const char* echo_strerror(int code);
 const char* echo_last_error(EchoCtx* ctx);  /* text of the last ECHO_ERR_CUDA on this context */
 /* Copies the device status word to *flags with a blocking 4-byte copy on `stream` and clears it. */
 int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream);
 int echo_set_option(EchoCtx* ctx, int key, int64_t value);
-/* Debug hook (only in a library built with -DECHO_WAIT_PROF; ECHO_ERR_UNSUPPORTED otherwise): copies the
- * per-CTA mbarrier wait-cycle counters of the last tcgen05 verify-attention launch to HOST memory
- * host_out[n_ctas][ECHO_PROF_SLOTS] (uint64) after a device synchronise.  Slots: K producer 0 total,
- * 1 wait K-empty, 2 wait Q-empty; V producer 4 total, 5 wait V-empty; MMA issuer 8 total, 9 K-full,
- * 10 P-full, 11 V-full, 12 O-free, 13 Q-full; softmax warp 16 total, 17 S-full, 18 O-full, 19 PV-done,
- * 20 V-full (ragged tile).  Returns the number of rows written or a negative EchoStatus. */
-int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas);
 
 /* ---- problem statement ----------------------------------- */
 /* Candidate draft trees G_i with parent function pa(j) and draft log-probabilities (Eq. 5). */

@@ -5,6 +5,19 @@
 
 static bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
+// A context belongs to one device: every compute entry point makes it current for the duration of the call, so that a
+// caller whose current device differs (or a second context on another GPU) launches where the context's memory lives.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(const EchoCtx* ctx) {
+    if (ctx && cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) switched = cudaSetDevice(ctx->device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
 extern "C" {
 
 const char* echo_strerror(int code) {
@@ -19,15 +32,23 @@ const char* echo_strerror(int code) {
   }
 }
 
-size_t echo_workspace_bytes(int32_t R, int32_t N, int32_t capacity, int32_t Hq) {
+size_t echo_workspace_bytes(int32_t R, int32_t N, int32_t capacity, int32_t Hq, int32_t max_splits) {
   if (R < 0 || N < 0 || capacity < 0 || Hq < 0) return 0;
-  size_t keys = align_up((size_t)N * sizeof(uint64_t), 256);
-  size_t parts = align_up((size_t)16 * capacity * Hq * (128 + 2) * sizeof(float), 256);
-  size_t toks = align_up((size_t)capacity * sizeof(int32_t), 256);
-  size_t plan = align_up((size_t)R * (Hq > 0 ? Hq : 1) * 16 * 32 + 65536, 256);  // <= R*Hkv*row_tiles*16 splits items of 32 B
-  size_t m = keys > parts ? keys : parts;
-  if (toks > m) m = toks;
-  return m + plan + 4096;  // partials and plan are used together; keys/tokens alias the partials
+  const size_t splits = max_splits <= 0 || max_splits > 16 ? 16 : (size_t)max_splits;
+  const size_t keys = align_up((size_t)N * sizeof(uint64_t), 256) + 256;  // select keys + threshold
+  // split-KV partials exist only when a stream is split; the work list sits behind them: <= R * Hkv * row tiles *
+  // splits records of 32 B, and Hkv * row tiles <= 2 Hq (row tiles = ceil(min(capacity, 128) * G / 128))
+  const size_t parts = splits > 1 ? align_up(splits * capacity * Hq * (128 + 1) * sizeof(float), 256) : 0;
+  const size_t plan = 256 + (size_t)R * 2 * (Hq > 0 ? Hq : 1) * splits * 32;
+  const size_t stats = ((size_t)capacity + R) * 8;  // echo_accept_stochastic: (max, Z) per logits row
+  size_t m = keys > parts + plan ? keys : parts + plan;
+  if (stats > m) m = stats;
+  return align_up(m, 256) + 4096;
+}
+
+int echo_attn_splits(EchoCtx* ctx, int32_t R, int32_t Hkv) {
+  if (!ctx || R < 0 || Hkv <= 0) return ECHO_ERR_INVALID_ARG;
+  return attn_split_policy(ctx, R, Hkv);
 }
 
 int echo_create(EchoCtx** out, int device, size_t workspace_bytes) {
@@ -62,8 +83,10 @@ int echo_create(EchoCtx** out, int device, size_t workspace_bytes) {
 
 int echo_destroy(EchoCtx* ctx) {
   if (!ctx) return ECHO_ERR_INVALID_ARG;
+  DeviceGuard dg(ctx);
   cudaFree(ctx->workspace);
   cudaFree(ctx->dev_status);
+  free_tmap_cache(ctx->tmaps);
   delete ctx;
   return ECHO_OK;
 }
@@ -71,6 +94,7 @@ int echo_destroy(EchoCtx* ctx) {
 const char* echo_last_error(EchoCtx* ctx) { return ctx ? ctx->last_error : "null context"; }
 
 int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !flags) return ECHO_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   ECHO_CUDA_TRY(ctx, cudaMemcpyAsync(flags, ctx->dev_status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
@@ -94,14 +118,12 @@ int echo_set_option(EchoCtx* ctx, int key, int64_t value) {
       if (value < 0 || value > 4096) return ECHO_ERR_INVALID_ARG;
       ctx->opt_num_ctas = value;
       return ECHO_OK;
+    case ECHO_OPT_ATTN_SAFE:
+      if (value < 0 || value > 1) return ECHO_ERR_INVALID_ARG;
+      ctx->opt_attn_safe = value;
+      return ECHO_OK;
     default: return ECHO_ERR_INVALID_ARG;
   }
-}
-
-int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas) {
-  if (!ctx || !host_out || n_ctas <= 0) return ECHO_ERR_INVALID_ARG;
-  ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
-  return debug_wait_prof(reinterpret_cast<unsigned long long*>(host_out), n_ctas);
 }
 
 static int check_gate(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, bool need_packed) {
@@ -125,6 +147,7 @@ static int check_gate(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoS
 }
 
 int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   const int rc = check_gate(ctx, t, g, o, true);
   if (rc != ECHO_OK) return rc;
   return launch_gate_select(ctx, t, g, o, reinterpret_cast<cudaStream_t>(stream));
@@ -132,6 +155,7 @@ int echo_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSe
 
 int echo_gate_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, uint64_t* keys,
                    echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   const int rc = check_gate(ctx, t, g, o, false);
   if (rc != ECHO_OK) return rc;
   if (t->total_cand > 0 && (!keys || misaligned(keys, 8))) return ECHO_ERR_INVALID_ARG;
@@ -140,6 +164,7 @@ int echo_gate_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSele
 
 int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, const uint64_t* local_keys,
                           const uint64_t* all_keys, int64_t n_all, EchoSelection* o, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   const int rc = check_gate(ctx, t, g, o, true);
   if (rc != ECHO_OK) return rc;
   if (n_all < 0 || (n_all > 0 && !all_keys) || (t->total_cand > 0 && !local_keys)) return ECHO_ERR_INVALID_ARG;
@@ -160,6 +185,7 @@ static int check_kv(const EchoPagedKV* kv, bool need_pools) {
 
 int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer, int32_t Hq,
                      int32_t R, const void* q, void* out, float* lse, float sm_scale, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !sel) return ECHO_ERR_INVALID_ARG;
   int rc = check_kv(kv, true);
   if (rc != ECHO_OK) return rc;
@@ -173,6 +199,7 @@ int echo_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* 
 
 int echo_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoSampleInputs* in, int32_t R, EchoPagedKV* kv,
                            EchoAccept* out, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !sel || !in || !out) return ECHO_ERR_INVALID_ARG;
   int rc = check_kv(kv, false);
   if (rc != ECHO_OK) return rc;
@@ -190,6 +217,7 @@ int echo_accept_stochastic(EchoCtx* ctx, const EchoSelection* sel, const EchoSam
 
 int echo_draft_expand(EchoCtx* ctx, const EchoDraftLevel* l, EchoTrees* t, int32_t* token, float* score_out,
                       echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !l || !t) return ECHO_ERR_INVALID_ARG;
   if (t->num_requests < 0 || l->level < 0 || l->topk < 1) return ECHO_ERR_INVALID_ARG;
   if (l->level >= ECHO_MAX_DEPTH || l->topk > ECHO_MAX_TOPK) return ECHO_ERR_UNSUPPORTED;
@@ -200,6 +228,7 @@ int echo_draft_expand(EchoCtx* ctx, const EchoDraftLevel* l, EchoTrees* t, int32
 }
 
 int echo_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibration* o, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !t || !o) return ECHO_ERR_INVALID_ARG;
   if (t->num_samples < 0 || !(delta == delta)) return ECHO_ERR_INVALID_ARG;
   if (t->num_samples > 0 && (!t->depth || !t->conf || !t->accepted)) return ECHO_ERR_INVALID_ARG;
@@ -210,6 +239,7 @@ int echo_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibrat
 
 int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t R, EchoPagedKV* kv,
                 EchoAccept* out, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
   if (!ctx || !sel || !res || !out) return ECHO_ERR_INVALID_ARG;
   int rc = check_kv(kv, false);
   if (rc != ECHO_OK) return rc;

@@ -9,6 +9,9 @@
 
 #include "../../include/echo.h"
 
+struct TmapCache;  // TMA tensor maps this context has encoded (verify_attn_tc.cu)
+void free_tmap_cache(TmapCache*);
+
 struct EchoCtx {
   int device;
   int num_sms;
@@ -18,8 +21,20 @@ struct EchoCtx {
   int64_t opt_force_splits;
   int64_t opt_attn_path;
   int64_t opt_num_ctas;
+  int64_t opt_attn_safe;
+  TmapCache* tmaps;
+  bool attn_attr_set, calib_attr_set;  // cudaFuncSetAttribute is per device, i.e. per context
   char last_error[256];
 };
+
+// split policy of echo_verify_attn (verify_attn.cu): the host knows only capacities (P_i, K_i are device-side)
+static inline int attn_split_policy(const EchoCtx* ctx, long R, long Hkv) {
+  int splits = 1;
+  if (ctx->opt_force_splits > 0) splits = (int)ctx->opt_force_splits;
+  else
+    while (splits < 8 && R * Hkv * splits < (long)ctx->num_sms) splits *= 2;
+  return splits > 16 ? 16 : splits;
+}
 
 #define ECHO_CUDA_TRY(ctx, expr)                                                              \
   do {                                                                                        \
@@ -69,7 +84,6 @@ int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32
 int launch_accept(EchoCtx*, const EchoSelection*, const EchoVerifyResult*, int32_t R, EchoPagedKV*, EchoAccept*,
                   cudaStream_t);
 // tcgen05 path (verify_attn_tc.cu); returns ECHO_ERR_UNSUPPORTED when the shape cannot use it
-int debug_wait_prof(unsigned long long* host_out, int n_ctas);
 int launch_verify_attn_tc(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
                           const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,
                           float* part_ml, cudaStream_t);

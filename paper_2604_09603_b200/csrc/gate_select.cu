@@ -57,9 +57,14 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
   pdl_launch_dependents();
   const int i = blockIdx.x;
   const int b = cand_offsets[i];
-  const int C = min(cand_offsets[i + 1] - b, ECHO_MAX_CAND);
+  const int C_all = cand_offsets[i + 1] - b;
+  const int C = min(C_all, ECHO_MAX_CAND);
   const int j = threadIdx.x;
   uint32_t bad = 0;
+  if (C_all > ECHO_MAX_CAND) {  // more candidates than a request may have (R:G-14): flag, and make the excess
+    bad |= ECHO_DEV_CAND_OVERFLOW;  // ineligible so that k_select never reads an unwritten key
+    for (int t = ECHO_MAX_CAND + j; t < C_all; t += ECHO_MAX_CAND) keys[b + t] = KEY_INELIGIBLE;
+  }
   if (j < ECHO_MAX_DEPTH) s_lvlmax[j] = 0u;
   if (j < C) {
     int p = parent[b + j];

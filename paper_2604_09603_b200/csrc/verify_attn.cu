@@ -165,13 +165,7 @@ int launch_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV
   // are fewer (request, KV head) streams than SMs, and then just enough to give every SM one: every split level
   // costs per-item set-up, the fp32 partials and the merge launch, and the planner already balances whole items.
   // Measured: cfg1 (256 streams) one split 0.068 ms, two 0.107 ms; cfg3 (512 streams) one 0.256 ms, two 0.312 ms.
-  int splits = 1;
-  if (ctx->opt_force_splits > 0) splits = (int)ctx->opt_force_splits;
-  else {
-    const long units = (long)R * Hkv;
-    while (splits < 8 && units * splits < (long)ctx->num_sms) splits *= 2;
-  }
-  if (splits > 16) splits = 16;
+  const int splits = attn_split_policy(ctx, R, Hkv);
   const size_t n_rows = (size_t)cap * Hq;
   // workspace layout: [keys: unused here][part_o: splits*n_rows*128 f32][part_lse: splits*n_rows f32]
   float* part_o = reinterpret_cast<float*>(ctx->workspace);

@@ -8,11 +8,15 @@
 //   warp 13     = issuer of S = Q K^T (SS, K-major x K-major) into one of three S buffers in TMEM
 //   warp 15     = issuer of O += P V (TS: P read from TMEM where the softmax wrote it over S, V as the MN-major B
 //                 operand straight from its TMA layout); accumulators never leave TMEM
-//   warps 0-7   = softmax, two warpgroups, thread = half a row (64 columns): weights against a running reference
-//                 without a row maximum first, two-pass fallback on a vote of the two warps of a row quarter; tree
-//                 mask only in tiles that touch positions >= P_i; a quarter of the prefix-tile weights take 2^x on
-//                 the FMA pipe; P written back to TMEM as bf16 over the first 32 columns of the thread's S half
-//   warps 8-11  = epilogue: O / l -> bf16 out + lse (or the fp32 split partial) while the softmax is on the next item
+//   warps 0-7   = softmax, two warpgroups that take ALTERNATE KV tiles (thread = one whole row of 128 columns): while
+//                 one warpgroup waits for its S tile, loads it from TMEM or hands P back, the other one computes, so
+//                 the two warps of an SM sub-partition are never stalled together.  Weights are taken against the
+//                 fixed reference 0 (fp32 and bf16 share the exponent range, so no running maximum is needed while
+//                 the row sums stay inside [2^-90, 2^100]); tree mask only in tiles that touch positions >= P_i; part
+//                 of the prefix-tile weights take 2^x on the FMA pipe; P written back to TMEM as bf16 over S.
+//   warps 8-11  = epilogue: O / l -> bf16 out + lse (or the fp32 split partial) while the softmax is on the next item;
+//                 it also checks the row sums: an item with a sum outside the window is flagged and redone at the end
+//                 by the same CTA in the SAFE form (running row maximum, O rescaled in TMEM; warpgroup 0 alone).
 //   setmaxnreg  : softmax 160, epilogue 80, single-lane warps 40 registers
 // Each KV page is read once per (KV head, row tile) and serves all rows of the tile.
 // Operator definition: include/echo.h (paper: P:39, P:85 names it only; readings R:A-1..A-8).
@@ -35,17 +39,23 @@ constexpr int GROUP_BYTES = 2048;         // 8 tokens x 128 d: d-half 0 (1 KB SW
 constexpr int SMEM_Q = 0;
 constexpr int SMEM_K = SMEM_Q + TILE_BYTES;
 constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
-constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;  // float stats[2][128]: 1 / l_rounded, lse of the item just finished
-constexpr int SMEM_XCHG = SMEM_STATS + 2 * TILE_M * 4;  // float xchg[2 warpgroups][128]: half-row maxima / sums
-constexpr int SMEM_BAR = SMEM_XCHG + 2 * TILE_M * 4;
-constexpr int SMEM_TOTAL = SMEM_BAR + 256;  // dynamic smem is declared 1024-byte aligned: no slack
-// warpgroups 0 and 1 (warps 0-3, 4-7) softmax: warpgroup w takes columns [64 w, 64 w + 64) of every S row, so each
-// SM sub-partition has two softmax warps to issue from; warpgroup 2 (warps 8-11) epilogue; warpgroup 3: warp 12 Q+K
-// producer, 13 QK^T MMA issuer, 14 V producer, 15 PV MMA issuer; warpgroup 4: warps 16 / 17 second K / V producer,
-// 18-19 idle (they pad the warpgroup so that setmaxnreg applies)
-constexpr int NTHREADS = 640;
-constexpr int W_EPI = 8, W_PROD_K0 = 12, W_MMA_QK = 13, W_PROD_V0 = 14, W_MMA_PV = 15, W_PROD_K1 = 16, W_PROD_V1 = 17;
-constexpr int REGS_SOFTMAX = 160, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 160 + 80 + 2 * 40) = 640 * 96, the launch allocation
+// float stats[5][128] of the item just finished: warpgroup 0's weight sum (exact), normaliser, reference; warpgroup
+// 1's weight sum and normaliser (single-buffered: the epilogue hands it back through B_STATFREE as soon as it is read)
+constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;
+constexpr int ST_L0 = 0, ST_N0 = 1, ST_M0 = 2, ST_L1 = 3, ST_N1 = 4;
+constexpr int SMEM_BAR = SMEM_STATS + 5 * TILE_M * 4;
+constexpr int BAR_BYTES = 256;                      // up to 32 mbarriers
+constexpr int SMEM_TMEM_SLOT = SMEM_BAR + BAR_BYTES;  // 16 bytes
+constexpr int SMEM_REDO = SMEM_TMEM_SLOT + 16;        // bitmap over this CTA's items: redo in the safe form
+constexpr int REDO_WORDS = 60;
+constexpr int REDO_CAP = REDO_WORDS * 32;  // items of a CTA beyond this take the safe form at once
+constexpr int SMEM_TOTAL = SMEM_REDO + REDO_WORDS * 4;  // = 227 KB exactly; dynamic smem is declared 1024-byte aligned
+static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
+// warpgroups 0 and 1 (warps 0-3, 4-7) softmax; warpgroup 2 (warps 8-11) epilogue; warpgroup 3: warp 12 K producer,
+// 13 QK^T MMA issuer, 14 V + Q producer, 15 PV MMA issuer
+constexpr int NTHREADS = 512;
+constexpr int W_EPI = 8, W_PROD_K = 12, W_MMA_QK = 13, W_PROD_V = 14, W_MMA_PV = 15;
+constexpr int REGS_SOFTMAX = 192, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 192 + 80 + 40) <= 512 * 128, the launch allocation
 constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
 constexpr int TMEM_O = NSBUF * TILE_N;
 constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
@@ -53,21 +63,27 @@ constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,51
 #ifndef ECHO_POLY_COUNT
 #define ECHO_POLY_COUNT 1
 #endif
-constexpr int POLY_PERIOD = 4, POLY_COUNT = ECHO_POLY_COUNT;  // measured best: 1 of 4 (2 of 4 and 3 of 8 are slower)
+#ifndef ECHO_POLY_PERIOD
+#define ECHO_POLY_PERIOD 4
+#endif
+constexpr int POLY_PERIOD = ECHO_POLY_PERIOD, POLY_COUNT = ECHO_POLY_COUNT;
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
-constexpr float WEIGHT_SUM_LIMIT = 4294967296.f;  // a tile whose weight sum exceeds 2^32 is redone against its own maximum
-// Every item starts from the reference 0 instead of the first tile's row maxima: weights are floating point, so any
-// reference within 2^-64 .. 2^32 of the true one gives the same O and lse; a first tile whose weight sum falls outside
-// that range is redone in the two-pass form, which takes the reference from the data.
-constexpr float WEIGHT_SUM_FLOOR = 5.421010862427522e-20f;  // 2^-64
+// The fast form takes every weight as 2^(s * scale * log2e) with no reference subtracted.  fp32 sums and bf16 weights
+// both carry 8 exponent bits, so the result is the same as with a running maximum as long as nothing overflows and
+// what underflows is negligible: an item whose row sum ends inside [2^-90, 2^100] has every weight <= 2^100 and has
+// lost at most 2^-126 per key to flush-to-zero (< 2^-21 of the sum over 32 768 keys).  Anything else -- inf, NaN
+// included -- sends the item to the safe form.
+constexpr float SUM_LO = 8.0779356694631609e-28f;  // 2^-90
+constexpr float SUM_HI = 1.2676506002282294e30f;   // 2^100
 
 constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
 enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
-       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_SFREE = 24, B_COUNT = 27 };
+       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_SFREE = 24, B_STATFREE = 27, B_PHASE = 28, B_COUNT = 29 };
+static_assert(B_COUNT * 8 <= BAR_BYTES, "barrier region");
 
 struct AttnParams {
   const int4* items;
@@ -82,6 +98,7 @@ struct AttnParams {
   float* lse;
   float scale_log2;
   int splits;
+  int force_safe;  // test hook: every item takes the safe form
   float* part_o;
   float* part_lse;
   size_t n_rows_cap;
@@ -89,9 +106,11 @@ struct AttnParams {
 };
 
 // Optional wait-time profile (build with -DECHO_WAIT_PROF): cycles each role spends blocked on each mbarrier,
-// per CTA, read back with echo_debug_wait_prof.  Compiled out otherwise.
+// per CTA, read back with echo_debug_wait_prof (csrc/debug_prof.h).  Compiled out otherwise.
 #ifdef ECHO_WAIT_PROF
+#include "debug_prof.h"
 __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
+__device__ long long g_trace[256][8];
 #define PROF_T0() const long long prof_t0_ = clock64()
 #define PROF_ADD(slot) prof_[slot] += clock64() - prof_t0_
 #define PROF_WAIT(slot, b, ph) do { const long long t_ = clock64(); tc::mbar_wait(b, ph); prof_[slot] += clock64() - t_; } while (0)
@@ -101,6 +120,10 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_FLUSH(base, n) do { if (blockIdx.x < ECHO_PROF_CTAS) for (int q_ = 0; q_ < n; ++q_) g_wait_prof[blockIdx.x][(base) + q_] = prof_[q_]; } while (0)
 #define PROF_SPAN_BEGIN() const long long span_t_ = clock64()
 #define PROF_SPAN_END(slot) prof_[slot] += clock64() - span_t_
+#define PROF_COUNT(slot) prof_[slot] += 1
+#define TRACE(gg, ev) do { if (blockIdx.x == 0 && (gg) < 256 && lane == 0) g_trace[gg][ev] = clock64(); } while (0)
+#define PROF_SPAN2_BEGIN() const long long span2_t_ = clock64()
+#define PROF_SPAN2_END(slot) prof_[slot] += clock64() - span2_t_
 #else
 #define PROF_T0() do {} while (0)
 #define PROF_ADD(slot) do {} while (0)
@@ -111,6 +134,10 @@ __device__ unsigned long long g_wait_prof[ECHO_PROF_CTAS][ECHO_PROF_SLOTS];
 #define PROF_FLUSH(base, n) do {} while (0)
 #define PROF_SPAN_BEGIN() do {} while (0)
 #define PROF_SPAN_END(slot) do {} while (0)
+#define PROF_COUNT(slot) do {} while (0)
+#define PROF_SPAN2_BEGIN() do {} while (0)
+#define PROF_SPAN2_END(slot) do {} while (0)
+#define TRACE(gg, ev) do {} while (0)
 #endif
 
 // work item record written by k_plan: two int4 = {req, kvh | rt<<8 | split<<16, jt0, jt1} {P_i, sel_offsets[i], K_i, 0}
@@ -125,6 +152,24 @@ __device__ __forceinline__ Item load_item(const int4* items, int idx) { return d
 // snake order over the length-sorted work list: round k of CTA c takes k*G+c (k even) or (k+1)*G-1-c (k odd)
 __device__ __forceinline__ int item_index(int k, int cta, int grid) {
   return (k & 1) ? (k + 1) * grid - 1 - cta : k * grid + cta;
+}
+
+// Every role walks the same sequence of items: first the CTA's share of the work list (phase 0; the items past
+// REDO_CAP in the safe form), then -- once the epilogue has seen the last row sums (B_PHASE) -- the items it flagged,
+// in the safe form.  fn(item index, safe).
+template <typename Fn>
+__device__ __forceinline__ void redo_phase(int cta, int grid, int n_items, const volatile uint32_t* redo, uint32_t bar_phase,
+                                           Fn&& fn) {
+  tc::mbar_wait_relaxed(bar_phase, 0);
+  uint32_t any = 0;
+#pragma unroll 4
+  for (int w = 0; w < REDO_WORDS; ++w) any |= redo[w];
+  if (!any) return;
+  for (int k = 0; k < REDO_CAP; ++k) {
+    const int idx = item_index(k, cta, grid);
+    if (idx >= n_items) break;
+    if ((redo[k >> 5] >> (k & 31)) & 1u) fn(idx, true);
+  }
 }
 
 __device__ __forceinline__ uint32_t mask_word(const uint4& m, int w) {
@@ -143,8 +188,6 @@ __device__ __forceinline__ uint32_t visible_word(const uint4& m, int P, int t0) 
   return bits;
 }
 
-// ---- softmax passes over this thread's half of an S row (64 fp32 columns in TMEM), two 32-column tcgen05.ld, the
-// second in flight while the first is processed ----
 __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
 #pragma unroll
   for (int e = 0; e < 32; ++e)
@@ -154,8 +197,8 @@ __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
 // 2^x for a pair of finite x on the FMA pipe instead of MUFU (16 ex2 per clock per SM, the busiest pipe of the
 // softmax): n = round(x) by the 1.5*2^23 trick, f = x - n in [-0.5, 0.5], 2^f by a degree-3 minimax polynomial
 // (relative error 7.5e-5, far below the bf16 rounding of P), then n is added to the exponent field.  x is clamped
-// to [-125, 126]: 2^-125 instead of less is negligible against the reference weight 1 (so this form is used only
-// where no key is masked), and 2^126 sends the tile to the two-pass fallback.
+// to [-125, 126]: 2^-125 instead of less is far below the window's lower end (so this form is used only where no
+// key is masked), and 2^126 puts the row sum above the window: the item is redone in the safe form.
 __device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
   float x0, x1;
   tc::unpack_f32x2(x2, x0, x1);
@@ -174,45 +217,60 @@ __device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
   p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
 }
 
-// weights p = 2^(s*scale_log2 + neg_m) for 64 columns: packed to bf16 in pk, exact fp32 sum in ts and (tail tiles
-// only) the sum of the bf16-rounded weights in tr.  Packed f32x2 FMA / ADD halve the issue slots.
-// TAIL = false (all 64 keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP / FADD2 with no
-// visibility selects and no rounded sum: 2.5 issue slots per weight.
+// weights p = 2^(s*scale_log2 + neg_m) of one 32-column chunk of a row: packed to bf16 in pk, added to the exact
+// fp32 partial sums in acc and (TAIL only) to the sums of the bf16-rounded weights in trr.  Packed f32x2 FMA / ADD
+// halve the issue slots.  TAIL = false (all keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP /
+// FADD2 with no visibility selects and no rounded sum: 2.5 issue slots per weight.
 template <bool TAIL>
-__device__ __forceinline__ void weights_pass(uint32_t tSh, const uint32_t (&vis)[2], float scale_log2, float neg_m,
-                                             uint32_t (&pk)[32], float& ts, float& tr) {
+__device__ __forceinline__ void weights_chunk(uint32_t (&sc)[32], uint32_t vis, uint64_t sc2, uint64_t nm2,
+                                              uint32_t (&pk)[16], uint64_t (&acc)[4], float (&trr)[2]) {
+  if (TAIL) mask_chunk(sc, vis);
+#pragma unroll
+  for (int e = 0; e < 32; e += 2) {
+    const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
+    float p0, p1;
+#ifdef ECHO_EXP_NOEXP
+    tc::unpack_f32x2(x2, p0, p1);
+#else
+    if (!TAIL && ((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
+      ex2_poly_x2(x2, p0, p1);
+    } else {
+      float x0, x1;
+      tc::unpack_f32x2(x2, x0, x1);
+      p0 = tc::ex2(x0);
+      p1 = tc::ex2(x1);
+    }
+#endif
+    const uint32_t w = tc::pack_bf16(p0, p1);
+    pk[e >> 1] = w;
+#ifndef ECHO_EXP_NOSUM
+    acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
+#endif
+    // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
+    // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
+    // combination of V rows; lse always uses the exact fp32 sum
+    if (TAIL) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
+  }
+}
+
+// One S row (128 fp32 columns in TMEM at tS) -> bf16 P over its first 64 columns, four 32-column chunks, the load of
+// chunk c+1 in flight while chunk c is processed.  ts = exact sum of the weights, tr = the normaliser's share.
+template <bool TAIL>
+__device__ __forceinline__ void tile_weights(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
+                                             float& ts, float& tr) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
   float trr[2] = {0.f, 0.f};
   uint32_t s[2][32];
-  tc::tmem_ld32(tSh, s[0]);
-  tc::tmem_wait_ld();
-  tc::tmem_ld32(tSh + 32, s[1]);
+  tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    if (c == 1) tc::tmem_wait_ld();
-    uint32_t(&sc)[32] = s[c];
-    if (TAIL) mask_chunk(sc, vis[c]);
-#pragma unroll
-    for (int e = 0; e < 32; e += 2) {
-      const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
-      float p0, p1;
-      if (!TAIL && ((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
-        ex2_poly_x2(x2, p0, p1);
-      } else {
-        float x0, x1;
-        tc::unpack_f32x2(x2, x0, x1);
-        p0 = tc::ex2(x0);
-        p1 = tc::ex2(x1);
-      }
-      const uint32_t w = tc::pack_bf16(p0, p1);
-      pk[c * 16 + (e >> 1)] = w;
-      acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
-      // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
-      // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
-      // combination of V rows; lse always uses the exact fp32 sum
-      if (TAIL) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
-    }
+  for (int c = 0; c < 4; ++c) {
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s[c & 1]);
+    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
+    uint32_t pk[16];
+    weights_chunk<TAIL>(s[c & 1], vis[c], sc2, nm2, pk, acc, trr);
+    tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunks already read (c/2 <= c)
   }
   float a0, a1;
   tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
@@ -220,36 +278,21 @@ __device__ __forceinline__ void weights_pass(uint32_t tSh, const uint32_t (&vis)
   tr = TAIL ? trr[0] + trr[1] : ts;
 }
 
-__device__ __forceinline__ float row_max_pass(uint32_t tSh, const uint32_t (&vis)[2]) {
+__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   uint32_t s[2][32];
-  tc::tmem_ld32(tSh, s[0]);
-  tc::tmem_ld32(tSh + 32, s[1]);
-  tc::tmem_wait_ld();
+  tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    mask_chunk(s[c], vis[c]);
+  for (int c = 0; c < 4; ++c) {
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s[c & 1]);
+    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
+    mask_chunk(s[c & 1], vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2)
-      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c][e]), __uint_as_float(s[c][e + 1]));
+      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c & 1][e]), __uint_as_float(s[c & 1][e + 1]));
   }
   return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
-}
-
-// named barrier over the two warps that share a TMEM lane quarter (one per softmax warpgroup), ids 1-4
-__device__ __forceinline__ bool pair_or(int quarter, bool pred) {
-  uint32_t r;
-  asm volatile(
-      "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\t"
-      "barrier.cta.red.or.pred q, %2, 64, p;\n\t"
-      "selp.u32 %0, 1, 0, q;\n\t}"
-      : "=r"(r)
-      : "r"((uint32_t)pred), "r"(quarter + 1)
-      : "memory");
-  return r != 0;
-}
-__device__ __forceinline__ void pair_sync(int quarter) {
-  asm volatile("barrier.cta.sync %0, 64;" ::"r"(quarter + 1) : "memory");
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_constant__ CUtensorMap tmap_q,
@@ -260,9 +303,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   const uint32_t sbase = tc::smem_u32(smem_raw);
   const uint32_t sQ = sbase + SMEM_Q, sK = sbase + SMEM_K, sV = sbase + SMEM_V, sBar = sbase + SMEM_BAR;
   uint8_t* gen_base = smem_raw;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_BAR + B_COUNT * 8);
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_TMEM_SLOT);
+  volatile uint32_t* redo = reinterpret_cast<volatile uint32_t*>(gen_base + SMEM_REDO);
   float* stats = reinterpret_cast<float*>(gen_base + SMEM_STATS);
-  float* xchg = reinterpret_cast<float*>(gen_base + SMEM_XCHG);
   auto bar = [&](int i) -> uint32_t { return sBar + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -270,11 +313,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   pdl_launch_dependents();  // echo_accept's kernel may queue behind this one (it waits for our completion itself)
 
   if (threadIdx.x == 0) {
-    if (sbase & 1023u) __trap();  // SW128 operand tiles need 1024-byte alignment
+    if (sbase & 1023u) atomicOr(p.status, ECHO_DEV_INTERNAL);  // SW128 operand tiles need 1024-byte alignment
     for (int i = 0; i < B_COUNT; ++i) {
-      const uint32_t cnt = (i >= B_KFULL && i < B_KFULL + NSTAGE) || (i >= B_VFULL && i < B_VFULL + NSTAGE) ? 2u
-                           : (i >= B_PFULL && i < B_PFULL + NSBUF) ? 8u  /* one arrival per softmax warp */
-                           : (i == B_OFREE || i == B_STATS) ? 128u : 1u;
+      const uint32_t cnt = (i >= B_PFULL && i < B_PFULL + NSBUF) ? 4u  /* one arrival per warp of the owning warpgroup */
+                           : (i == B_OFREE || i == B_STATFREE || i == B_PHASE) ? 128u
+                           : (i == B_STATS) ? 256u : 1u;
       tc::mbar_init(bar(i), cnt);
     }
     tc::fence_barrier_init();
@@ -282,7 +325,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     tc::prefetch_tmap(&tmap_k);
     tc::prefetch_tmap(&tmap_v);
   }
-  if (warp == W_MMA_QK) tc::tmem_alloc(sBar + B_COUNT * 8, TMEM_COLS);
+  if (threadIdx.x < REDO_WORDS) redo[threadIdx.x] = 0u;
+  if (warp == W_MMA_QK) tc::tmem_alloc(sbase + SMEM_TMEM_SLOT, TMEM_COLS);
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
@@ -291,25 +335,96 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   // k_plan; the work list is read only after k_plan has completed.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   const int n_items = *p.n_items;
+  const bool force_safe = p.force_safe != 0;
 
   if (warp >= 12) tc::setmaxnreg_dec<REGS_AUX>();
-  if (warp == W_PROD_K0 || warp == W_PROD_V0 || warp == W_PROD_K1 || warp == W_PROD_V1) {
-    // ============================== TMA producers: Q + K ring, V ring ==============================
-    // One cp.async.bulk.tensor costs its issuing thread 110-170 cycles whatever the box size (measured), so a page
-    // (16 tokens x 128 d of one KV head, 4 KB contiguous in the pool) is one 4-D box {64 d, 8 tokens, 2 d-halves,
-    // 2 token groups} and each ring has two issuing threads in different warps: thread h takes pages 4h..4h+3 of
-    // every 128-token tile.  The whole loop runs in one lane so that every TMA operand is warp-uniform; page ids of
-    // tile j+1 are fetched while tile j is being issued.
-    if (lane == 0) {
-      const bool is_k = warp == W_PROD_K0 || warp == W_PROD_K1;
-      const int half = (warp == W_PROD_K1 || warp == W_PROD_V1) ? 1 : 0;
-      const bool loads_q = warp == W_PROD_K0;
+  if (warp == W_PROD_K || warp == W_PROD_V) {
+    // ============================== TMA producers: K ring, V ring + Q ==============================
+    // A page (16 tokens x 128 d of one KV head, 4 KB contiguous in the pool) is one 4-D box {64 d, 8 tokens, 2 d-halves,
+    // 2 token groups}; a 128-token tile is eight of them, their ids read from the page table by lanes 0-7 one tile
+    // ahead.  All 32 lanes walk the loop (same addresses, same values: every TMA operand is provably warp-uniform),
+    // one elected lane issues.  The Q tile belongs to the V warp, so that the K tiles of the next item are requested
+    // without waiting for the last QK^T of this one to release Q.
+    {
+      const bool is_k = warp == W_PROD_K;
+      const bool loads_q = !is_k;
       const uint32_t s_dst = is_k ? sK : sV;
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
       int g = 0, itc = 0;
       PROF_DECL(3);
       PROF_T0();
+      // The next item's Q tile (V warp) and its rows' ancestor masks (K warp) are pulled into L2 one item ahead: the
+      // masks are read by the softmax threads at the item boundary, where a DRAM miss under a saturated memory
+      // system cost them ~3000 cycles per dependent load (wait profile, round 2).
+      auto prefetch_next = [&](const Item& nx) {
+        const int node0 = tc::uniform(nx.off) + tc::uniform(nx.rt) * (TILE_M >> p.log2G);
+        if (loads_q) {
+          const int h0 = tc::uniform(nx.kvh) * p.G;
+          if (tc::elect_one()) {
+            tc::tma_prefetch_3d(&tmap_q, 0, h0, node0);
+            tc::tma_prefetch_3d(&tmap_q, 64, h0, node0);
+          }
+          __syncwarp();
+        } else {
+          const int bytes = min(TILE_M >> p.log2G, max(0, nx.Ki - nx.rt * (TILE_M >> p.log2G))) * 16;
+          if (lane * 128 < bytes) tc::prefetch_l2(reinterpret_cast<const uint8_t*>(p.anc_mask + node0) + lane * 128);
+        }
+      };
+      auto produce = [&](const Item& t, const Item* next) {
+        Item it;
+        it.req = tc::uniform(t.req); it.kvh = tc::uniform(t.kvh); it.rt = tc::uniform(t.rt);
+        it.jt0 = tc::uniform(t.jt0); it.jt1 = tc::uniform(t.jt1); it.P = tc::uniform(t.P); it.off = tc::uniform(t.off);
+        it.Ki = tc::uniform(t.Ki);
+        const int total = it.P + it.Ki;
+        if (loads_q) {
+          PROF_WAIT_BACKOFF(2, bar(B_QEMPTY), (itc & 1) ^ 1);
+          const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
+          if (tc::elect_one()) {
+            tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
+            tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
+            tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
+          }
+          __syncwarp();
+          TRACE(g, 6);
+        }
+        const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
+        int npages = (total + PAGE - 1) / PAGE;
+        if (npages > p.max_pages) {  // page table too short: flag, load what exists
+          if (is_k && lane == 0) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
+          npages = p.max_pages;
+        }
+        auto tile_page = [&](int j) -> int {  // lane e < 8: id of page e of tile j
+          const int pi = j * 8 + (lane & 7);
+          return pi < npages ? pt[pi] : 0;
+        };
+        int cur = tile_page(it.jt0);
+        for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+          const int nxt = j + 1 < it.jt1 ? tile_page(j + 1) : 0;
+          const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
+          const int npv = max(0, min(8, npages - j * 8));  // pages of this tile that hold tokens
+          const uint32_t dst = s_dst + slot * TILE_BYTES;
+          const uint32_t fb = bar(b_full + slot);
+          int pg[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) pg[e] = __shfl_sync(0xffffffffu, cur, e);
+          PROF_WAIT_BACKOFF(1, bar(b_empty + slot), ph ^ 1);
+          if (tc::elect_one()) {
+            tc::mbar_expect_tx(fb, npv * PAGE_BYTES);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+              if (e < npv) {
+                const int grp = ((p.page_row_base + pg[e]) * p.Hkv + it.kvh) * (PAGE / 8);  // 8-token group index
+                tc::tma_load_4d(dst + e * PAGE_BYTES, tmap, fb, 0, 0, 0, grp);
+              }
+            }
+          }
+          __syncwarp();
+          cur = nxt;
+          if (j == it.jt0 && next) prefetch_next(*next);  // its record was requested before this item began
+        }
+        ++itc;
+      };
       Item nx = {};
       bool more = item_index(0, cta, grid) < n_items;  // item indices grow with k
       if (more) nx = load_item(p.items, item_index(0, cta, grid));
@@ -317,70 +432,29 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const Item it = nx;
         more = item_index(k, cta, grid) < n_items;
         if (more) nx = load_item(p.items, item_index(k, cta, grid));
-        const int total = it.P + it.Ki;
-        if (loads_q) {
-          PROF_WAIT_BACKOFF(2, bar(B_QEMPTY), (itc & 1) ^ 1);
-          tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
-          const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
-          tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
-          tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
-        }
-        const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
-        int npages = (total + PAGE - 1) / PAGE;
-        if (npages > p.max_pages) {  // page table too short: flag, load what exists
-          if (loads_q) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
-          npages = p.max_pages;
-        }
-        int cur[4], nxt[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int pi = it.jt0 * 8 + half * 4 + e;
-          cur[e] = pi < npages ? pt[pi] : 0;
-        }
-        for (int j = it.jt0; j < it.jt1; ++j, ++g) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int pi = (j + 1) * 8 + half * 4 + e;
-            nxt[e] = (j + 1 < it.jt1 && pi < npages) ? pt[pi] : 0;
-          }
-          const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
-          const int npv = max(0, min(4, npages - j * 8 - half * 4));  // my pages of this tile that hold tokens
-          const uint32_t dst = s_dst + slot * TILE_BYTES + half * 4 * PAGE_BYTES;
-          const uint32_t fb = bar(b_full + slot);
-          PROF_WAIT_BACKOFF(1, bar(b_empty + slot), ph ^ 1);
-          tc::mbar_expect_tx(fb, npv * PAGE_BYTES);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            if (e < npv) {
-              const int grp = ((p.page_row_base + cur[e]) * p.Hkv + it.kvh) * (PAGE / 8);  // 8-token group index
-              tc::tma_load_4d(dst + e * PAGE_BYTES, tmap, fb, 0, 0, 0, grp);
-            }
-          }
-#pragma unroll
-          for (int e = 0; e < 4; ++e) cur[e] = nxt[e];
-        }
-        ++itc;
+        produce(it, more ? &nx : nullptr);
       }
+      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) { produce(load_item(p.items, idx), nullptr); });
       PROF_ADD(0);
-      if (half == 0) PROF_FLUSH(is_k ? 0 : 4, 3);
+      if (lane == 0) PROF_FLUSH(is_k ? 0 : 4, 3);
     }
-    __syncwarp();
   } else if (warp == W_MMA_QK) {
     // ============================== MMA issuer for S = Q K^T (one lane) ==============================
     // Two issuing threads, one per product: a single thread retires a 128x128x16 tcgen05.mma only every ~110
     // cycles, two threads keep the tensor pipe at 70-85 cycles per instruction (measured).  This thread runs up to
     // NSBUF tiles ahead of the PV issuer; S/P buffer b is handed back through B_SFREE when the PV that read P_b is done.
-    if (lane == 0) {
+    // All 32 lanes walk the loop (every operand warp-uniform), one elected lane issues.
+    {
       int g = 0, itc = 0;
       PROF_DECL(6);
       PROF_T0();
+      const uint32_t tmem_u = (uint32_t)tc::uniform((int)tmem);
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
-      for (int k = 0;; ++k) {
-        const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) break;  // item indices grow with k
+      auto issue = [&](int idx, bool) {
         const int4 rec = p.items[2 * idx];
-        const int n = rec.w - rec.z;
-        PROF_WAIT(5, bar(B_QFULL), itc & 1);
+        const int n = tc::uniform(rec.w - rec.z);
+        PROF_WAIT(3, bar(B_QFULL), itc & 1);
+        TRACE(g, 7);
         for (int j = 0; j < n; ++j, ++g) {
           const int slot = g % NSTAGE, b = g % NSBUF;
           PROF_WAIT(1, bar(B_KFULL + slot), (g / NSTAGE) & 1);
@@ -388,32 +462,42 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           tc::tc_fence_after();
           // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half h at +1 KB inside a group
           const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, GROUP_BYTES);
+          TRACE(g, 0);
+          if (tc::elect_one()) {
 #pragma unroll
-          for (int kk = 0; kk < D / 16; ++kk) {
-            const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
-            const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
-            tc::mma_ss(tmem + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
+            for (int kk = 0; kk < D / 16; ++kk) {
+              const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
+              const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
+              tc::mma_ss(tmem_u + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
+            }
+            tc::mma_commit(bar(B_SFULL + b));
+            tc::mma_commit(bar(B_KEMPTY + slot));
+            if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
           }
-          tc::mma_commit(bar(B_SFULL + b));
-          tc::mma_commit(bar(B_KEMPTY + slot));
-          if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
+          __syncwarp();
+          TRACE(g, 1);
         }
         ++itc;
+      };
+      for (int k = 0;; ++k) {
+        const int idx = item_index(k, cta, grid);
+        if (idx >= n_items) break;  // item indices grow with k
+        issue(idx, false);
       }
+      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), issue);
       PROF_ADD(0);
-      PROF_FLUSH(8, 6);
+      if (lane == 0) PROF_FLUSH(8, 4);
     }
     __syncwarp();
   } else if (warp == W_MMA_PV) {
     // ============================== MMA issuer for O += P V (one lane) ==============================
-    if (lane == 0) {
+    {
       int g = 0, itc = 0;
-      const uint32_t tO = tmem + TMEM_O;
-      for (int k = 0;; ++k) {
-        const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) break;
+      const uint32_t tmem_u = (uint32_t)tc::uniform((int)tmem);
+      const uint32_t tO = tmem_u + TMEM_O;
+      auto issue = [&](int idx, bool) {
         const int4 rec = p.items[2 * idx];
-        const int n = rec.w - rec.z;
+        const int n = tc::uniform(rec.w - rec.z);
         for (int j = 0; j < n; ++j, ++g) {
           const int b = g % NSBUF, slot = g % NSTAGE;
           tc::mbar_wait(bar(B_PFULL + b), (g / NSBUF) & 1);
@@ -421,93 +505,85 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
           tc::tc_fence_after();
           // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO).
-          // P of tokens [0,64) sits in columns [0,32) of S_b, P of tokens [64,128) in columns [64,96): each softmax
-          // warpgroup overwrites only columns of its own half of S.
+          // P (bf16 pairs) sits in columns [0,64) of S_b: 16 tokens = 8 columns per MMA.
           const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, 1024, GROUP_BYTES);
+          TRACE(g, 4);
+          if (tc::elect_one()) {
 #pragma unroll
-          for (int kk = 0; kk < TILE_N / 16; ++kk)
-            tc::mma_ts(tO, tmem + b * TILE_N + (kk >> 2) * 64 + (kk & 3) * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV,
-                       (j > 0) || (kk > 0));
-          tc::mma_commit(bar(B_VEMPTY + slot));
-          tc::mma_commit(bar(B_SFREE + b));
-          tc::mma_commit(bar(B_PVDONE));
-          if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+            for (int kk = 0; kk < TILE_N / 16; ++kk)
+              tc::mma_ts(tO, tmem_u + b * TILE_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV, (j > 0) || (kk > 0));
+            tc::mma_commit(bar(B_VEMPTY + slot));
+            tc::mma_commit(bar(B_SFREE + b));
+            tc::mma_commit(bar(B_PVDONE));
+            if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+          }
+          __syncwarp();
+          TRACE(g, 5);
         }
         ++itc;
+      };
+      for (int k = 0;; ++k) {
+        const int idx = item_index(k, cta, grid);
+        if (idx >= n_items) break;
+        issue(idx, false);
       }
+      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), issue);
     }
     __syncwarp();
   } else if (warp < W_EPI) {
-    // ============================== softmax (warpgroups 0 and 1, thread = half of a row) ==============================
-    // Both halves of a row keep the same running reference m_used (it changes only in the pair-synchronised
-    // two-pass branch) and their own partial weight sums, added up once per item.
+    // ============================== softmax (warpgroups 0 and 1, thread = row) ==============================
+    // KV tile g (counted over the CTA's whole run) belongs to warpgroup g & 1; in the safe form every tile belongs
+    // to warpgroup 0, which then keeps the running row maximum.  Each warpgroup adds up the weights of its own tiles
+    // and publishes them once per item; the epilogue adds the two.
     tc::setmaxnreg_inc<REGS_SOFTMAX>();
-    const int wg = warp >> 2;  // which 64 columns of every S row
+    int wg = warp >> 2;
+    asm volatile("" : "+r"(wg));  // keep it in a register: recomputing it from %tid (S2R) in every loop costs ~5 %
     const int wq = warp & 3;   // TMEM lane quarter this warp may access
     const int row = wq * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
-    float* xchg_mine = xchg + wg * TILE_M + row;
-    const float* xchg_other = xchg + (wg ^ 1) * TILE_M + row;
     int g = 0, itc = 0;
     PROF_DECL(7);
     PROF_T0();
-    // Item records are fetched two items ahead and the row's ancestor mask one item ahead, so that no global-load
-    // latency sits between the last tile of one item and the first tile of the next.
+#ifdef ECHO_WAIT_PROF
+    long long gap_t_ = clock64();
+#endif
     auto row_mask = [&](const int4& r0, const int4& r1) -> uint4 {
       const int l = ((((r0.y >> 8) & 0xff) * TILE_M + row) >> p.log2G);
       return l < r1.z ? p.anc_mask[r1.y + l] : make_uint4(0u, 0u, 0u, 0u);
     };
-    const int4 zero4 = make_int4(0, 0, 0, 0);
-    int4 a0 = zero4, a1 = zero4, b0 = zero4, b1 = zero4;  // records of the next item (a) and the one after (b)
-    uint4 mk_next = make_uint4(0u, 0u, 0u, 0u);
-    bool more = item_index(0, cta, grid) < n_items;
-    if (more) { a0 = p.items[2 * item_index(0, cta, grid)]; a1 = p.items[2 * item_index(0, cta, grid) + 1]; }
-    if (item_index(1, cta, grid) < n_items) { b0 = p.items[2 * item_index(1, cta, grid)]; b1 = p.items[2 * item_index(1, cta, grid) + 1]; }
-    if (more) mk_next = row_mask(a0, a1);
-    for (int k = 0; more; ++k) {
-      const Item it = decode(a0, a1);
-      const uint4 mk = mk_next;
-      more = item_index(k + 1, cta, grid) < n_items;
-      a0 = b0; a1 = b1;
-      if (item_index(k + 2, cta, grid) < n_items) { b0 = p.items[2 * item_index(k + 2, cta, grid)]; b1 = p.items[2 * item_index(k + 2, cta, grid) + 1]; }
-      if (more) mk_next = row_mask(a0, a1);
+    auto do_item = [&](const Item& it, const uint4& mk, const bool safe) {
       const int P = it.P, total = it.P + it.Ki;
-      float m_used = 0.f, lsum = 0.f, lsum_r = 0.f;
-      const uint32_t tOh = tmem + TMEM_O + wg * 64 + lane_addr;
-
-      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+      float m_used = safe ? -INFINITY : 0.f, lsum = 0.f, lnorm = 0.f;
+      const uint32_t tO = tmem + TMEM_O + lane_addr;
+      // my tiles of this item: every second one, or all / none in the safe form
+      const int first = safe ? (wg ? it.jt1 - it.jt0 : 0) : ((g ^ wg) & 1), step = safe ? 1 : 2;
+      const int g_end = g + (it.jt1 - it.jt0);
+      g += first;
+      for (int j = it.jt0 + first; j < it.jt1; j += step, g += step) {
         const int b = g % NSBUF;
-        const uint32_t tSh = tmem + b * TILE_N + wg * 64 + lane_addr;  // my 64 columns of S; P goes to their first 32
+        const uint32_t tS = tmem + b * TILE_N + lane_addr;
+#ifdef ECHO_WAIT_PROF
+        if (j == it.jt0 + first) prof_[4] += clock64() - gap_t_; else prof_[2] += clock64() - gap_t_;
+#endif
         PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
+        PROF_SPAN_BEGIN();
+        if (wq == 0) TRACE(g, 2);
         tc::tc_fence_after();
-        const int tile0 = j * TILE_N, tok0 = tile0 + wg * 64;
-        const bool tail = tok0 + 64 > P;  // my keys touch tree positions or the ragged end: apply visibility
-        uint32_t vis[2] = {0xffffffffu, 0xffffffffu};
+        const int tile0 = j * TILE_N;
+        const bool tail = tile0 + TILE_N > P;  // the tile touches tree positions or the ragged end: apply visibility
+        uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
         if (tail) {
-          vis[0] = visible_word(mk, P, tok0);
-          vis[1] = visible_word(mk, P, tok0 + 32);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tile0 + 32 * c);
         }
-        uint32_t pk[32];  // my half of the bf16 P row
-        float ts = 0.f, tr = 0.f;  // this tile's exact / bf16-rounded weight sums
-        // Fast path: the weights are taken against the running reference m_used without looking at this tile's
-        // maximum first; only if a weight sum leaves [0, 2^32] (reference too low, or no reference yet) do the
-        // two warps of the row quarter fall back to the two-pass form (row maximum, rescale, weights).  P is
-        // stored only after that check, so S is still intact for the second pass.
-        bool slow = __any_sync(0xffffffffu, m_used == -INFINITY);  // the same in both halves
-        if (!slow) {
-          PROF_SPAN_BEGIN();
-          if (tail) weights_pass<true>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
-          else weights_pass<false>(tSh, vis, p.scale_log2, -m_used, pk, ts, tr);
-          slow = pair_or(wq, !(ts <= WEIGHT_SUM_LIMIT) || (j == it.jt0 && ts < WEIGHT_SUM_FLOOR));
-          PROF_SPAN_END(5);
-        }
-        if (slow) {
-          if (j == it.jt0) m_used = -INFINITY;  // nothing accumulated yet: drop the guessed reference
-          float mx = row_max_pass(tSh, vis);
-          *xchg_mine = mx;
-          pair_sync(wq);
-          mx = fmaxf(mx, *xchg_other);
-          pair_sync(wq);  // both halves have read before the slots are written again
+        float ts = 0.f, tr = 0.f;  // this tile's exact weight sum / share of the normaliser
+        if (!safe) {
+          if (tail) tile_weights<true>(tS, vis, p.scale_log2, 0.f, ts, tr);
+          else tile_weights<false>(tS, vis, p.scale_log2, 0.f, ts, tr);
+        } else {
+          // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same path:
+          // the TMEM instructions are warp-wide)
+          const float mx = row_max_pass(tS, vis);
           const float m_new = fmaxf(m_used, mx * p.scale_log2);
           float alpha = 1.f;
           if (m_new > m_used) {
@@ -515,73 +591,93 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             m_used = m_new;
           }
           lsum *= alpha;
-          lsum_r *= alpha;
-          if (j > it.jt0) {  // O holds PV of earlier tiles: wait for the last one, rescale my 64 columns in TMEM
+          lnorm *= alpha;
+          if (j > it.jt0 && __any_sync(0xffffffffu, alpha != 1.f)) {  // O holds PV of earlier tiles
             PROF_WAIT(3, bar(B_PVDONE), (g - 1) & 1);
             tc::tc_fence_after();
 #pragma unroll
-            for (int c = 0; c < 2; ++c) {
+            for (int c = 0; c < 4; ++c) {
               uint32_t o[32];
-              tc::tmem_ld32(tOh + c * 32, o);
+              tc::tmem_ld32(tO + c * 32, o);
               tc::tmem_wait_ld();
+              tc::reg_fence32(o);
 #pragma unroll
               for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-              tc::tmem_st32(tOh + c * 32, o);
+              tc::tmem_st32(tO + c * 32, o);
             }
             tc::tmem_wait_st();
           }
           const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-          weights_pass<true>(tSh, vis, p.scale_log2, -m_eff, pk, ts, tr);  // vis is all ones off the tail
+          tile_weights<true>(tS, vis, p.scale_log2, -m_eff, ts, tr);  // vis is all ones off the tail
         }
         lsum += ts;
-        lsum_r += tr;
-        PROF_SPAN_BEGIN();
-        tc::tmem_st32(tSh, pk);
+        lnorm += tr;
         tc::tmem_wait_st();
         if (tile0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
           const int slot = g % NSTAGE;
           PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
-          if (row >= total - tile0) {  // warpgroup w clears d-half w of V row `row`
-            uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (row >> 3) * GROUP_BYTES + wg * 1024 +
-                                               (row & 7) * 128);
+          if (row >= total - tile0) {  // both d-halves of V row `row`
 #pragma unroll
-            for (int e = 0; e < 8; ++e) z[e] = make_uint4(0u, 0u, 0u, 0u);
+            for (int h = 0; h < 2; ++h) {
+              uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (row >> 3) * GROUP_BYTES + h * 1024 +
+                                                 (row & 7) * 128);
+#pragma unroll
+              for (int e = 0; e < 8; ++e) z[e] = make_uint4(0u, 0u, 0u, 0u);
+            }
           }
           tc::fence_proxy_async();
         }
         tc::tc_fence_before();
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
-        PROF_SPAN_END(6);
+        if (wq == 0) TRACE(g, 3);
+        PROF_SPAN_END(5);
+        PROF_COUNT(6);
+#ifdef ECHO_WAIT_PROF
+        gap_t_ = clock64();
+#endif
       }
-
-      // ---- add the two halves' sums; warpgroup 0 hands 1 / l_rounded and lse = ln2 * (m + log2 l) to the epilogue ----
-      if (wg == 1) {
-        xchg_mine[0] = lsum;
-        // the rounded sum travels in warpgroup 0's slot, which warpgroup 0 itself does not write here
-        const_cast<float*>(xchg_other)[0] = lsum_r;
-      }
-      pair_sync(wq);
-      if (wg == 0) {
-        lsum += *xchg_other;
-        lsum_r += *xchg_mine;
-        const float inv = lsum_r > 0.f ? 1.f / lsum_r : 0.f;
-        const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-        const float lse_v = lsum > 0.f ? (m_eff + log2f(lsum)) * LN2 : -INFINITY;
-        tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of item itc-1 has read its statistics
-        stats[row] = inv;
-        stats[TILE_M + row] = lse_v;
-        tc::mbar_arrive(bar(B_STATS));
-      }
-      pair_sync(wq);  // the exchange slots are free again
+      g = g_end;
+      // ---- publish this warpgroup's sums (and warpgroup 0's reference) for the epilogue ----
+      PROF_SPAN2_BEGIN();
+      PROF_WAIT(2, bar(B_STATFREE), (itc & 1) ^ 1);  // the epilogue has read the statistics of the previous item
+      stats[(wg ? ST_L1 : ST_L0) * TILE_M + row] = lsum;
+      stats[(wg ? ST_N1 : ST_N0) * TILE_M + row] = lnorm;
+      if (wg == 0) stats[ST_M0 * TILE_M + row] = (m_used == -INFINITY) ? 0.f : m_used;
+      tc::mbar_arrive(bar(B_STATS));
+      PROF_SPAN2_END(3);
       ++itc;
+    };
+    // Phase 0: item records are fetched two items ahead and the row's ancestor mask one item ahead, so that no
+    // global-load latency sits between the last tile of one item and the first tile of the next.
+    {
+      const int4 zero4 = make_int4(0, 0, 0, 0);
+      int4 a0 = zero4, a1 = zero4, b0 = zero4, b1 = zero4;  // records of the next item (a) and the one after (b)
+      uint4 mk_next = make_uint4(0u, 0u, 0u, 0u);
+      bool more = item_index(0, cta, grid) < n_items;
+      if (more) { a0 = p.items[2 * item_index(0, cta, grid)]; a1 = p.items[2 * item_index(0, cta, grid) + 1]; }
+      if (item_index(1, cta, grid) < n_items) { b0 = p.items[2 * item_index(1, cta, grid)]; b1 = p.items[2 * item_index(1, cta, grid) + 1]; }
+      if (more) mk_next = row_mask(a0, a1);
+      for (int k = 0; more; ++k) {
+        const Item it = decode(a0, a1);
+        const uint4 mk = mk_next;
+        more = item_index(k + 1, cta, grid) < n_items;
+        a0 = b0; a1 = b1;
+        if (item_index(k + 2, cta, grid) < n_items) { b0 = p.items[2 * item_index(k + 2, cta, grid)]; b1 = p.items[2 * item_index(k + 2, cta, grid) + 1]; }
+        if (more) mk_next = row_mask(a0, a1);
+        do_item(it, mk, force_safe || k >= REDO_CAP);
+      }
     }
+    redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) {
+      const int4 r0 = p.items[2 * idx], r1 = p.items[2 * idx + 1];
+      do_item(decode(r0, r1), row_mask(r0, r1), true);
+    });
     PROF_ADD(0);
-    if (warp == 0 && lane == 0) PROF_FLUSH(16, 7);
-  } else if (warp < W_PROD_K0) {
+    if ((warp & 3) == 0 && lane == 0) PROF_FLUSH(16 + 8 * wg, 7);
+  } else if (warp < W_PROD_K) {
     // ============================== epilogue (warpgroup 2, thread = row) ==============================
-    // O of item n is normalised and stored here while the softmax warpgroup is already on item n+1 (O and the
-    // statistics are double buffered by item parity).
+    // O of item n is normalised and stored here while the softmax warpgroups are already on item n+1.  The row sums
+    // of the fast form are checked here: outside the window -> the item's bit in the redo bitmap.
     tc::setmaxnreg_dec<REGS_EPILOGUE>();
     const int wq = warp & 3;
     const int row = wq * 32 + lane;
@@ -589,19 +685,28 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     int itc = 0;
     PROF_DECL(3);
     PROF_T0();
-    for (int k = 0;; ++k) {
-      const int idx = item_index(k, cta, grid);
-      if (idx >= n_items) break;
+    auto finish = [&](int idx, int k, bool safe) {
       const Item it = load_item(p.items, idx);
       const int r_glob = it.rt * TILE_M + row;
       const int l = r_glob >> p.log2G, gq = r_glob & (p.G - 1);
       const bool valid = l < it.Ki;
-      const int opar = itc & 1;
       const uint32_t tO = tmem + TMEM_O + lane_addr;
       const size_t rowg = (size_t)(it.off + l) * p.Hq + it.kvh * p.G + gq;
       PROF_WAIT_RELAXED(1, bar(B_STATS), itc & 1);
-      const float inv = stats[row];
-      const float lse_v = stats[TILE_M + row];
+      const float lsum = stats[ST_L0 * TILE_M + row] + stats[ST_L1 * TILE_M + row];
+      const float lnorm = stats[ST_N0 * TILE_M + row] + stats[ST_N1 * TILE_M + row];
+      const float m_ref = stats[ST_M0 * TILE_M + row];
+      tc::mbar_arrive(bar(B_STATFREE));
+      if (!safe) {
+#ifdef ECHO_EXP_NOCHECK
+        const bool bad = false;
+#else
+        const bool bad = valid && !(lsum >= SUM_LO && lsum <= SUM_HI);
+#endif
+        if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(const_cast<uint32_t*>(redo) + (k >> 5), 1u << (k & 31));
+      }
+      const float inv = lnorm > 0.f ? 1.f / lnorm : 0.f;
+      const float lse_v = lsum > 0.f ? (m_ref + log2f(lsum)) * LN2 : -INFINITY;
       PROF_WAIT(2, bar(B_OFULL), itc & 1);
       tc::tc_fence_after();
       uint32_t o[2][32];
@@ -609,6 +714,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         tc::tmem_wait_ld();
+        tc::reg_fence32(o[c & 1]);
         if (c < 3) tc::tmem_ld32(tO + (c + 1) * 32, o[(c + 1) & 1]);
         uint32_t(&oc)[32] = o[c & 1];
         if (valid) {
@@ -639,9 +745,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       tc::tc_fence_before();
       tc::mbar_arrive(bar(B_OFREE));
       ++itc;
+    };
+    for (int k = 0;; ++k) {
+      const int idx = item_index(k, cta, grid);
+      if (idx >= n_items) break;
+      finish(idx, k, force_safe || k >= REDO_CAP);
     }
+    tc::mbar_arrive(bar(B_PHASE));  // the bitmap is final (release); every role, this one included, now reads it
+    redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) { finish(idx, 0, true); });
     PROF_ADD(0);
-    if (warp == W_EPI && lane == 0) PROF_FLUSH(24, 3);
+    if (warp == W_EPI && lane == 0) PROF_FLUSH(12, 3);
   }
 
   // ---- teardown ----
@@ -656,8 +769,8 @@ constexpr int PLAN_THREADS = 256;   // one request per thread and pass at the ba
 constexpr int PLAN_BUCKETS = 1024;  // tile counts above 1023 (131 k tokens) share the last bucket
 __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict__ sel_offsets,
                                                        const int32_t* __restrict__ prefix_len, int R, int Hkv, int G,
-                                                       int splits, int max_items, int4* __restrict__ items,
-                                                       int32_t* __restrict__ n_items) {
+                                                       int splits, int max_items, int max_rt, int4* __restrict__ items,
+                                                       int32_t* __restrict__ n_items, uint32_t* __restrict__ status) {
   __shared__ int s_cnt[PLAN_BUCKETS];
   __shared__ int s_warp[32];
   pdl_launch_dependents();  // let k_verify_attn_tc set itself up meanwhile
@@ -668,10 +781,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
   __syncthreads();
   auto for_items = [&](auto&& fn) {
     for (int r = tid; r < R; r += PLAN_THREADS) {
-      const int off = sel_offsets[r], Ki = sel_offsets[r + 1] - off, P = prefix_len[r];
+      const int off = sel_offsets[r], P = prefix_len[r];
+      int Ki = sel_offsets[r + 1] - off;
       if (Ki <= 0) continue;
+      if (Ki > ECHO_MAX_CAND) {  // more packed nodes than a request can have: clamp and flag (never silently truncate)
+        atomicOr(status, ECHO_DEV_CAND_OVERFLOW);
+        Ki = ECHO_MAX_CAND;
+      }
       const int n_tiles = (P + Ki + TILE_N - 1) / TILE_N;
-      const int n_rt = (Ki * G + TILE_M - 1) / TILE_M;
+      const int n_rt = min((Ki * G + TILE_M - 1) / TILE_M, max_rt);
       const int tps = (n_tiles + splits - 1) / splits;
       for (int s = 0; s * tps < n_tiles; ++s) {
         const int j0 = s * tps, j1 = min(n_tiles, j0 + tps);
@@ -731,16 +849,85 @@ EncodeTiledFn get_encode() {
 
 }  // namespace
 
-int debug_wait_prof(unsigned long long* host_out, int n_ctas) {
-#ifdef ECHO_WAIT_PROF
-  if (n_ctas > ECHO_PROF_CTAS) n_ctas = ECHO_PROF_CTAS;
-  return cudaMemcpyFromSymbol(host_out, g_wait_prof, sizeof(unsigned long long) * ECHO_PROF_SLOTS * n_ctas) == cudaSuccess
-             ? n_ctas : ECHO_ERR_CUDA;
-#else
-  (void)host_out; (void)n_ctas;
-  return ECHO_ERR_UNSUPPORTED;
-#endif
+// Tensor maps are a pure function of (base pointer, shape): the context keeps the few it has encoded (the Q buffers of
+// a double-buffered serving loop, the K and V pools) instead of calling the driver three times per launch.
+struct TmapCache {
+  struct Entry {
+    const void* base;
+    uint64_t a, b, c;  // shape key
+    CUtensorMap map;
+  };
+  static constexpr int N = 16;
+  Entry e[N];
+  int used = 0, next = 0;
+};
+
+void free_tmap_cache(TmapCache* c) { delete c; }
+
+static const CUtensorMap* cached_tmap(EchoCtx* ctx, const void* base, uint64_t a, uint64_t b, uint64_t c,
+                                      int (*encode)(EchoCtx*, CUtensorMap*, const void*, uint64_t, uint64_t, uint64_t)) {
+  if (!ctx->tmaps) ctx->tmaps = new TmapCache();
+  TmapCache* tc_ = ctx->tmaps;
+  for (int i = 0; i < tc_->used; ++i)
+    if (tc_->e[i].base == base && tc_->e[i].a == a && tc_->e[i].b == b && tc_->e[i].c == c) return &tc_->e[i].map;
+  TmapCache::Entry& ent = tc_->e[tc_->next];
+  if (encode(ctx, &ent.map, base, a, b, c) != ECHO_OK) {
+    ent.base = nullptr;
+    return nullptr;
+  }
+  ent.base = base; ent.a = a; ent.b = b; ent.c = c;
+  tc_->next = (tc_->next + 1) % TmapCache::N;
+  if (tc_->used < TmapCache::N) ++tc_->used;
+  return &ent.map;
 }
+
+// Q / out [cap][Hq][128] bf16 as a 3-D map, box = {64 d, G heads, 128/G nodes}
+static int encode_q(EchoCtx* ctx, CUtensorMap* m, const void* q, uint64_t cap, uint64_t Hq, uint64_t G) {
+  EncodeTiledFn enc = get_encode();
+  cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)cap};
+  cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
+  cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)(TILE_M / G)};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(Q) failed: %d", (int)r);
+    return ECHO_ERR_CUDA;
+  }
+  return ECHO_OK;
+}
+// pool rows [token][128 d] seen as [8-token group][d-half][token in group][64 d]: one box = one page
+static int encode_pool(EchoCtx* ctx, CUtensorMap* m, const void* pool, uint64_t total_rows, uint64_t, uint64_t) {
+  EncodeTiledFn enc = get_encode();
+  cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)(total_rows / 8)};
+  cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)D * 2 * 8};
+  cuuint32_t box[4] = {64, 8, 2, (cuuint32_t)(PAGE / 8)};
+  cuuint32_t es[4] = {1, 1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(pool), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(KV) failed: %d", (int)r);
+    return ECHO_ERR_CUDA;
+  }
+  return ECHO_OK;
+}
+
+#ifdef ECHO_WAIT_PROF
+extern "C" int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas) {
+  if (ctx && host_out && n_ctas == -1) {  // event trace of CTA 0: [256 tiles][8 events] clock64
+    ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
+    ECHO_CUDA_TRY(ctx, cudaMemcpyFromSymbol(host_out, g_trace, sizeof(long long) * 256 * 8));
+    return 256;
+  }
+  if (!ctx || !host_out || n_ctas <= 0) return ECHO_ERR_INVALID_ARG;
+  if (n_ctas > ECHO_PROF_CTAS) n_ctas = ECHO_PROF_CTAS;
+  ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
+  ECHO_CUDA_TRY(ctx, cudaMemcpyFromSymbol(host_out, g_wait_prof, sizeof(unsigned long long) * ECHO_PROF_SLOTS * n_ctas));
+  return n_ctas;
+}
+#endif
 
 int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV* kv, int32_t layer, int32_t Hq,
                           int32_t R, const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,
@@ -749,41 +936,16 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   int log2G = 0;
   while ((1 << log2G) < G) ++log2G;
   if ((1 << log2G) != G || G > 128 || !(sm_scale > 0.f)) return ECHO_ERR_UNSUPPORTED;
-  EncodeTiledFn enc = get_encode();
-  if (!enc) {
+  if (!get_encode()) {
     snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled entry point not found");
     return ECHO_ERR_CUDA;
   }
   const size_t total_rows = (size_t)kv->num_layers * kv->num_pages * Hkv * PAGE;
   if (total_rows >= (1ull << 31)) return ECHO_ERR_UNSUPPORTED;
-  CUtensorMap tq, tk, tv;
-  {
-    cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)cap};
-    cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
-    cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)(TILE_M / G)};
-    cuuint32_t es[3] = {1, 1, 1};
-    CUresult r = enc(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, es,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-      snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(Q) failed: %d", (int)r);
-      return ECHO_ERR_CUDA;
-    }
-  }
-  for (int which = 0; which < 2; ++which) {
-    // pool rows [token][128 d] seen as [8-token group][d-half][token in group][64 d]: one box = one page
-    cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)(total_rows / 8)};
-    cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)D * 2 * 8};
-    cuuint32_t box[4] = {64, 8, 2, (cuuint32_t)(PAGE / 8)};
-    cuuint32_t es[4] = {1, 1, 1, 1};
-    CUresult r = enc(which ? &tv : &tk, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, which ? kv->v_pool : kv->k_pool, dims,
-                     strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-      snprintf(ctx->last_error, sizeof(ctx->last_error), "cuTensorMapEncodeTiled(KV) failed: %d", (int)r);
-      return ECHO_ERR_CUDA;
-    }
-  }
+  const CUtensorMap* tq = cached_tmap(ctx, q, (uint64_t)cap, (uint64_t)Hq, (uint64_t)G, encode_q);
+  const CUtensorMap* tk = cached_tmap(ctx, kv->k_pool, total_rows, 0, 0, encode_pool);
+  const CUtensorMap* tv = cached_tmap(ctx, kv->v_pool, total_rows, 0, 0, encode_pool);
+  if (!tq || !tk || !tv) return ECHO_ERR_CUDA;
   // plan region sits behind the split partials in the workspace
   const size_t n_rows = (size_t)cap * Hq;
   const size_t part_bytes = splits > 1 ? align_up((size_t)splits * n_rows * (D + 1) * sizeof(float), 256) : 0;
@@ -795,12 +957,11 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   int32_t* n_items = reinterpret_cast<int32_t*>(plan);
   int4* items = reinterpret_cast<int4*>(plan + 256);
   ECHO_CUDA_TRY(ctx, launch_pdl(k_plan, dim3(1), dim3(PLAN_THREADS), 0, st, sel->sel_offsets, kv->prefix_len, R, Hkv, G,
-                                splits, (int)max_items, items, n_items));
+                                splits, (int)max_items, max_rt, items, n_items, ctx->dev_status));
 
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!ctx->attn_attr_set) {  // per context, i.e. per device (the attribute is a per-device property of the function)
     ECHO_CUDA_TRY(ctx, cudaFuncSetAttribute(k_verify_attn_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL));
-    attr_set = true;
+    ctx->attn_attr_set = true;
   }
   AttnParams p;
   p.items = items; p.n_items = n_items; p.sel_offsets = sel->sel_offsets;
@@ -808,6 +969,7 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   p.page_table = kv->page_table; p.prefix_len = kv->prefix_len; p.max_pages = kv->max_pages_per_req;
   p.Hkv = Hkv; p.Hq = Hq; p.G = G; p.log2G = log2G; p.page_row_base = layer * kv->num_pages;
   p.out = reinterpret_cast<__nv_bfloat16*>(out); p.lse = lse; p.scale_log2 = sm_scale * LOG2E; p.splits = splits;
+  p.force_safe = ctx->opt_attn_safe ? 1 : 0;
   p.part_o = part_o; p.part_lse = part_lse; p.n_rows_cap = n_rows; p.status = ctx->dev_status;
   int grid = ctx->opt_num_ctas > 0 ? (int)ctx->opt_num_ctas : ctx->num_sms;
   if ((size_t)grid > max_items) grid = (int)(max_items ? max_items : 1);
@@ -822,7 +984,7 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, tq, tk, tv, p));
+    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, *tq, *tk, *tv, p));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

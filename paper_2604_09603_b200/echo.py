@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libecho.so")
 
 ECHO_OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5
-OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS = 1, 2, 3
+OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS, OPT_ATTN_SAFE = 1, 2, 3, 4
 SCHED_TOPB, SCHED_ALG1 = 0, 1  # EchoGate.schedule: global top-B (north_star) / Algorithm 1 as printed
 ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
 MAX_ACCEPT = 32
@@ -26,7 +26,7 @@ CUT_NEVER = 0x7FFFFFFF
 DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
-           "echo_device_status", "echo_set_option", "echo_debug_wait_prof", "echo_gate_select", "echo_verify_attn", "echo_accept",
+           "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_gate_select", "echo_verify_attn", "echo_accept",
            "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand",
            "echo_accept_stochastic"]
 
@@ -110,7 +110,9 @@ def load_library():
     lib.echo_create.restype = C.c_int
     lib.echo_destroy.argtypes = [C.c_void_p]
     lib.echo_destroy.restype = C.c_int
-    lib.echo_workspace_bytes.argtypes = [C.c_int32] * 4
+    lib.echo_workspace_bytes.argtypes = [C.c_int32] * 5
+    lib.echo_attn_splits.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+    lib.echo_attn_splits.restype = C.c_int
     lib.echo_workspace_bytes.restype = C.c_size_t
     lib.echo_strerror.argtypes = [C.c_int]
     lib.echo_strerror.restype = C.c_char_p
@@ -120,8 +122,9 @@ def load_library():
     lib.echo_device_status.restype = C.c_int
     lib.echo_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
     lib.echo_set_option.restype = C.c_int
-    lib.echo_debug_wait_prof.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
-    lib.echo_debug_wait_prof.restype = C.c_int
+    if hasattr(lib, "echo_debug_wait_prof"):  # private hook of a library built with ECHO_WAIT_PROF=1 (csrc/debug_prof.h)
+        lib.echo_debug_wait_prof.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        lib.echo_debug_wait_prof.restype = C.c_int
     lib.echo_gate_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p, C.c_void_p]
     lib.echo_gate_keys.restype = C.c_int
     lib.echo_gate_select_keys.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), C.c_void_p, C.c_void_p, C.c_int64,
@@ -259,8 +262,9 @@ class EchoContext:
         import torch
         return C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
 
-    def ensure_workspace(self, R: int, N: int, capacity: int, Hq: int):
-        need = int(self.lib.echo_workspace_bytes(R, N, capacity, Hq))
+    def ensure_workspace(self, R: int, N: int, capacity: int, Hq: int, Hkv: int = 0):
+        splits = int(self.lib.echo_attn_splits(self._h, R, Hkv)) if Hq > 0 and Hkv > 0 else 1
+        need = int(self.lib.echo_workspace_bytes(R, N, capacity, Hq, splits))
         if need > self.workspace_bytes:
             import torch
             torch.cuda.synchronize(self.device)
@@ -284,6 +288,8 @@ class EchoContext:
     def debug_wait_prof(self, n_ctas: int = 148):
         """[n_ctas][32] uint64 wait-cycle counters of the last tcgen05 launch (library built with ECHO_WAIT_PROF=1)."""
         import numpy as np
+        if not hasattr(self.lib, "echo_debug_wait_prof"):
+            raise RuntimeError("libecho.so was built without ECHO_WAIT_PROF=1")
         buf = np.zeros((n_ctas, 32), np.uint64)
         rc = self.lib.echo_debug_wait_prof(self._h, buf.ctypes.data, n_ctas)
         if rc < 0:
@@ -373,7 +379,7 @@ class EchoContext:
         """echo_verify_attn.  q bf16 [capacity][Hq][128] -> (out bf16 same shape, lse f32 [capacity][Hq])."""
         import torch
         Hq = q.shape[1]
-        self.ensure_workspace(sel.R, 0, sel.capacity, Hq)
+        self.ensure_workspace(sel.R, 0, sel.capacity, Hq, kv.k_pool.shape[2])
         if out is None:
             out = torch.zeros_like(q)
         if lse is None:

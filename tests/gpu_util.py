@@ -20,6 +20,7 @@ def get_ctx():
     ctx.set_option(echo.OPT_FORCE_SPLITS, 0)
     ctx.set_option(echo.OPT_ATTN_PATH, 0)
     ctx.set_option(echo.OPT_NUM_CTAS, 0)
+    ctx.set_option(echo.OPT_ATTN_SAFE, 0)
     return ctx
 
 

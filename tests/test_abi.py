@@ -37,8 +37,14 @@ def test_binding_lists_same_symbols():
 def test_strerror_and_workspace(lib):
     assert lib.echo_strerror(0) == b"ok"
     assert b"workspace" in lib.echo_strerror(-3)
-    assert lib.echo_workspace_bytes(128, 10240, 2048, 64) >= 16 * 2048 * 64 * 130 * 4
-    assert lib.echo_workspace_bytes(-1, 0, 0, 0) == 0
+    lib.echo_workspace_bytes.restype = C.c_size_t
+    assert lib.echo_workspace_bytes(128, 10240, 2048, 64, 0) >= 16 * 2048 * 64 * 129 * 4   # max_splits <= 0: the limit, 16
+    assert lib.echo_workspace_bytes(128, 10240, 2048, 64, 2) >= 2 * 2048 * 64 * 129 * 4
+    one = lib.echo_workspace_bytes(128, 10240, 2048, 64, 1)                               # unsplit: no partials at all
+    assert 10240 * 8 <= one < 4 * 1024 * 1024
+    assert lib.echo_workspace_bytes(256, 0, 4096, 0, 1) >= (4096 + 256) * 8               # echo_accept_stochastic statistics
+    assert lib.echo_workspace_bytes(-1, 0, 0, 0, 1) == 0
+    assert lib.echo_attn_splits(None, 4, 2) == -1
 
 
 def test_null_arguments_rejected(lib):
