@@ -44,10 +44,10 @@ constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
 constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;
 constexpr int ST_L0 = 0, ST_N0 = 1, ST_M0 = 2, ST_L1 = 3, ST_N1 = 4;
 constexpr int SMEM_BAR = SMEM_STATS + 5 * TILE_M * 4;
-constexpr int BAR_BYTES = 256;                      // up to 32 mbarriers
+constexpr int BAR_BYTES = 320;                      // up to 40 mbarriers
 constexpr int SMEM_TMEM_SLOT = SMEM_BAR + BAR_BYTES;  // 16 bytes
 constexpr int SMEM_REDO = SMEM_TMEM_SLOT + 16;        // bitmap over this CTA's items: redo in the safe form
-constexpr int REDO_WORDS = 60;
+constexpr int REDO_WORDS = 44;
 constexpr int REDO_CAP = REDO_WORDS * 32;  // items of a CTA beyond this take the safe form at once
 constexpr int SMEM_TOTAL = SMEM_REDO + REDO_WORDS * 4;  // = 227 KB exactly; dynamic smem is declared 1024-byte aligned
 static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
@@ -56,9 +56,14 @@ static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
 constexpr int NTHREADS = 512;
 constexpr int W_EPI = 8, W_PROD_K = 12, W_MMA_QK = 13, W_PROD_V = 14, W_MMA_PV = 15;
 constexpr int REGS_SOFTMAX = 192, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 192 + 80 + 40) <= 512 * 128, the launch allocation
-constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
-constexpr int TMEM_O = NSBUF * TILE_N;
-constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
+// S is produced, turned into P and consumed in HALF tiles of 64 tokens: half-tile u = 2 g + h (g = KV tile counted over
+// the CTA's whole run, h = token half) lives in TMEM buffer u % NSBUF.  The loop QK^T -> softmax -> PV -> next QK^T of a
+// buffer is then ~2000 cycles for six buffers in flight; with whole tiles and three buffers it was ~4000 for three and
+// set the pace of the kernel (event trace, round 2).
+constexpr int HALF_N = 64;
+constexpr int NSBUF = 6;
+constexpr int TMEM_O = NSBUF * HALF_N;
+constexpr int TMEM_COLS = 512;  // S_b [64 b, 64 b + 64) for b < 6, O [384,512); P_b (bf16 pairs) aliases S_b[0,32)
 // of every POLY_PERIOD weight pairs in a prefix tile, POLY_COUNT take 2^x on the FMA pipe, the rest on MUFU
 #ifndef ECHO_POLY_COUNT
 #define ECHO_POLY_COUNT 1
@@ -77,12 +82,12 @@ constexpr float LN2 = 0.6931471805599453f;
 constexpr float SUM_LO = 8.0779356694631609e-28f;  // 2^-90
 constexpr float SUM_HI = 1.2676506002282294e30f;   // 2^100
 
-constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
+constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, HALF_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
-enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
-       B_PVDONE = 20, B_OFULL = 21, B_OFREE = 22, B_STATS = 23, B_SFREE = 24, B_STATFREE = 27, B_PHASE = 28, B_COUNT = 29 };
+enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 20,
+       B_SFREE = 26, B_OFULL = 32, B_OFREE = 33, B_STATS = 34, B_STATFREE = 35, B_PHASE = 36, B_COUNT = 37 };
 static_assert(B_COUNT * 8 <= BAR_BYTES, "barrier region");
 
 struct AttnParams {
@@ -218,7 +223,7 @@ __device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
 }
 
 // weights p = 2^(s*scale_log2 + neg_m) of one 32-column chunk of a row: packed to bf16 in pk, added to the exact
-// fp32 partial sums in acc and (TAIL only) to the sums of the bf16-rounded weights in trr.  Packed f32x2 FMA / ADD
+// fp32 partial sums in acc; TAIL also adds (bf16-rounded weight - weight) to trr.  Packed f32x2 FMA / ADD
 // halve the issue slots.  TAIL = false (all keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP /
 // FADD2 with no visibility selects and no rounded sum: 2.5 issue slots per weight.
 template <bool TAIL>
@@ -249,48 +254,60 @@ __device__ __forceinline__ void weights_chunk(uint32_t (&sc)[32], uint32_t vis, 
     // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
     // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
     // combination of V rows; lse always uses the exact fp32 sum
-    if (TAIL) trr[(e >> 1) & 1] += __uint_as_float(w << 16) + __uint_as_float(w & 0xffff0000u);
+    if (TAIL) trr[(e >> 1) & 1] += (__uint_as_float(w << 16) - p0) + (__uint_as_float(w & 0xffff0000u) - p1);
   }
 }
 
-// One S row (128 fp32 columns in TMEM at tS) -> bf16 P over its first 64 columns, four 32-column chunks, the load of
-// chunk c+1 in flight while chunk c is processed.  ts = exact sum of the weights, tr = the normaliser's share.
-template <bool TAIL>
-__device__ __forceinline__ void tile_weights(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
+// One half of an S row (64 fp32 columns in TMEM at tS) -> bf16 P over its first 32 columns, two 32-column chunks, the
+// load of the second in flight while the first is processed.  ts = exact sum of the weights, tr = the normaliser's
+// share.  MASKED = the half touches tree positions or the ragged end; even then most of its chunks are all-visible
+// (prefix) or all-invisible (past the tree) for every row of the warp, which is decided per chunk by a vote: the
+// former take the mask-free form, the latter store zeros, only the chunks that hold the tree pay for the selects.
+template <bool MASKED>
+__device__ __forceinline__ void half_weights(uint32_t tS, const uint32_t (&vis)[2], float scale_log2, float neg_m,
                                              float& ts, float& tr) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
-  float trr[2] = {0.f, 0.f};
+  float trr[2] = {0.f, 0.f};                   // (rounded - exact) weight sums of the masked chunks
   uint32_t s[2][32];
   tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
+  for (int c = 0; c < 2; ++c) {
     tc::tmem_wait_ld();
-    tc::reg_fence32(s[c & 1]);
-    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
+    tc::reg_fence32(s[c]);
+    if (c == 0) tc::tmem_ld32(tS + 32, s[1]);
     uint32_t pk[16];
-    weights_chunk<TAIL>(s[c & 1], vis[c], sc2, nm2, pk, acc, trr);
-    tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunks already read (c/2 <= c)
+    if (!MASKED) {
+      weights_chunk<false>(s[c], vis[c], sc2, nm2, pk, acc, trr);
+    } else if (__all_sync(0xffffffffu, vis[c] == 0xffffffffu)) {
+      weights_chunk<false>(s[c], vis[c], sc2, nm2, pk, acc, trr);
+    } else if (__all_sync(0xffffffffu, vis[c] == 0u)) {
+#pragma unroll
+      for (int e = 0; e < 16; ++e) pk[e] = 0u;
+    } else {
+      weights_chunk<true>(s[c], vis[c], sc2, nm2, pk, acc, trr);
+    }
+    tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunk 0, which has been read
   }
   float a0, a1;
   tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
   ts = a0 + a1;
-  tr = TAIL ? trr[0] + trr[1] : ts;
+  tr = MASKED ? ts + (trr[0] + trr[1]) : ts;
 }
 
-__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
+__device__ __forceinline__ float row_max_half(uint32_t tS, const uint32_t (&vis)[2]) {
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   uint32_t s[2][32];
   tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
+  for (int c = 0; c < 2; ++c) {
     tc::tmem_wait_ld();
-    tc::reg_fence32(s[c & 1]);
-    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
-    mask_chunk(s[c & 1], vis[c]);
+    tc::reg_fence32(s[c]);
+    if (c == 0) tc::tmem_ld32(tS + 32, s[1]);
+    mask_chunk(s[c], vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2)
-      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c & 1][e]), __uint_as_float(s[c & 1][e + 1]));
+      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c][e]), __uint_as_float(s[c][e + 1]));
   }
   return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
 }
@@ -456,26 +473,32 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         PROF_WAIT(3, bar(B_QFULL), itc & 1);
         TRACE(g, 7);
         for (int j = 0; j < n; ++j, ++g) {
-          const int slot = g % NSTAGE, b = g % NSBUF;
+          const int slot = g % NSTAGE;
           PROF_WAIT(1, bar(B_KFULL + slot), (g / NSTAGE) & 1);
-          PROF_WAIT(2, bar(B_SFREE + b), ((g / NSBUF) & 1) ^ 1);  // PV of tile g - NSBUF has read P_b
-          tc::tc_fence_after();
-          // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half h at +1 KB inside a group
-          const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, GROUP_BYTES);
-          TRACE(g, 0);
-          if (tc::elect_one()) {
 #pragma unroll
-            for (int kk = 0; kk < D / 16; ++kk) {
-              const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
-              const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
-              tc::mma_ss(tmem_u + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
+          for (int h = 0; h < 2; ++h) {
+            const int u = 2 * g + h, b = u % NSBUF;
+            PROF_WAIT(2, bar(B_SFREE + b), ((u / NSBUF) & 1) ^ 1);  // PV of half-tile u - NSBUF has read P_b
+            tc::tc_fence_after();
+            // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half at +1 KB inside a group; token half h = groups 8h..
+            const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES + h * (HALF_N / 8) * GROUP_BYTES, 16, GROUP_BYTES);
+            TRACE(u, 0);
+            if (tc::elect_one()) {
+#pragma unroll
+              for (int kk = 0; kk < D / 16; ++kk) {
+                const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
+                const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
+                tc::mma_ss(tmem_u + b * HALF_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
+              }
+              tc::mma_commit(bar(B_SFULL + b));
+              if (h == 1) {
+                tc::mma_commit(bar(B_KEMPTY + slot));
+                if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
+              }
             }
-            tc::mma_commit(bar(B_SFULL + b));
-            tc::mma_commit(bar(B_KEMPTY + slot));
-            if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
+            __syncwarp();
+            TRACE(u, 1);
           }
-          __syncwarp();
-          TRACE(g, 1);
         }
         ++itc;
       };
@@ -499,26 +522,34 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         const int4 rec = p.items[2 * idx];
         const int n = tc::uniform(rec.w - rec.z);
         for (int j = 0; j < n; ++j, ++g) {
-          const int b = g % NSBUF, slot = g % NSTAGE;
-          tc::mbar_wait(bar(B_PFULL + b), (g / NSBUF) & 1);
-          tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
-          if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
-          tc::tc_fence_after();
-          // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO).
-          // P (bf16 pairs) sits in columns [0,64) of S_b: 16 tokens = 8 columns per MMA.
-          const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, 1024, GROUP_BYTES);
-          TRACE(g, 4);
-          if (tc::elect_one()) {
+          const int slot = g % NSTAGE;
 #pragma unroll
-            for (int kk = 0; kk < TILE_N / 16; ++kk)
-              tc::mma_ts(tO, tmem_u + b * TILE_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV, (j > 0) || (kk > 0));
-            tc::mma_commit(bar(B_VEMPTY + slot));
-            tc::mma_commit(bar(B_SFREE + b));
-            tc::mma_commit(bar(B_PVDONE));
-            if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+          for (int h = 0; h < 2; ++h) {
+            const int u = 2 * g + h, b = u % NSBUF;
+            tc::mbar_wait(bar(B_PFULL + b), (u / NSBUF) & 1);
+            if (h == 0) {
+              tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
+              if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
+            }
+            tc::tc_fence_after();
+            // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO); token
+            // half h = groups 8h..  P (bf16 pairs) sits in columns [0,32) of S_b: 16 tokens = 8 columns per MMA.
+            const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES + h * (HALF_N / 8) * GROUP_BYTES, 1024, GROUP_BYTES);
+            TRACE(u, 4);
+            if (tc::elect_one()) {
+#pragma unroll
+              for (int kk = 0; kk < HALF_N / 16; ++kk)
+                tc::mma_ts(tO, tmem_u + b * HALF_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV,
+                           (j > 0) || (h > 0) || (kk > 0));
+              tc::mma_commit(bar(B_SFREE + b));
+              if (h == 1) {
+                tc::mma_commit(bar(B_VEMPTY + slot));
+                if (j == n - 1) tc::mma_commit(bar(B_OFULL));
+              }
+            }
+            __syncwarp();
+            TRACE(u, 5);
           }
-          __syncwarp();
-          TRACE(g, 5);
         }
         ++itc;
       };
@@ -532,9 +563,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     __syncwarp();
   } else if (warp < W_EPI) {
     // ============================== softmax (warpgroups 0 and 1, thread = row) ==============================
-    // KV tile g (counted over the CTA's whole run) belongs to warpgroup g & 1; in the safe form every tile belongs
-    // to warpgroup 0, which then keeps the running row maximum.  Each warpgroup adds up the weights of its own tiles
-    // and publishes them once per item; the epilogue adds the two.
+    // Warpgroup w takes token half w (64 columns) of every KV tile, each half with its own S-full / P-full barrier, so
+    // the two warpgroups never wait for one another; in the safe form warpgroup 0 takes both halves in order and keeps
+    // the running row maximum.  Each warpgroup adds up the weights of its halves and publishes them once per item; the
+    // epilogue adds the two.
     tc::setmaxnreg_inc<REGS_SOFTMAX>();
     int wg = warp >> 2;
     asm volatile("" : "+r"(wg));  // keep it in a register: recomputing it from %tid (S2R) in every loop costs ~5 %
@@ -555,89 +587,91 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const int P = it.P, total = it.P + it.Ki;
       float m_used = safe ? -INFINITY : 0.f, lsum = 0.f, lnorm = 0.f;
       const uint32_t tO = tmem + TMEM_O + lane_addr;
-      // my tiles of this item: every second one, or all / none in the safe form
-      const int first = safe ? (wg ? it.jt1 - it.jt0 : 0) : ((g ^ wg) & 1), step = safe ? 1 : 2;
-      const int g_end = g + (it.jt1 - it.jt0);
-      g += first;
-      for (int j = it.jt0 + first; j < it.jt1; j += step, g += step) {
-        const int b = g % NSBUF;
-        const uint32_t tS = tmem + b * TILE_N + lane_addr;
+      const int u_first = 2 * g;
+      // fast form: warpgroup w takes token half w of every tile; safe form: warpgroup 0 takes both halves in order
+      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
+#pragma unroll 1
+        for (int h = safe ? 0 : wg; h < (safe ? (wg ? 0 : 2) : wg + 1); ++h) {
+          const int u = 2 * g + h, b = u % NSBUF;
+          const uint32_t tS = tmem + b * HALF_N + lane_addr;
 #ifdef ECHO_WAIT_PROF
-        if (j == it.jt0 + first) prof_[4] += clock64() - gap_t_; else prof_[2] += clock64() - gap_t_;
+          prof_[4] += clock64() - gap_t_;
 #endif
-        PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
-        PROF_SPAN_BEGIN();
-        if (wq == 0) TRACE(g, 2);
-        tc::tc_fence_after();
-        const int tile0 = j * TILE_N;
-        const bool tail = tile0 + TILE_N > P;  // the tile touches tree positions or the ragged end: apply visibility
-        uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
-        if (tail) {
-#pragma unroll
-          for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tile0 + 32 * c);
-        }
-        float ts = 0.f, tr = 0.f;  // this tile's exact weight sum / share of the normaliser
-        if (!safe) {
-          if (tail) tile_weights<true>(tS, vis, p.scale_log2, 0.f, ts, tr);
-          else tile_weights<false>(tS, vis, p.scale_log2, 0.f, ts, tr);
-        } else {
-          // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same path:
-          // the TMEM instructions are warp-wide)
-          const float mx = row_max_pass(tS, vis);
-          const float m_new = fmaxf(m_used, mx * p.scale_log2);
-          float alpha = 1.f;
-          if (m_new > m_used) {
-            alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
-            m_used = m_new;
+          PROF_WAIT(1, bar(B_SFULL + b), (u / NSBUF) & 1);
+          PROF_SPAN_BEGIN();
+          if (wq == 0) TRACE(u, 2);
+          tc::tc_fence_after();
+          const int tok0 = j * TILE_N + h * HALF_N;
+          const bool masked = tok0 + HALF_N > P;  // the half touches tree positions or the ragged end
+          uint32_t vis[2] = {0xffffffffu, 0xffffffffu};
+          if (masked) {
+            vis[0] = visible_word(mk, P, tok0);
+            vis[1] = visible_word(mk, P, tok0 + 32);
           }
-          lsum *= alpha;
-          lnorm *= alpha;
-          if (j > it.jt0 && __any_sync(0xffffffffu, alpha != 1.f)) {  // O holds PV of earlier tiles
-            PROF_WAIT(3, bar(B_PVDONE), (g - 1) & 1);
-            tc::tc_fence_after();
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              uint32_t o[32];
-              tc::tmem_ld32(tO + c * 32, o);
-              tc::tmem_wait_ld();
-              tc::reg_fence32(o);
-#pragma unroll
-              for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-              tc::tmem_st32(tO + c * 32, o);
+          float ts = 0.f, tr = 0.f;  // this half's exact weight sum / share of the normaliser
+          if (!safe) {
+            if (masked) half_weights<true>(tS, vis, p.scale_log2, 0.f, ts, tr);
+            else half_weights<false>(tS, vis, p.scale_log2, 0.f, ts, tr);
+          } else {
+            // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same
+            // path: the TMEM instructions are warp-wide)
+            const float mx = row_max_half(tS, vis);
+            const float m_new = fmaxf(m_used, mx * p.scale_log2);
+            float alpha = 1.f;
+            if (m_new > m_used) {
+              alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
+              m_used = m_new;
             }
-            tc::tmem_wait_st();
-          }
-          const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-          tile_weights<true>(tS, vis, p.scale_log2, -m_eff, ts, tr);  // vis is all ones off the tail
-        }
-        lsum += ts;
-        lnorm += tr;
-        tc::tmem_wait_st();
-        if (tile0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
-          const int slot = g % NSTAGE;
-          PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
-          if (row >= total - tile0) {  // both d-halves of V row `row`
+            lsum *= alpha;
+            lnorm *= alpha;
+            if (u > u_first && __any_sync(0xffffffffu, alpha != 1.f)) {  // O holds PV of earlier halves
+              // every PV issued so far must have landed: the last one is PV(u-1), whose commit frees its S buffer.
+              // That barrier is at most one phase behind here (QK(u) was issued after PV(u-6), hence PV(u-7), was
+              // done), so the parity wait is unambiguous -- a single per-half "PV done" barrier can lag by several.
+              PROF_WAIT(3, bar(B_SFREE + (u - 1) % NSBUF), ((u - 1) / NSBUF) & 1);
+              tc::tc_fence_after();
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (row >> 3) * GROUP_BYTES + h * 1024 +
-                                                 (row & 7) * 128);
+              for (int c = 0; c < 4; ++c) {
+                uint32_t o[32];
+                tc::tmem_ld32(tO + c * 32, o);
+                tc::tmem_wait_ld();
+                tc::reg_fence32(o);
+#pragma unroll
+                for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+                tc::tmem_st32(tO + c * 32, o);
+              }
+              tc::tmem_wait_st();
+            }
+            const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+            half_weights<true>(tS, vis, p.scale_log2, -m_eff, ts, tr);
+          }
+          lsum += ts;
+          lnorm += tr;
+          tc::tmem_wait_st();
+          if (tok0 + HALF_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
+            const int slot = g % NSTAGE;
+            PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
+            // the warpgroup's 128 threads clear the 64 token rows of this half, thread = (d-half, token)
+            const int t_loc = row & 63, dh = row >> 6, tok = h * HALF_N + t_loc;
+            if (tok0 + t_loc >= total) {
+              uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (tok >> 3) * GROUP_BYTES + dh * 1024 +
+                                                 (tok & 7) * 128);
 #pragma unroll
               for (int e = 0; e < 8; ++e) z[e] = make_uint4(0u, 0u, 0u, 0u);
             }
+            tc::fence_proxy_async();
           }
-          tc::fence_proxy_async();
-        }
-        tc::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
-        if (wq == 0) TRACE(g, 3);
-        PROF_SPAN_END(5);
-        PROF_COUNT(6);
+          tc::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
+          if (wq == 0) TRACE(u, 3);
+          PROF_SPAN_END(5);
+          PROF_COUNT(6);
 #ifdef ECHO_WAIT_PROF
-        gap_t_ = clock64();
+          gap_t_ = clock64();
 #endif
+        }
       }
-      g = g_end;
       // ---- publish this warpgroup's sums (and warpgroup 0's reference) for the epilogue ----
       PROF_SPAN2_BEGIN();
       PROF_WAIT(2, bar(B_STATFREE), (itc & 1) ^ 1);  // the epilogue has read the statistics of the previous item
@@ -864,21 +898,25 @@ struct TmapCache {
 
 void free_tmap_cache(TmapCache* c) { delete c; }
 
-static const CUtensorMap* cached_tmap(EchoCtx* ctx, const void* base, uint64_t a, uint64_t b, uint64_t c,
-                                      int (*encode)(EchoCtx*, CUtensorMap*, const void*, uint64_t, uint64_t, uint64_t)) {
+// Copies the map out: a later insertion of the same call may recycle the slot a hit was found in.
+static int cached_tmap(EchoCtx* ctx, CUtensorMap* out, const void* base, uint64_t a, uint64_t b, uint64_t c,
+                       int (*encode)(EchoCtx*, CUtensorMap*, const void*, uint64_t, uint64_t, uint64_t)) {
   if (!ctx->tmaps) ctx->tmaps = new TmapCache();
   TmapCache* tc_ = ctx->tmaps;
   for (int i = 0; i < tc_->used; ++i)
-    if (tc_->e[i].base == base && tc_->e[i].a == a && tc_->e[i].b == b && tc_->e[i].c == c) return &tc_->e[i].map;
+    if (tc_->e[i].base == base && tc_->e[i].a == a && tc_->e[i].b == b && tc_->e[i].c == c) {
+      *out = tc_->e[i].map;
+      return ECHO_OK;
+    }
   TmapCache::Entry& ent = tc_->e[tc_->next];
-  if (encode(ctx, &ent.map, base, a, b, c) != ECHO_OK) {
-    ent.base = nullptr;
-    return nullptr;
-  }
+  ent.base = nullptr;
+  const int rc = encode(ctx, &ent.map, base, a, b, c);
+  if (rc != ECHO_OK) return rc;
   ent.base = base; ent.a = a; ent.b = b; ent.c = c;
   tc_->next = (tc_->next + 1) % TmapCache::N;
   if (tc_->used < TmapCache::N) ++tc_->used;
-  return &ent.map;
+  *out = ent.map;
+  return ECHO_OK;
 }
 
 // Q / out [cap][Hq][128] bf16 as a 3-D map, box = {64 d, G heads, 128/G nodes}
@@ -942,10 +980,11 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   }
   const size_t total_rows = (size_t)kv->num_layers * kv->num_pages * Hkv * PAGE;
   if (total_rows >= (1ull << 31)) return ECHO_ERR_UNSUPPORTED;
-  const CUtensorMap* tq = cached_tmap(ctx, q, (uint64_t)cap, (uint64_t)Hq, (uint64_t)G, encode_q);
-  const CUtensorMap* tk = cached_tmap(ctx, kv->k_pool, total_rows, 0, 0, encode_pool);
-  const CUtensorMap* tv = cached_tmap(ctx, kv->v_pool, total_rows, 0, 0, encode_pool);
-  if (!tq || !tk || !tv) return ECHO_ERR_CUDA;
+  CUtensorMap tq, tk, tv;
+  if (cached_tmap(ctx, &tq, q, (uint64_t)cap, (uint64_t)Hq, (uint64_t)G, encode_q) != ECHO_OK ||
+      cached_tmap(ctx, &tk, kv->k_pool, total_rows, 0, 0, encode_pool) != ECHO_OK ||
+      cached_tmap(ctx, &tv, kv->v_pool, total_rows, 0, 0, encode_pool) != ECHO_OK)
+    return ECHO_ERR_CUDA;
   // plan region sits behind the split partials in the workspace
   const size_t n_rows = (size_t)cap * Hq;
   const size_t part_bytes = splits > 1 ? align_up((size_t)splits * n_rows * (D + 1) * sizeof(float), 256) : 0;
@@ -984,7 +1023,7 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, *tq, *tk, *tv, p));
+    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, tq, tk, tv, p));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

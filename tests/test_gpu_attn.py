@@ -178,6 +178,28 @@ def test_attn_extreme_scores(path, regime):
     assert ctx.device_status() == 0
 
 
+@pytest.mark.parametrize("cfg,R,splits", [(0, None, 1), (0, None, 3), (1, 3, 0), (2, 3, 1)])
+def test_attn_safe_form_on_regular_scores(cfg, R, splits):
+    """ECHO_OPT_ATTN_SAFE: every item takes the tcgen05 kernel's safe form (running row maximum, O rescaled in TMEM,
+    one warpgroup) -- the form an item is redone in when its row sums leave the fast form's window -- on ordinary
+    scores, where the oracle and the fast form are known to agree."""
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(cfg, R=R, gated=True)
+    ctx, sel, want_sel, q, k, v = _setup(wl, poison=True)
+    ctx.set_option(echo.OPT_ATTN_PATH, 2)
+    ctx.set_option(echo.OPT_ATTN_SAFE, 1)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, splits)
+    out, lse = ctx.verify_attn(sel, make_kv(wl, k, v), q, SM_SCALE)
+    n = want_sel["n_selected"]
+    if cfg == 0:
+        _compare(wl, want_sel, q, k, v, out, lse)
+    else:
+        rng = np.random.default_rng(31 + cfg)
+        rows = [(int(rng.integers(0, n)), int(rng.integers(0, wl.Hq))) for _ in range(96)] + [(0, 0), (n - 1, wl.Hq - 1)]
+        _compare(wl, want_sel, q, k, v, out, lse, rows=rows)
+    assert ctx.device_status() == 0
+
+
 @pytest.mark.parametrize("cfg,static", [(2, False), (2, True), (3, False)])
 def test_attn_full_size_bench_configuration(cfg, static):
     """BASELINE.json's full sizes (BS=128) in the launch configuration bench.py times (default path, default
