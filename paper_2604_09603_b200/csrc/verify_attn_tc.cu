@@ -44,10 +44,10 @@ constexpr int SMEM_V = SMEM_K + NSTAGE * TILE_BYTES;
 constexpr int SMEM_STATS = SMEM_V + NSTAGE * TILE_BYTES;
 constexpr int ST_L0 = 0, ST_N0 = 1, ST_M0 = 2, ST_L1 = 3, ST_N1 = 4;
 constexpr int SMEM_BAR = SMEM_STATS + 5 * TILE_M * 4;
-constexpr int BAR_BYTES = 320;                      // up to 40 mbarriers
+constexpr int BAR_BYTES = 256;                      // up to 32 mbarriers
 constexpr int SMEM_TMEM_SLOT = SMEM_BAR + BAR_BYTES;  // 16 bytes
 constexpr int SMEM_REDO = SMEM_TMEM_SLOT + 16;        // bitmap over this CTA's items: redo in the safe form
-constexpr int REDO_WORDS = 44;
+constexpr int REDO_WORDS = 60;
 constexpr int REDO_CAP = REDO_WORDS * 32;  // items of a CTA beyond this take the safe form at once
 constexpr int SMEM_TOTAL = SMEM_REDO + REDO_WORDS * 4;  // = 227 KB exactly; dynamic smem is declared 1024-byte aligned
 static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
@@ -56,14 +56,9 @@ static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
 constexpr int NTHREADS = 512;
 constexpr int W_EPI = 8, W_PROD_K = 12, W_MMA_QK = 13, W_PROD_V = 14, W_MMA_PV = 15;
 constexpr int REGS_SOFTMAX = 192, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 192 + 80 + 40) <= 512 * 128, the launch allocation
-// S is produced, turned into P and consumed in HALF tiles of 64 tokens: half-tile u = 2 g + h (g = KV tile counted over
-// the CTA's whole run, h = token half) lives in TMEM buffer u % NSBUF.  The loop QK^T -> softmax -> PV -> next QK^T of a
-// buffer is then ~2000 cycles for six buffers in flight; with whole tiles and three buffers it was ~4000 for three and
-// set the pace of the kernel (event trace, round 2).
-constexpr int HALF_N = 64;
-constexpr int NSBUF = 6;
-constexpr int TMEM_O = NSBUF * HALF_N;
-constexpr int TMEM_COLS = 512;  // S_b [64 b, 64 b + 64) for b < 6, O [384,512); P_b (bf16 pairs) aliases S_b[0,32)
+constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
+constexpr int TMEM_O = NSBUF * TILE_N;
+constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
 // of every POLY_PERIOD weight pairs in a prefix tile, POLY_COUNT take 2^x on the FMA pipe, the rest on MUFU
 #ifndef ECHO_POLY_COUNT
 #define ECHO_POLY_COUNT 1
@@ -82,12 +77,12 @@ constexpr float LN2 = 0.6931471805599453f;
 constexpr float SUM_LO = 8.0779356694631609e-28f;  // 2^-90
 constexpr float SUM_HI = 1.2676506002282294e30f;   // 2^100
 
-constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, HALF_N, 0, 0);
+constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
-enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 20,
-       B_SFREE = 26, B_OFULL = 32, B_OFREE = 33, B_STATS = 34, B_STATFREE = 35, B_PHASE = 36, B_COUNT = 37 };
+enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
+       B_SFREE = 20, B_OFULL = 23, B_OFREE = 24, B_STATS = 25, B_STATFREE = 26, B_PHASE = 27, B_COUNT = 28 };
 static_assert(B_COUNT * 8 <= BAR_BYTES, "barrier region");
 
 struct AttnParams {
@@ -159,21 +154,58 @@ __device__ __forceinline__ int item_index(int k, int cta, int grid) {
   return (k & 1) ? (k + 1) * grid - 1 - cta : k * grid + cta;
 }
 
+// Work-list records without a global load per item: every lane of a warp holds the record of one of the CTA's items
+// k with k / 32 == blk (lane = k % 32), fetched 32 at a time, and an item's fields are broadcast by shuffles.  Under a
+// saturated memory system a dependent global load costs 2500-3500 cycles; per-item loads at the item boundaries, in
+// six roles one after another, were a third of the kernel (event trace, round 2).  A prefetch held in registers does
+// not help: ptxas spills it right behind the load, which then waits for it.
+struct ItemFeed {
+  int4 r0, r1;
+  int blk;
+  __device__ __forceinline__ void init() { blk = -1; r0 = r1 = make_int4(0, 0, 0, 0); }
+  __device__ __forceinline__ void ensure(const int4* items, int k, int cta, int grid, int n_items, int lane) {
+    if ((k >> 5) != blk) {  // warp-uniform
+      blk = k >> 5;
+      const int idx = item_index((k & ~31) + lane, cta, grid);
+      r0 = r1 = make_int4(0, 0, 0, 0);  // past the end of the list: an item without nodes or tiles
+      if (idx < n_items) { r0 = items[2 * idx]; r1 = items[2 * idx + 1]; }
+    }
+  }
+  // record of item k (any k of the block held), the same in every lane
+  __device__ __forceinline__ Item get(const int4* items, int k, int cta, int grid, int n_items, int lane) {
+    ensure(items, k, cta, grid, n_items, lane);
+    const int src = k & 31;
+    int4 a, b;
+    a.x = __shfl_sync(0xffffffffu, r0.x, src); a.y = __shfl_sync(0xffffffffu, r0.y, src);
+    a.z = __shfl_sync(0xffffffffu, r0.z, src); a.w = __shfl_sync(0xffffffffu, r0.w, src);
+    b.x = __shfl_sync(0xffffffffu, r1.x, src); b.y = __shfl_sync(0xffffffffu, r1.y, src);
+    b.z = __shfl_sync(0xffffffffu, r1.z, src); b.w = 0;
+    return decode(a, b);
+  }
+};
+
 // Every role walks the same sequence of items: first the CTA's share of the work list (phase 0; the items past
 // REDO_CAP in the safe form), then -- once the epilogue has seen the last row sums (B_PHASE) -- the items it flagged,
-// in the safe form.  fn(item index, safe).
-template <typename Fn>
-__device__ __forceinline__ void redo_phase(int cta, int grid, int n_items, const volatile uint32_t* redo, uint32_t bar_phase,
-                                           Fn&& fn) {
-  tc::mbar_wait_relaxed(bar_phase, 0);
-  uint32_t any = 0;
+// in the safe form.  fn(k, safe), k = the item's ordinal in the CTA's list.
+template <typename Fn, typename Between>
+__device__ __forceinline__ void walk_items(int cta, int grid, int n_items, bool force_safe, const volatile uint32_t* redo,
+                                           uint32_t bar_phase, Between&& between, Fn&& fn) {
+  // ONE call site of fn for both phases: the per-item code is cold (it runs once per ~14 KV tiles), and instruction
+  // fetches that miss under a saturated memory system cost hundreds of cycles per 128-byte line -- every duplicate
+  // of the item body is paid for at every item boundary.
+  for (int ph = 0; ph < 2; ++ph) {
+    if (ph == 1) {
+      between();
+      tc::mbar_wait_relaxed(bar_phase, 0);
+      uint32_t any = 0;
 #pragma unroll 4
-  for (int w = 0; w < REDO_WORDS; ++w) any |= redo[w];
-  if (!any) return;
-  for (int k = 0; k < REDO_CAP; ++k) {
-    const int idx = item_index(k, cta, grid);
-    if (idx >= n_items) break;
-    if ((redo[k >> 5] >> (k & 31)) & 1u) fn(idx, true);
+      for (int w = 0; w < REDO_WORDS; ++w) any |= redo[w];
+      if (!any) break;
+    }
+    for (int k = 0; item_index(k, cta, grid) < n_items; ++k) {  // item indices grow with k
+      if (ph == 1 && (k >= REDO_CAP || !((redo[k >> 5] >> (k & 31)) & 1u))) continue;
+      fn(k, ph, ph == 1 || force_safe || k >= REDO_CAP);
+    }
   }
 }
 
@@ -222,14 +254,12 @@ __device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
   p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
 }
 
-// weights p = 2^(s*scale_log2 + neg_m) of one 32-column chunk of a row: packed to bf16 in pk, added to the exact
-// fp32 partial sums in acc; TAIL also adds (bf16-rounded weight - weight) to trr.  Packed f32x2 FMA / ADD
-// halve the issue slots.  TAIL = false (all keys inside the prefix) compiles to straight-line FFMA2 / MUFU / F2FP /
-// FADD2 with no visibility selects and no rounded sum: 2.5 issue slots per weight.
-template <bool TAIL>
-__device__ __forceinline__ void weights_chunk(uint32_t (&sc)[32], uint32_t vis, uint64_t sc2, uint64_t nm2,
-                                              uint32_t (&pk)[16], uint64_t (&acc)[4], float (&trr)[2]) {
-  if (TAIL) mask_chunk(sc, vis);
+// weights p = 2^(s*scale_log2 + neg_m) of one 32-column chunk of a row: packed to bf16 in pk, added to the exact fp32
+// partial sums in acc.  Packed f32x2 FMA / ADD halve the issue slots: straight-line FFMA2 / MUFU / F2FP / FADD2, 2.5
+// issue slots per weight.  A masked key arrives as -inf: MUFU turns it into 0, the polynomial form (which clamps at
+// -125) into 2^-125, which is below anything the row-sum window lets through.
+__device__ __forceinline__ void weights_chunk(const uint32_t (&sc)[32], uint64_t sc2, uint64_t nm2, uint32_t (&pk)[16],
+                                              uint64_t (&acc)[4]) {
 #pragma unroll
   for (int e = 0; e < 32; e += 2) {
     const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
@@ -237,7 +267,7 @@ __device__ __forceinline__ void weights_chunk(uint32_t (&sc)[32], uint32_t vis, 
 #ifdef ECHO_EXP_NOEXP
     tc::unpack_f32x2(x2, p0, p1);
 #else
-    if (!TAIL && ((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
+    if (((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
       ex2_poly_x2(x2, p0, p1);
     } else {
       float x0, x1;
@@ -246,68 +276,111 @@ __device__ __forceinline__ void weights_chunk(uint32_t (&sc)[32], uint32_t vis, 
       p1 = tc::ex2(x1);
     }
 #endif
-    const uint32_t w = tc::pack_bf16(p0, p1);
-    pk[e >> 1] = w;
+    pk[e >> 1] = tc::pack_bf16(p0, p1);
 #ifndef ECHO_EXP_NOSUM
     acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
 #endif
-    // tiles that touch the tree / ragged end may have a handful of visible keys: there O is normalised by the
-    // sum of the bf16-rounded weights the tensor core multiplies with, so that O stays an exact convex
-    // combination of V rows; lse always uses the exact fp32 sum
-    if (TAIL) trr[(e >> 1) & 1] += (__uint_as_float(w << 16) - p0) + (__uint_as_float(w & 0xffff0000u) - p1);
   }
 }
 
-// One half of an S row (64 fp32 columns in TMEM at tS) -> bf16 P over its first 32 columns, two 32-column chunks, the
-// load of the second in flight while the first is processed.  ts = exact sum of the weights, tr = the normaliser's
-// share.  MASKED = the half touches tree positions or the ragged end; even then most of its chunks are all-visible
-// (prefix) or all-invisible (past the tree) for every row of the warp, which is decided per chunk by a vote: the
-// former take the mask-free form, the latter store zeros, only the chunks that hold the tree pay for the selects.
-template <bool MASKED>
-__device__ __forceinline__ void half_weights(uint32_t tS, const uint32_t (&vis)[2], float scale_log2, float neg_m,
-                                             float& ts, float& tr) {
+__device__ __forceinline__ float acc_total(const uint64_t (&acc)[4]) {
+  float a0, a1;
+  tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
+  return a0 + a1;
+}
+
+// One chunk of a row, S registers -> P in TMEM.  In a tile that touches the tree or the ragged end (`masked`, uniform
+// over the CTA) a vote over the warp's rows sorts the chunk: all keys visible -> nothing to do; none visible -> zeros;
+// else the invisible keys are set to -inf and the chunk's share of the normaliser becomes the sum of the bf16-ROUNDED
+// weights (few visible keys: O must stay an exact convex combination of V rows; lse always takes the exact sum).
+// One body for both kinds of tile, on purpose: the masked tile runs once per item, and code that runs once per item
+// is fetched from L2 every time -- the separate masked instantiation cost ~2000 cycles per item in instruction misses.
+__device__ __forceinline__ void chunk_to_p(uint32_t (&sc)[32], uint32_t vis, bool masked, uint64_t sc2, uint64_t nm2,
+                                           uint32_t tP, uint64_t (&acc)[4], float& tr_adj) {
+  uint32_t pk[16];
+  bool partial = false;
+  if (masked && !__all_sync(0xffffffffu, vis == 0xffffffffu)) {
+    if (__all_sync(0xffffffffu, vis == 0u)) {
+#pragma unroll
+      for (int e = 0; e < 16; ++e) pk[e] = 0u;
+      tc::tmem_st16(tP, pk);
+      return;
+    }
+    mask_chunk(sc, vis);
+    partial = true;
+  }
+  const float before = partial ? acc_total(acc) : 0.f;
+  weights_chunk(sc, sc2, nm2, pk, acc);
+  if (partial) {  // (rounded - exact) sum of this chunk's weights
+    float r0 = 0.f, r1 = 0.f;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      r0 += __uint_as_float(pk[e] << 16);
+      r1 += __uint_as_float(pk[e] & 0xffff0000u);
+    }
+    tr_adj += (r0 + r1) - (acc_total(acc) - before);
+  }
+  tc::tmem_st16(tP, pk);
+}
+
+// One S row (128 fp32 columns in TMEM at tS) -> bf16 P over its first 64 columns, four 32-column chunks, the load of
+// chunk c+1 in flight while chunk c is processed.  ts = exact sum of the weights.  This is the hot loop of the kernel:
+// every key inside the prefix, no visibility logic, fully unrolled.
+__device__ __forceinline__ void tile_weights_fast(uint32_t tS, float scale_log2, float neg_m, float& ts) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
-  float trr[2] = {0.f, 0.f};                   // (rounded - exact) weight sums of the masked chunks
   uint32_t s[2][32];
   tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 2; ++c) {
+  for (int c = 0; c < 4; ++c) {
     tc::tmem_wait_ld();
-    tc::reg_fence32(s[c]);
-    if (c == 0) tc::tmem_ld32(tS + 32, s[1]);
+    tc::reg_fence32(s[c & 1]);
+    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
     uint32_t pk[16];
-    if (!MASKED) {
-      weights_chunk<false>(s[c], vis[c], sc2, nm2, pk, acc, trr);
-    } else if (__all_sync(0xffffffffu, vis[c] == 0xffffffffu)) {
-      weights_chunk<false>(s[c], vis[c], sc2, nm2, pk, acc, trr);
-    } else if (__all_sync(0xffffffffu, vis[c] == 0u)) {
-#pragma unroll
-      for (int e = 0; e < 16; ++e) pk[e] = 0u;
-    } else {
-      weights_chunk<true>(s[c], vis[c], sc2, nm2, pk, acc, trr);
-    }
-    tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunk 0, which has been read
+    weights_chunk(s[c & 1], sc2, nm2, pk, acc);
+    tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunks already read (c/2 <= c)
   }
-  float a0, a1;
-  tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
-  ts = a0 + a1;
-  tr = MASKED ? ts + (trr[0] + trr[1]) : ts;
+  ts = acc_total(acc);
 }
 
-__device__ __forceinline__ float row_max_half(uint32_t tS, const uint32_t (&vis)[2]) {
+// The same for a tile that touches the tree or the ragged end (once or twice per item) and for the safe form: the
+// loop is rolled over chunk pairs and shares one body for all kinds of chunk -- compact rather than fast, because
+// code that runs once per item is fetched from L2 every time.  tr = the normaliser's share.
+__device__ __forceinline__ void tile_weights_masked(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
+                                                    float& ts, float& tr) {
+  const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
+  uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};
+  float tr_adj = 0.f;
+  uint32_t s0[32], s1[32];
+  tc::tmem_ld32(tS, s0);
+#pragma unroll 1
+  for (int cc = 0; cc < 2; ++cc) {
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s0);
+    tc::tmem_ld32(tS + 64 * cc + 32, s1);
+    chunk_to_p(s0, cc ? vis[2] : vis[0], true, sc2, nm2, tS + 32 * cc, acc, tr_adj);  // P columns [32cc, 32cc+16)
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s1);
+    if (cc == 0) tc::tmem_ld32(tS + 64, s0);
+    chunk_to_p(s1, cc ? vis[3] : vis[1], true, sc2, nm2, tS + 32 * cc + 16, acc, tr_adj);
+  }
+  ts = acc_total(acc);
+  tr = ts + tr_adj;
+}
+
+__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   uint32_t s[2][32];
   tc::tmem_ld32(tS, s[0]);
 #pragma unroll
-  for (int c = 0; c < 2; ++c) {
+  for (int c = 0; c < 4; ++c) {
     tc::tmem_wait_ld();
-    tc::reg_fence32(s[c]);
-    if (c == 0) tc::tmem_ld32(tS + 32, s[1]);
-    mask_chunk(s[c], vis[c]);
+    tc::reg_fence32(s[c & 1]);
+    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
+    mask_chunk(s[c & 1], vis[c]);
 #pragma unroll
     for (int e = 0; e < 32; e += 2)
-      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c][e]), __uint_as_float(s[c][e + 1]));
+      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c & 1][e]), __uint_as_float(s[c & 1][e + 1]));
   }
   return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
 }
@@ -371,28 +444,26 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       int g = 0, itc = 0;
       PROF_DECL(3);
       PROF_T0();
-      // The next item's Q tile (V warp) and its rows' ancestor masks (K warp) are pulled into L2 one item ahead: the
-      // masks are read by the softmax threads at the item boundary, where a DRAM miss under a saturated memory
-      // system cost them ~3000 cycles per dependent load (wait profile, round 2).
-      auto prefetch_next = [&](const Item& nx) {
-        const int node0 = tc::uniform(nx.off) + tc::uniform(nx.rt) * (TILE_M >> p.log2G);
-        if (loads_q) {
-          const int h0 = tc::uniform(nx.kvh) * p.G;
-          if (tc::elect_one()) {
-            tc::tma_prefetch_3d(&tmap_q, 0, h0, node0);
-            tc::tma_prefetch_3d(&tmap_q, 64, h0, node0);
-          }
-          __syncwarp();
-        } else {
-          const int bytes = min(TILE_M >> p.log2G, max(0, nx.Ki - nx.rt * (TILE_M >> p.log2G))) * 16;
-          if (lane * 128 < bytes) tc::prefetch_l2(reinterpret_cast<const uint8_t*>(p.anc_mask + node0) + lane * 128);
-        }
-      };
-      auto produce = [&](const Item& t, const Item* next) {
+      ItemFeed feed;
+      feed.init();
+      auto fetch = [&](int k) {  // record of item k with every field provably warp-uniform (TMA operands)
+        const Item t = feed.get(p.items, k, cta, grid, n_items, lane);
         Item it;
-        it.req = tc::uniform(t.req); it.kvh = tc::uniform(t.kvh); it.rt = tc::uniform(t.rt);
+        it.req = tc::uniform(t.req); it.kvh = tc::uniform(t.kvh); it.rt = tc::uniform(t.rt); it.split = 0;
         it.jt0 = tc::uniform(t.jt0); it.jt1 = tc::uniform(t.jt1); it.P = tc::uniform(t.P); it.off = tc::uniform(t.off);
         it.Ki = tc::uniform(t.Ki);
+        return it;
+      };
+      auto n_pages = [&](const Item& it) { return min((it.P + it.Ki + PAGE - 1) / PAGE, p.max_pages); };
+      auto tile_page = [&](const Item& it, int j) -> int {  // lane e < 8: id of page e of tile j (0 past the end)
+        const int pi = j * 8 + (lane & 7);
+        return pi < n_pages(it) ? p.page_table[(size_t)it.req * p.max_pages + pi] : 0;
+      };
+      int cur = 0;            // page ids of the tile about to be issued, fetched one tile ahead -- across items too
+      bool cur_valid = false;
+      // `ahead`: the item after this one in the list (phase 0), whose first tile's page ids and Q tile are requested
+      // before this item ends, or nullptr
+      auto produce = [&](const Item& it, const Item* ahead) {
         const int total = it.P + it.Ki;
         if (loads_q) {
           PROF_WAIT_BACKOFF(2, bar(B_QEMPTY), (itc & 1) ^ 1);
@@ -404,20 +475,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           }
           __syncwarp();
           TRACE(g, 6);
+          if (ahead && ahead->jt1 > ahead->jt0) {  // the next item's Q tile into L2 while this item runs
+            const int node1 = ahead->off + ahead->rt * (TILE_M >> p.log2G);
+            if (tc::elect_one()) {
+              tc::tma_prefetch_3d(&tmap_q, 0, ahead->kvh * p.G, node1);
+              tc::tma_prefetch_3d(&tmap_q, 64, ahead->kvh * p.G, node1);
+            }
+            __syncwarp();
+          }
         }
-        const int32_t* pt = p.page_table + (size_t)it.req * p.max_pages;
-        int npages = (total + PAGE - 1) / PAGE;
-        if (npages > p.max_pages) {  // page table too short: flag, load what exists
-          if (is_k && lane == 0) atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);
-          npages = p.max_pages;
-        }
-        auto tile_page = [&](int j) -> int {  // lane e < 8: id of page e of tile j
-          const int pi = j * 8 + (lane & 7);
-          return pi < npages ? pt[pi] : 0;
-        };
-        int cur = tile_page(it.jt0);
+        if ((total + PAGE - 1) / PAGE > p.max_pages && is_k && lane == 0)
+          atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);  // page table too short: flag, load what exists
+        const int npages = n_pages(it);
+        if (!cur_valid) cur = tile_page(it, it.jt0);
         for (int j = it.jt0; j < it.jt1; ++j, ++g) {
-          const int nxt = j + 1 < it.jt1 ? tile_page(j + 1) : 0;
+          int nxt = 0;
+          cur_valid = false;
+          if (j + 1 < it.jt1) nxt = tile_page(it, j + 1);
+          else if (ahead && ahead->jt1 > ahead->jt0) { nxt = tile_page(*ahead, ahead->jt0); cur_valid = true; }
           const int slot = g % NSTAGE, ph = (g / NSTAGE) & 1;
           const int npv = max(0, min(8, npages - j * 8));  // pages of this tile that hold tokens
           const uint32_t dst = s_dst + slot * TILE_BYTES;
@@ -438,20 +513,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           }
           __syncwarp();
           cur = nxt;
-          if (j == it.jt0 && next) prefetch_next(*next);  // its record was requested before this item began
         }
         ++itc;
       };
-      Item nx = {};
-      bool more = item_index(0, cta, grid) < n_items;  // item indices grow with k
-      if (more) nx = load_item(p.items, item_index(0, cta, grid));
-      for (int k = 1; more; ++k) {
-        const Item it = nx;
-        more = item_index(k, cta, grid) < n_items;
-        if (more) nx = load_item(p.items, item_index(k, cta, grid));
+      walk_items(cta, grid, n_items, force_safe, redo, bar(B_PHASE), [&]() { cur_valid = false; }, [&](int k, int ph, bool) {
+        const Item it = fetch(k);
+        const bool more = ph == 0 && item_index(k + 1, cta, grid) < n_items;
+        Item nx = it;
+        if (more) nx = fetch(k + 1);  // same 32-block except once in 32 items
+        if (ph == 1) cur_valid = false;
         produce(it, more ? &nx : nullptr);
-      }
-      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) { produce(load_item(p.items, idx), nullptr); });
+      });
       PROF_ADD(0);
       if (lane == 0) PROF_FLUSH(is_k ? 0 : 4, 3);
     }
@@ -467,47 +539,39 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       PROF_T0();
       const uint32_t tmem_u = (uint32_t)tc::uniform((int)tmem);
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
-      auto issue = [&](int idx, bool) {
-        const int4 rec = p.items[2 * idx];
-        const int n = tc::uniform(rec.w - rec.z);
+      ItemFeed feed;
+      feed.init();
+      auto issue = [&](int k, int, bool) {
+        const Item rec = feed.get(p.items, k, cta, grid, n_items, lane);
+        const int n = tc::uniform(rec.jt1 - rec.jt0);
         PROF_WAIT(3, bar(B_QFULL), itc & 1);
         TRACE(g, 7);
         for (int j = 0; j < n; ++j, ++g) {
           const int slot = g % NSTAGE;
           PROF_WAIT(1, bar(B_KFULL + slot), (g / NSTAGE) & 1);
+          const int b = g % NSBUF;
+          PROF_WAIT(2, bar(B_SFREE + b), ((g / NSBUF) & 1) ^ 1);  // PV of tile g - NSBUF has read P_b
+          tc::tc_fence_after();
+          // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half at +1 KB inside a group
+          const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES, 16, GROUP_BYTES);
+          TRACE(g, 0);
+          if (tc::elect_one()) {
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int u = 2 * g + h, b = u % NSBUF;
-            PROF_WAIT(2, bar(B_SFREE + b), ((u / NSBUF) & 1) ^ 1);  // PV of half-tile u - NSBUF has read P_b
-            tc::tc_fence_after();
-            // K tile: 8-token groups GROUP_BYTES apart (SBO), d-half at +1 KB inside a group; token half h = groups 8h..
-            const uint64_t kdesc = tc::smem_desc_sw128(sK + slot * TILE_BYTES + h * (HALF_N / 8) * GROUP_BYTES, 16, GROUP_BYTES);
-            TRACE(u, 0);
-            if (tc::elect_one()) {
-#pragma unroll
-              for (int kk = 0; kk < D / 16; ++kk) {
-                const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
-                const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
-                tc::mma_ss(tmem_u + b * HALF_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
-              }
-              tc::mma_commit(bar(B_SFULL + b));
-              if (h == 1) {
-                tc::mma_commit(bar(B_KEMPTY + slot));
-                if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
-              }
+            for (int kk = 0; kk < D / 16; ++kk) {
+              const uint32_t q16 = ((kk & 3) * 32 + (kk >> 2) * HALF_BYTES) >> 4;
+              const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
+              tc::mma_ss(tmem_u + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
             }
-            __syncwarp();
-            TRACE(u, 1);
+            tc::mma_commit(bar(B_SFULL + b));
+            tc::mma_commit(bar(B_KEMPTY + slot));
+            if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
           }
+          __syncwarp();
+          TRACE(g, 1);
         }
         ++itc;
       };
-      for (int k = 0;; ++k) {
-        const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) break;  // item indices grow with k
-        issue(idx, false);
-      }
-      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), issue);
+      walk_items(cta, grid, n_items, force_safe, redo, bar(B_PHASE), []() {}, issue);
       PROF_ADD(0);
       if (lane == 0) PROF_FLUSH(8, 4);
     }
@@ -518,55 +582,46 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       int g = 0, itc = 0;
       const uint32_t tmem_u = (uint32_t)tc::uniform((int)tmem);
       const uint32_t tO = tmem_u + TMEM_O;
-      auto issue = [&](int idx, bool) {
-        const int4 rec = p.items[2 * idx];
-        const int n = tc::uniform(rec.w - rec.z);
+      ItemFeed feed;
+      feed.init();
+      auto issue = [&](int k, int, bool) {
+        const Item rec = feed.get(p.items, k, cta, grid, n_items, lane);
+        const int n = tc::uniform(rec.jt1 - rec.jt0);
         for (int j = 0; j < n; ++j, ++g) {
-          const int slot = g % NSTAGE;
+          const int b = g % NSBUF, slot = g % NSTAGE;
+          tc::mbar_wait(bar(B_PFULL + b), (g / NSBUF) & 1);
+          tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
+          if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
+          tc::tc_fence_after();
+          // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO).
+          // P (bf16 pairs) sits in columns [0,64) of S_b: 16 tokens = 8 columns per MMA.
+          const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES, 1024, GROUP_BYTES);
+          TRACE(g, 4);
+          if (tc::elect_one()) {
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int u = 2 * g + h, b = u % NSBUF;
-            tc::mbar_wait(bar(B_PFULL + b), (u / NSBUF) & 1);
-            if (h == 0) {
-              tc::mbar_wait(bar(B_VFULL + slot), (g / NSTAGE) & 1);
-              if (j == 0) tc::mbar_wait(bar(B_OFREE), (itc & 1) ^ 1);  // epilogue of the previous item has read O
-            }
-            tc::tc_fence_after();
-            // V tile as MN-major B: 64-wide d atoms 1 KB apart (LBO), 8-token groups GROUP_BYTES apart (SBO); token
-            // half h = groups 8h..  P (bf16 pairs) sits in columns [0,32) of S_b: 16 tokens = 8 columns per MMA.
-            const uint64_t vdesc = tc::smem_desc_sw128(sV + slot * TILE_BYTES + h * (HALF_N / 8) * GROUP_BYTES, 1024, GROUP_BYTES);
-            TRACE(u, 4);
-            if (tc::elect_one()) {
-#pragma unroll
-              for (int kk = 0; kk < HALF_N / 16; ++kk)
-                tc::mma_ts(tO, tmem_u + b * HALF_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV,
-                           (j > 0) || (h > 0) || (kk > 0));
-              tc::mma_commit(bar(B_SFREE + b));
-              if (h == 1) {
-                tc::mma_commit(bar(B_VEMPTY + slot));
-                if (j == n - 1) tc::mma_commit(bar(B_OFULL));
-              }
-            }
-            __syncwarp();
-            TRACE(u, 5);
+            for (int kk = 0; kk < TILE_N / 16; ++kk)
+              tc::mma_ts(tO, tmem_u + b * TILE_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV, (j > 0) || (kk > 0));
+            tc::mma_commit(bar(B_VEMPTY + slot));
+            tc::mma_commit(bar(B_SFREE + b));
+            if (j == n - 1) tc::mma_commit(bar(B_OFULL));
           }
+          __syncwarp();
+          TRACE(g, 5);
         }
         ++itc;
       };
-      for (int k = 0;; ++k) {
-        const int idx = item_index(k, cta, grid);
-        if (idx >= n_items) break;
-        issue(idx, false);
-      }
-      redo_phase(cta, grid, n_items, redo, bar(B_PHASE), issue);
+      walk_items(cta, grid, n_items, force_safe, redo, bar(B_PHASE), []() {}, issue);
     }
     __syncwarp();
   } else if (warp < W_EPI) {
     // ============================== softmax (warpgroups 0 and 1, thread = row) ==============================
-    // Warpgroup w takes token half w (64 columns) of every KV tile, each half with its own S-full / P-full barrier, so
-    // the two warpgroups never wait for one another; in the safe form warpgroup 0 takes both halves in order and keeps
-    // the running row maximum.  Each warpgroup adds up the weights of its halves and publishes them once per item; the
-    // epilogue adds the two.
+    // Warpgroup w takes the KV tiles with g & 1 == w (g counted over the CTA's whole run), thread = row.  The two warps
+    // of an SM sub-partition are then on different tiles and out of step: one computes while the other waits for S,
+    // loads it from TMEM or hands P back.  (Tried: both warpgroups on the two token halves of one tile, separate
+    // barriers per half -- they run in lockstep and 64 columns cost 1380 cycles instead of 800; halves of 64 tokens
+    // with their own QK^T products -- the N = 64 product re-reads Q for half the work and is bound by shared-memory
+    // reads.)  In the safe form warpgroup 0 takes every tile and keeps the running row maximum.  Each warpgroup adds
+    // up the weights of its tiles and publishes them once per item; the epilogue adds the two.
     tc::setmaxnreg_inc<REGS_SOFTMAX>();
     int wg = warp >> 2;
     asm volatile("" : "+r"(wg));  // keep it in a register: recomputing it from %tid (S2R) in every loop costs ~5 %
@@ -579,99 +634,99 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 #ifdef ECHO_WAIT_PROF
     long long gap_t_ = clock64();
 #endif
-    auto row_mask = [&](const int4& r0, const int4& r1) -> uint4 {
-      const int l = ((((r0.y >> 8) & 0xff) * TILE_M + row) >> p.log2G);
-      return l < r1.z ? p.anc_mask[r1.y + l] : make_uint4(0u, 0u, 0u, 0u);
-    };
     auto do_item = [&](const Item& it, const uint4& mk, const bool safe) {
       const int P = it.P, total = it.P + it.Ki;
       float m_used = safe ? -INFINITY : 0.f, lsum = 0.f, lnorm = 0.f;
       const uint32_t tO = tmem + TMEM_O + lane_addr;
-      const int u_first = 2 * g;
-      // fast form: warpgroup w takes token half w of every tile; safe form: warpgroup 0 takes both halves in order
-      for (int j = it.jt0; j < it.jt1; ++j, ++g) {
-#pragma unroll 1
-        for (int h = safe ? 0 : wg; h < (safe ? (wg ? 0 : 2) : wg + 1); ++h) {
-          const int u = 2 * g + h, b = u % NSBUF;
-          const uint32_t tS = tmem + b * HALF_N + lane_addr;
+      // fast form: warpgroup w takes the tiles with g & 1 == w; safe form: warpgroup 0 takes all of them
+      const int n_t = it.jt1 - it.jt0, g_first = g, g_end = g + n_t;
+      const int first = safe ? (wg ? n_t : 0) : ((g ^ wg) & 1), step = safe ? 1 : 2;
+      g += first;
+      for (int j = it.jt0 + first; j < it.jt1; j += step, g += step) {
+        const int b = g % NSBUF;
+        const uint32_t tS = tmem + b * TILE_N + lane_addr;
 #ifdef ECHO_WAIT_PROF
-          prof_[4] += clock64() - gap_t_;
+        prof_[4] += clock64() - gap_t_;
 #endif
-          PROF_WAIT(1, bar(B_SFULL + b), (u / NSBUF) & 1);
-          PROF_SPAN_BEGIN();
-          if (wq == 0) TRACE(u, 2);
-          tc::tc_fence_after();
-          const int tok0 = j * TILE_N + h * HALF_N;
-          const bool masked = tok0 + HALF_N > P;  // the half touches tree positions or the ragged end
-          uint32_t vis[2] = {0xffffffffu, 0xffffffffu};
-          if (masked) {
-            vis[0] = visible_word(mk, P, tok0);
-            vis[1] = visible_word(mk, P, tok0 + 32);
-          }
-          float ts = 0.f, tr = 0.f;  // this half's exact weight sum / share of the normaliser
-          if (!safe) {
-            if (masked) half_weights<true>(tS, vis, p.scale_log2, 0.f, ts, tr);
-            else half_weights<false>(tS, vis, p.scale_log2, 0.f, ts, tr);
-          } else {
-            // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same
-            // path: the TMEM instructions are warp-wide)
-            const float mx = row_max_half(tS, vis);
-            const float m_new = fmaxf(m_used, mx * p.scale_log2);
-            float alpha = 1.f;
-            if (m_new > m_used) {
-              alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
-              m_used = m_new;
-            }
-            lsum *= alpha;
-            lnorm *= alpha;
-            if (u > u_first && __any_sync(0xffffffffu, alpha != 1.f)) {  // O holds PV of earlier halves
-              // every PV issued so far must have landed: the last one is PV(u-1), whose commit frees its S buffer.
-              // That barrier is at most one phase behind here (QK(u) was issued after PV(u-6), hence PV(u-7), was
-              // done), so the parity wait is unambiguous -- a single per-half "PV done" barrier can lag by several.
-              PROF_WAIT(3, bar(B_SFREE + (u - 1) % NSBUF), ((u - 1) / NSBUF) & 1);
-              tc::tc_fence_after();
+        PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
+        PROF_SPAN_BEGIN();
+        if (wq == 0) TRACE(g, 2);
+        tc::tc_fence_after();
+        const int tile0 = j * TILE_N;
+        const bool masked = tile0 + TILE_N > P;  // the tile touches tree positions or the ragged end
+        uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
+        if (masked) {
 #pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                uint32_t o[32];
-                tc::tmem_ld32(tO + c * 32, o);
-                tc::tmem_wait_ld();
-                tc::reg_fence32(o);
-#pragma unroll
-                for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-                tc::tmem_st32(tO + c * 32, o);
-              }
-              tc::tmem_wait_st();
-            }
-            const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-            half_weights<true>(tS, vis, p.scale_log2, -m_eff, ts, tr);
+          for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tile0 + 32 * c);
+        }
+        float ts = 0.f, tr = 0.f;  // this tile's exact weight sum / share of the normaliser
+        if (!safe && !masked) {
+          tile_weights_fast(tS, p.scale_log2, 0.f, ts);
+          tr = ts;
+        } else if (!safe) {
+          tile_weights_masked(tS, vis, p.scale_log2, 0.f, ts, tr);
+        } else {
+          // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same path:
+          // the TMEM instructions are warp-wide)
+          const float mx = row_max_pass(tS, vis);
+          const float m_new = fmaxf(m_used, mx * p.scale_log2);
+          float alpha = 1.f;
+          if (m_new > m_used) {
+            alpha = (m_used == -INFINITY) ? 0.f : tc::ex2(m_used - m_new);
+            m_used = m_new;
           }
-          lsum += ts;
-          lnorm += tr;
-          tc::tmem_wait_st();
-          if (tok0 + HALF_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
-            const int slot = g % NSTAGE;
-            PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
-            // the warpgroup's 128 threads clear the 64 token rows of this half, thread = (d-half, token)
-            const int t_loc = row & 63, dh = row >> 6, tok = h * HALF_N + t_loc;
-            if (tok0 + t_loc >= total) {
-              uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (tok >> 3) * GROUP_BYTES + dh * 1024 +
-                                                 (tok & 7) * 128);
+          lsum *= alpha;
+          lnorm *= alpha;
+          if (g > g_first && __any_sync(0xffffffffu, alpha != 1.f)) {  // O holds PV of earlier tiles
+            // every PV issued so far must have landed: the last one is PV(g-1), whose commit frees its S buffer.  That
+            // barrier is at most one phase behind here (QK(g) was issued after PV(g-3), hence PV(g-4), was done), so
+            // the parity wait is unambiguous -- one shared "PV done" barrier can lag by two phases and let O be
+            // rescaled under a running PV.
+            PROF_WAIT(3, bar(B_SFREE + (g - 1) % NSBUF), ((g - 1) / NSBUF) & 1);
+            tc::tc_fence_after();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint32_t o[32];
+              tc::tmem_ld32(tO + c * 32, o);
+              tc::tmem_wait_ld();
+              tc::reg_fence32(o);
+#pragma unroll
+              for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+              tc::tmem_st32(tO + c * 32, o);
+            }
+            tc::tmem_wait_st();
+          }
+          const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
+          tile_weights_masked(tS, vis, p.scale_log2, -m_eff, ts, tr);
+        }
+        lsum += ts;
+        lnorm += tr;
+        tc::tmem_wait_st();
+        if (tile0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
+          const int slot = g % NSTAGE;
+          PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
+          if (row >= total - tile0) {  // both d-halves of V row `row`
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              uint4* z = reinterpret_cast<uint4*>(gen_base + SMEM_V + slot * TILE_BYTES + (row >> 3) * GROUP_BYTES + h * 1024 +
+                                                 (row & 7) * 128);
 #pragma unroll
               for (int e = 0; e < 8; ++e) z[e] = make_uint4(0u, 0u, 0u, 0u);
             }
-            tc::fence_proxy_async();
           }
-          tc::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
-          if (wq == 0) TRACE(u, 3);
-          PROF_SPAN_END(5);
-          PROF_COUNT(6);
-#ifdef ECHO_WAIT_PROF
-          gap_t_ = clock64();
-#endif
+          tc::fence_proxy_async();
         }
+        tc::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(bar(B_PFULL + b));
+        if (wq == 0) TRACE(g, 3);
+        PROF_SPAN_END(5);
+        PROF_COUNT(6);
+#ifdef ECHO_WAIT_PROF
+        gap_t_ = clock64();
+#endif
       }
+      g = g_end;
       // ---- publish this warpgroup's sums (and warpgroup 0's reference) for the epilogue ----
       PROF_SPAN2_BEGIN();
       PROF_WAIT(2, bar(B_STATFREE), (itc & 1) ^ 1);  // the epilogue has read the statistics of the previous item
@@ -682,29 +737,39 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       PROF_SPAN2_END(3);
       ++itc;
     };
-    // Phase 0: item records are fetched two items ahead and the row's ancestor mask one item ahead, so that no
-    // global-load latency sits between the last tile of one item and the first tile of the next.
-    {
-      const int4 zero4 = make_int4(0, 0, 0, 0);
-      int4 a0 = zero4, a1 = zero4, b0 = zero4, b1 = zero4;  // records of the next item (a) and the one after (b)
-      uint4 mk_next = make_uint4(0u, 0u, 0u, 0u);
-      bool more = item_index(0, cta, grid) < n_items;
-      if (more) { a0 = p.items[2 * item_index(0, cta, grid)]; a1 = p.items[2 * item_index(0, cta, grid) + 1]; }
-      if (item_index(1, cta, grid) < n_items) { b0 = p.items[2 * item_index(1, cta, grid)]; b1 = p.items[2 * item_index(1, cta, grid) + 1]; }
-      if (more) mk_next = row_mask(a0, a1);
-      for (int k = 0; more; ++k) {
-        const Item it = decode(a0, a1);
-        const uint4 mk = mk_next;
-        more = item_index(k + 1, cta, grid) < n_items;
-        a0 = b0; a1 = b1;
-        if (item_index(k + 2, cta, grid) < n_items) { b0 = p.items[2 * item_index(k + 2, cta, grid)]; b1 = p.items[2 * item_index(k + 2, cta, grid) + 1]; }
-        if (more) mk_next = row_mask(a0, a1);
-        do_item(it, mk, force_safe || k >= REDO_CAP);
+    // Records come from the lane-distributed feed; the rows' ancestor masks likewise: the 32 rows of a warp belong to
+    // npw = 32 / G nodes, so the 32 lanes hold the masks of `slots` = 32 / npw consecutive items (lane = slot * npw +
+    // node), fetched together every `slots` items -- one exposed load latency per block instead of one per item.
+    ItemFeed feed;
+    feed.init();
+    const int npw = p.log2G < 5 ? (32 >> p.log2G) : 1, slots = 32 / npw;
+    uint4 mblk = make_uint4(0u, 0u, 0u, 0u);
+    int mblk_k0 = -(1 << 30);
+    auto item_mask = [&](int k, bool stream) -> uint4 {
+      if (!stream) {  // redo phase: items come out of order, one load per item
+        const Item t = feed.get(p.items, k, cta, grid, n_items, lane);
+        const int l = (t.rt * TILE_M + row) >> p.log2G;
+        return l < t.Ki ? p.anc_mask[t.off + l] : make_uint4(0u, 0u, 0u, 0u);
       }
-    }
-    redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) {
-      const int4 r0 = p.items[2 * idx], r1 = p.items[2 * idx + 1];
-      do_item(decode(r0, r1), row_mask(r0, r1), true);
+      if (k - mblk_k0 >= slots) {  // warp-uniform
+        mblk_k0 = k - (k % slots);
+        const int kk = mblk_k0 + lane / npw;  // same 32-block as k: slots divides 32
+        feed.ensure(p.items, k, cta, grid, n_items, lane);
+        const int rt = (__shfl_sync(0xffffffffu, feed.r0.y, kk & 31) >> 8) & 0xff;
+        const int off = __shfl_sync(0xffffffffu, feed.r1.y, kk & 31), Ki = __shfl_sync(0xffffffffu, feed.r1.z, kk & 31);
+        const int l = ((rt * TILE_M + wq * 32) >> p.log2G) + lane % npw;
+        mblk = l < Ki ? p.anc_mask[off + l] : make_uint4(0u, 0u, 0u, 0u);
+      }
+      const int src = (k - mblk_k0) * npw + (p.log2G < 5 ? (lane >> p.log2G) : 0);
+      uint4 m;
+      m.x = __shfl_sync(0xffffffffu, mblk.x, src); m.y = __shfl_sync(0xffffffffu, mblk.y, src);
+      m.z = __shfl_sync(0xffffffffu, mblk.z, src); m.w = __shfl_sync(0xffffffffu, mblk.w, src);
+      return m;
+    };
+    walk_items(cta, grid, n_items, force_safe, redo, bar(B_PHASE), []() {}, [&](int k, int ph, bool safe) {
+      const Item it = feed.get(p.items, k, cta, grid, n_items, lane);
+      const uint4 mk = item_mask(k, ph == 0);
+      do_item(it, mk, safe);
     });
     PROF_ADD(0);
     if ((warp & 3) == 0 && lane == 0) PROF_FLUSH(16 + 8 * wg, 7);
@@ -719,8 +784,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     int itc = 0;
     PROF_DECL(3);
     PROF_T0();
-    auto finish = [&](int idx, int k, bool safe) {
-      const Item it = load_item(p.items, idx);
+    ItemFeed feed;
+    feed.init();
+    auto finish = [&](int k, int, bool safe) {
+      const Item it = feed.get(p.items, k, cta, grid, n_items, lane);
       const int r_glob = it.rt * TILE_M + row;
       const int l = r_glob >> p.log2G, gq = r_glob & (p.G - 1);
       const bool valid = l < it.Ki;
@@ -780,13 +847,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       tc::mbar_arrive(bar(B_OFREE));
       ++itc;
     };
-    for (int k = 0;; ++k) {
-      const int idx = item_index(k, cta, grid);
-      if (idx >= n_items) break;
-      finish(idx, k, force_safe || k >= REDO_CAP);
-    }
-    tc::mbar_arrive(bar(B_PHASE));  // the bitmap is final (release); every role, this one included, now reads it
-    redo_phase(cta, grid, n_items, redo, bar(B_PHASE), [&](int idx, bool) { finish(idx, 0, true); });
+    // between the phases: the bitmap is final (release); every role, this one included, then reads it
+    walk_items(cta, grid, n_items, force_safe, redo, bar(B_PHASE), [&]() { tc::mbar_arrive(bar(B_PHASE)); }, finish);
     PROF_ADD(0);
     if (warp == W_EPI && lane == 0) PROF_FLUSH(12, 3);
   }
