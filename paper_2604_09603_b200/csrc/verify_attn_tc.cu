@@ -433,11 +433,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
     // A page (16 tokens x 128 d of one KV head, 4 KB contiguous in the pool) is one 4-D box {64 d, 8 tokens, 2 d-halves,
     // 2 token groups}; a 128-token tile is eight of them, their ids read from the page table by lanes 0-7 one tile
     // ahead.  All 32 lanes walk the loop (same addresses, same values: every TMA operand is provably warp-uniform),
-    // one elected lane issues.  The Q tile belongs to the V warp, so that the K tiles of the next item are requested
-    // without waiting for the last QK^T of this one to release Q.
+    // one elected lane issues.  (The Q tile is loaded by the QK^T issuer itself.)
     {
       const bool is_k = warp == W_PROD_K;
-      const bool loads_q = !is_k;
       const uint32_t s_dst = is_k ? sK : sV;
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
@@ -461,29 +459,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       };
       int cur = 0;            // page ids of the tile about to be issued, fetched one tile ahead -- across items too
       bool cur_valid = false;
-      // `ahead`: the item after this one in the list (phase 0), whose first tile's page ids and Q tile are requested
-      // before this item ends, or nullptr
+      // `ahead`: the item after this one in the list (phase 0), whose first tile's page ids are requested before this
+      // item ends, or nullptr
       auto produce = [&](const Item& it, const Item* ahead) {
         const int total = it.P + it.Ki;
-        if (loads_q) {
-          PROF_WAIT_BACKOFF(2, bar(B_QEMPTY), (itc & 1) ^ 1);
-          const int node0 = it.off + it.rt * (TILE_M >> p.log2G);
-          if (tc::elect_one()) {
-            tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
-            tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, it.kvh * p.G, node0);
-            tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, it.kvh * p.G, node0);
-          }
-          __syncwarp();
-          TRACE(g, 6);
-          if (ahead && ahead->jt1 > ahead->jt0) {  // the next item's Q tile into L2 while this item runs
-            const int node1 = ahead->off + ahead->rt * (TILE_M >> p.log2G);
-            if (tc::elect_one()) {
-              tc::tma_prefetch_3d(&tmap_q, 0, ahead->kvh * p.G, node1);
-              tc::tma_prefetch_3d(&tmap_q, 64, ahead->kvh * p.G, node1);
-            }
-            __syncwarp();
-          }
-        }
         if ((total + PAGE - 1) / PAGE > p.max_pages && is_k && lane == 0)
           atomicOr(p.status, ECHO_DEV_PAGE_OVERFLOW);  // page table too short: flag, load what exists
         const int npages = n_pages(it);
@@ -541,12 +520,40 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const uint64_t qdesc = tc::smem_desc_sw128(sQ, 16, 1024);
       ItemFeed feed;
       feed.init();
-      auto issue = [&](int k, int, bool) {
+      // This warp also loads the Q tile: it is the one that knows when the last QK^T of the previous item has read
+      // it (its own commit), so the load goes out the moment the buffer is free instead of when a producer warp gets
+      // there (1300 cycles later on average); and three tiles before an item ends it pulls the next item's Q tile
+      // into L2, which turns the 2600-cycle load at the boundary into an L2 hit (a prefetch a whole item ahead is
+      // evicted again: the KV stream turns the L2 over every ~20 us).
+      auto q_coords = [&](const Item& t, int& h0, int& node0) {
+        h0 = tc::uniform(t.kvh) * p.G;
+        node0 = tc::uniform(t.off) + tc::uniform(t.rt) * (TILE_M >> p.log2G);
+      };
+      auto issue = [&](int k, int ph, bool) {
         const Item rec = feed.get(p.items, k, cta, grid, n_items, lane);
         const int n = tc::uniform(rec.jt1 - rec.jt0);
+        int h0, node0;
+        q_coords(rec, h0, node0);
+        PROF_WAIT(3, bar(B_QEMPTY), (itc & 1) ^ 1);
+        if (tc::elect_one()) {
+          tc::mbar_expect_tx(bar(B_QFULL), TILE_BYTES);
+          tc::tma_load_3d(sQ, &tmap_q, bar(B_QFULL), 0, h0, node0);
+          tc::tma_load_3d(sQ + HALF_BYTES, &tmap_q, bar(B_QFULL), 64, h0, node0);
+        }
+        __syncwarp();
+        const bool more = ph == 0 && item_index(k + 1, cta, grid) < n_items;
+        int h1 = 0, node1 = 0;
+        if (more) q_coords(feed.get(p.items, k + 1, cta, grid, n_items, lane), h1, node1);
         PROF_WAIT(3, bar(B_QFULL), itc & 1);
         TRACE(g, 7);
         for (int j = 0; j < n; ++j, ++g) {
+          if (more && j == max(0, n - 4)) {
+            if (tc::elect_one()) {
+              tc::tma_prefetch_3d(&tmap_q, 0, h1, node1);
+              tc::tma_prefetch_3d(&tmap_q, 64, h1, node1);
+            }
+            __syncwarp();
+          }
           const int slot = g % NSTAGE;
           PROF_WAIT(1, bar(B_KFULL + slot), (g / NSTAGE) & 1);
           const int b = g % NSBUF;
