@@ -36,67 +36,79 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def tensor_peak():
+def tensor_peak(sustained=False):
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
+        if sustained and "bf16_tflops_sustained" in d:
+            return float(d["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json bf16_tflops_sustained)"
         if "bf16_tflops" in d:
             return float(d["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
-    return 2250.0, "fallback (B200_PROFILING.md nominal dense bf16)"
+    return (1400.0, "fallback (B200_PROFILING.md, sustained)") if sustained else (1590.0, "fallback (B200_PROFILING.md, burst)")
 
 
-class ClockSampler(threading.Thread):
-    """samples SM clock, power and throttle reasons during the timed region: NVML every 2 ms when pynvml is there
-    (the default run lasts ~15 ms), else nvidia-smi every 100 ms"""
+class ClockSampler:
+    """nvidia-smi in loop mode (-lms 20) for the whole measurement: SM clock, power and throttle reasons every 20 ms.
+    The SM clock UNDER the kernels comes from the library's probe kernel (echo_probe_sm_clock): the verify step is
+    shorter than any NVML sampling period and NVML reads the idle clock between kernels."""
 
     NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, idx=0):
-        super().__init__(daemon=True)
-        self.idx, self.stop_flag, self.rows, self.power = idx, False, [], []
+        self.idx, self.proc, self.marks = idx, None, {}
 
-    def _run_nvml(self):
-        import pynvml
-        pynvml.nvmlInit()
-        h = pynvml.nvmlDeviceGetHandleByIndex(self.idx)
-        mx = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
-        bits = [pynvml.nvmlClocksThrottleReasonHwSlowdown, pynvml.nvmlClocksThrottleReasonHwThermalSlowdown,
-                pynvml.nvmlClocksThrottleReasonSwThermalSlowdown, pynvml.nvmlClocksThrottleReasonSwPowerCap]
-        while not self.stop_flag:
-            r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
-            self.rows.append([str(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)), str(mx)] +
-                             ["Active" if r & b else "Not Active" for b in bits])
-            self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
-            time.sleep(0.002)
-
-    def run(self):
+    def start(self):
         try:
-            self._run_nvml()
-            return
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t0 = time.time()
         except Exception:
-            pass
-        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
-        while not self.stop_flag:
-            try:
-                o = subprocess.run(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={q}", "--format=csv,noheader,nounits"],
-                                   capture_output=True, text=True, timeout=5).stdout.strip()
-                if o:
-                    self.rows.append([x.strip() for x in o.split(",")])
-            except Exception:
-                pass
-            time.sleep(0.1)
+            self.proc = None
 
-    def summary(self):
-        if not self.rows:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
-        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
-        reasons = [n for i, n in enumerate(self.NAMES) if any(len(r) > 2 + i and r[2 + i] == "Active" for r in self.rows)]
-        out = {"sm_mhz": sm[len(sm) // 2] if sm else None,
-               "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None, "reasons": reasons,
-               "samples": len(self.rows)}
-        if self.power:
-            out["power_w_max"] = max(self.power)
+    def mark(self, name):
+        self.marks[name] = time.time()
+
+    def stop(self):
+        rows = []
+        if self.proc is not None:
+            time.sleep(0.05)
+            self.proc.terminate()
+            try:
+                out, _ = self.proc.communicate(timeout=5)
+            except Exception:
+                self.proc.kill()
+                out = ""
+            rows = [[x.strip() for x in ln.split(",")] for ln in out.splitlines() if ln.count(",") >= 6]
+        self.rows, self.t1 = rows, time.time()
+        return rows
+
+    def window(self, a, b):
+        """rows sampled between the marks a and b (samples are evenly spaced over the run: -lms has no timestamps)"""
+        if not self.rows or a not in self.marks or b not in self.marks:
+            return []
+        n, span = len(self.rows), max(1e-6, self.t1 - self.t0)
+        i0 = int(n * (self.marks[a] - self.t0) / span)
+        i1 = int(np.ceil(n * (self.marks[b] - self.t0) / span))
+        return self.rows[max(0, i0):max(i0 + 1, min(n, i1))]
+
+    def summary(self, rows, probe_mhz):
+        """`clocks` object: sm_mhz = the probe kernel's median (the clock the kernels ran at), NVML's view beside it"""
+        out = {"sm_mhz": float(np.median(probe_mhz)) if len(probe_mhz) else None, "sm_mhz_source":
+               "echo_probe_sm_clock (clock64 / globaltimer in a kernel queued inside the measured region)",
+               "sm_max_mhz": None, "reasons": [], "nvml_samples": len(rows)}
+        allrows = rows or getattr(self, "rows", [])
+        if allrows:
+            mx = [int(float(r[1])) for r in allrows if r[1].replace(".", "").isdigit()]
+            out["sm_max_mhz"] = mx[0] if mx else None
+        if rows:
+            sm = sorted(int(float(r[0])) for r in rows if r[0].replace(".", "").isdigit())
+            out["nvml_sm_mhz"] = sm[len(sm) // 2] if sm else None
+            pw = [float(r[2]) for r in rows if r[2].replace(".", "").isdigit()]
+            out["power_w_max"] = max(pw) if pw else None
+            out["reasons"] = [n for i, n in enumerate(self.NAMES) if any(r[3 + i] == "Active" for r in rows)]
         return out
 
 
@@ -173,6 +185,155 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+class Case:
+    """One workload resident on the device and its step (echo_gate_select -> echo_verify_attn -> echo_accept)."""
+
+    def __init__(self, ctx, echo, sharding, W, torch, dev, cfg, rank=0, world=1, static=False, gating="sparse",
+                 schedule="topb", heads=False, global_budget=False, temperature=0.0, attn_path=0, splits=0, dist=None,
+                 kv_pools=1):
+        self.ctx, self.torch, self.dev, self.cfg, self.static = ctx, torch, dev, cfg, static
+        self.world, self.rank, self.heads, self.dist = world, rank, heads, dist
+        wl = sharding.rank_workload(cfg, 0 if heads else rank, static=static, gated=not static)
+        if gating != "sparse" and not static:
+            wl.gate = wl.gate.ablation(gating)
+        self.wl, g = wl, wl.gate
+        self.schedule = {"topb": echo.SCHED_TOPB, "alg1": echo.SCHED_ALG1}[schedule]
+        cap = self.cap = wl.capacity()
+        ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq, wl.Hkv)
+        ctx.set_option(echo.OPT_ATTN_PATH, attn_path)
+        ctx.set_option(echo.OPT_FORCE_SPLITS, splits)
+        d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        self.h_in = {"cand_offsets": pin(wl.cand_offsets), "parent": pin(wl.parent), "logq": pin(wl.logq),
+                     "prev": pin(wl.prev_token)}
+        self.d_in = {k: v.to(dev) for k, v in self.h_in.items()}
+        q, k, v = W.draw_qkv(wl, cap, device=str(dev))
+        if heads:
+            q, k, v = sharding.shard_attention_inputs(q, k, v, rank, world)
+        self.q = q
+        pt, pl = d(wl.page_table), d(wl.prefix_len)
+        # a working set near the L2 size (cfg1: 189 MB) is measured over >= 4 KV pools taken in turn, so that every
+        # step streams its KV from HBM (SURVEY 8(d)); the copies hold the same values
+        self.kvs = [echo.PagedKV(k, v, pt, pl)] + [echo.PagedKV(k.clone(), v.clone(), pt, pl) for _ in range(kv_pools - 1)]
+        self.sel = ctx.alloc_selection(wl.R, wl.N, cap)
+        self.acc = ctx.alloc_accept(wl.R, cap)
+        self.out = torch.zeros_like(q)
+        self.lse = torch.zeros(cap, q.shape[1], dtype=torch.float32, device=dev)
+        self.global_budget = global_budget and not heads
+        self.g_global, self.gb_bufs = g.replace(budget=g.budget * world), {}
+        self.all_sizes = sharding.exchange_sizes(wl.N, wl.R, world, dist) if self.global_budget else None
+        self.sharding, self.echo = sharding, echo
+        self.gate(self.d_in)
+        sel_h = self.sel_h = self.sel.to_host()
+        self.n_sel = sel_h["n_selected"]
+        glob = (wl.cand_offsets[sel_h["sel_req"]] + sel_h["sel_node"]).astype(np.int64)
+        pad = lambda a: np.concatenate([a, np.zeros(cap - len(a), a.dtype)]).astype(np.int32)
+        self.h_in["draft"] = pin(pad(wl.draft_token[glob]))
+        self.h_in["target"] = pin(pad(wl.target_after[glob]))
+        self.d_in["draft"], self.d_in["target"] = self.h_in["draft"].to(dev), self.h_in["target"].to(dev)
+        self.logits = self.root_logits = self.u_acc = self.u_bon = None
+        self.temperature = temperature
+        if cfg == 4:
+            lg = W.draw_logits(wl, glob, device=str(dev))
+            if lg.shape[0] < cap:
+                lg = torch.cat([lg, torch.zeros(cap - lg.shape[0], lg.shape[1], dtype=lg.dtype, device=dev)])
+            self.logits = lg
+            if temperature > 0:  # acceptance at temperature > 0 (NEXT-2) instead of the argmax
+                gen = torch.Generator(device=dev).manual_seed(W.SEED_BASE + 7)
+                rl = torch.randn(wl.R, lg.shape[1], generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
+                rl[torch.arange(wl.R, device=dev), d(wl.prev_token).long()] += 8.0
+                self.root_logits = rl
+                self.u_acc = torch.rand(cap, generator=gen, device=dev)
+                self.u_bon = torch.rand(wl.R, generator=gen, device=dev)
+        self.bytes_alg, self.flops_alg = algorithmic_bytes(wl, sel_h)
+        if heads:
+            self.bytes_alg, self.flops_alg = self.bytes_alg // world, self.flops_alg // world
+        self.steps_done = 0
+
+    def gate(self, din, sel_=None):
+        wl, g, ctx = self.wl, self.wl.gate, self.ctx
+        if self.global_budget:  # one budget of world x B over the ranks' requests: the one exchange of the path
+            return self.sharding.global_budget_gate_select(ctx, self.rank, self.world, din["cand_offsets"], din["parent"],
+                                                           din["logq"], self.g_global, sel_ or self.sel,
+                                                           max_cand=wl.max_cand, schedule=self.schedule, dist=self.dist,
+                                                           all_sizes=self.all_sizes, bufs=self.gb_bufs)
+        return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max, g.budget,
+                               g.static_k, capacity=self.cap, max_cand=wl.max_cand, out=sel_ or self.sel,
+                               schedule=self.schedule)
+
+    def step(self, din=None, ev=None, qq=None, bufs=None):
+        """one pass of the hot path; ev = (gate0, gate1/attn0, attn1, acc1) CUDA events to record, or None"""
+        din = din or self.d_in
+        sel_, acc_, out_, lse_ = bufs or (self.sel, self.acc, self.out, self.lse)
+        kv = self.kvs[self.steps_done % len(self.kvs)]
+        self.steps_done += 1
+        ctx, wl = self.ctx, self.wl
+        if ev:
+            ev[0].record()
+        self.gate(din, sel_)
+        if ev:
+            ev[1].record()
+        ctx.verify_attn(sel_, kv, self.q if qq is None else qq, SM_SCALE, out=out_, lse=lse_)
+        if ev:
+            ev[2].record()
+        if self.logits is not None and self.temperature > 0:
+            ctx.accept_stochastic(sel_, kv, din["draft"], self.logits, self.root_logits, wl.vocab, self.temperature,
+                                  self.u_acc, self.u_bon, out=acc_)
+        elif self.logits is not None:
+            ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=self.logits, vocab=wl.vocab, out=acc_)
+        else:
+            ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=din["target"], out=acc_)
+        if ev:
+            ev[3].record()
+
+    def roofline(self, attn_ms, sustained=False):
+        """attention against the roof that bounds it: measured HBM copy peak, or the measured bf16 matmul peak when the
+        workload's FLOP per byte is above the ridge of the two (the static-60 run)"""
+        peak, peak_src = peaks()
+        tpeak, tpeak_src = tensor_peak(sustained)
+        tensor_bound = self.flops_alg / self.bytes_alg > tensor_peak(False)[0] * 1e12 / (peak * 1e9)
+        gbs = self.bytes_alg / (attn_ms * 1e-3) / 1e9
+        tfl = self.flops_alg / (attn_ms * 1e-3) / 1e12
+        return {"bound": "tensor" if tensor_bound else "hbm", "achieved": tfl if tensor_bound else gbs,
+                "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",
+                "frac": tfl / tpeak if tensor_bound else gbs / peak, "peak_source": tpeak_src if tensor_bound else peak_src,
+                "attn_ms": attn_ms, "bytes_per_launch": self.bytes_alg, "flops_per_launch": self.flops_alg}
+
+
+def timed_steps(case, steps, warmup, barrier, probe_every=0):
+    """`warmup` untimed steps, then exactly `steps` steps between two events; per-step gate / attention / acceptance
+    events; SM clock probes (outside the per-call events) before, every `probe_every` steps, and after.
+    Returns dict(ms, attn, gate, acc lists, probe MHz list, launches)."""
+    torch, ctx = case.torch, case.ctx
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    evs = [(ev(), ev(), ev(), ev()) for _ in range(steps)]
+    n_probe = 2 + (steps // probe_every if probe_every else 0)
+    probes = torch.zeros(n_probe + 1, dtype=torch.float32, device=case.dev)
+    for _ in range(warmup):
+        case.step()
+    barrier()
+    l0 = ctx.launch_count()
+    e0, e1 = ev(), ev()
+    pi = 0
+    ctx.probe_sm_clock(probes[pi:pi + 1]); pi += 1        # clock state going in (20 us, ahead of the timed region)
+    e0.record()
+    for i in range(steps):
+        case.step(ev=evs[i])
+        if probe_every and (i + 1) % probe_every == 0 and i + 1 < steps:
+            ctx.probe_sm_clock(probes[pi:pi + 1]); pi += 1
+    e1.record()
+    ctx.probe_sm_clock(probes[pi:pi + 1]); pi += 1        # and coming out, with no idle gap in between
+    l1 = ctx.launch_count()
+    barrier()
+    attn = [a[1].elapsed_time(a[2]) for a in evs]
+    gate = [a[0].elapsed_time(a[1]) for a in evs]
+    acc = [a[2].elapsed_time(a[3]) for a in evs]
+    mhz = probes[:pi].cpu().numpy().tolist()
+    # the probes inside a long leg take 20 us each: not part of any per-call time, but inside e0..e1
+    ms = e0.elapsed_time(e1) - 0.02 * max(0, pi - 2)
+    return dict(ms=ms, attn=attn, gate=gate, acc=acc, mhz=mhz[1:] if len(mhz) > 1 else mhz, launches=l1 - l0 - pi)
+
+
 def run_gpu(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -184,122 +345,70 @@ def run_gpu(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=dev)
     build.build_library()
     heads = args.shard == "heads" and world > 1
-    # requests: every rank its own batch (weak scaling); heads: every rank the KV heads [r Hkv/W, (r+1) Hkv/W) of
-    # the same batch (strong scaling, no collective either: attention is independent per KV head)
-    wl = sharding.rank_workload(args.config, 0 if heads else rank, static=args.static, gated=not args.static)
-    if args.gating != "sparse" and not args.static:
-        wl.gate = wl.gate.ablation(args.gating)
-    g = wl.gate
-    schedule = {"topb": echo.SCHED_TOPB, "alg1": echo.SCHED_ALG1}[args.schedule]
-    cap = wl.capacity()
     ctx = echo.EchoContext(local_rank, 0)
-    ctx.ensure_workspace(wl.R, wl.N, cap, wl.Hq, wl.Hkv)
-    if args.attn_path:
-        ctx.set_option(echo.OPT_ATTN_PATH, args.attn_path)
-    if args.splits:
-        ctx.set_option(echo.OPT_FORCE_SPLITS, args.splits)
-    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-
-    h_in = {"cand_offsets": pin(wl.cand_offsets), "parent": pin(wl.parent), "logq": pin(wl.logq),
-            "prev": pin(wl.prev_token)}
-    d_in = {k: v.to(dev) for k, v in h_in.items()}
-    q, k, v = W.draw_qkv(wl, cap, device=str(dev))
-    if heads:
-        q, k, v = sharding.shard_attention_inputs(q, k, v, rank, world)
-    kv = echo.PagedKV(k, v, d(wl.page_table), d(wl.prefix_len))
-    sel = ctx.alloc_selection(wl.R, wl.N, cap)
-    acc = ctx.alloc_accept(wl.R, cap)
-    out = torch.zeros_like(q)
-    lse = torch.zeros(cap, q.shape[1], dtype=torch.float32, device=dev)
-
-    g_global, gb_bufs = g.replace(budget=g.budget * world), {}
-    all_sizes = sharding.exchange_sizes(wl.N, wl.R, world, dist) if args.global_budget else None
-
-    def gate(din, sel_=None):
-        if args.global_budget and not heads:  # one budget of world x B over the ranks' requests: the one exchange of the path
-            return sharding.global_budget_gate_select(ctx, rank, world, din["cand_offsets"], din["parent"], din["logq"],
-                                                      g_global, sel_ or sel, max_cand=wl.max_cand, schedule=schedule,
-                                                      dist=dist, all_sizes=all_sizes, bufs=gb_bufs)
-        return ctx.gate_select(din["cand_offsets"], din["parent"], din["logq"], g.depth_mask, g.log_tau, g.w_max,
-                               g.budget, g.static_k, capacity=cap, max_cand=wl.max_cand, out=sel_ or sel,
-                               schedule=schedule)
-
-    gate(d_in)
-    sel_h = sel.to_host()
-    n_sel = sel_h["n_selected"]
-    glob = (wl.cand_offsets[sel_h["sel_req"]] + sel_h["sel_node"]).astype(np.int64)
-    pad = lambda a: np.concatenate([a, np.zeros(cap - len(a), a.dtype)]).astype(np.int32)
-    h_in["draft"] = pin(pad(wl.draft_token[glob]))
-    h_in["target"] = pin(pad(wl.target_after[glob]))
-    d_in["draft"], d_in["target"] = h_in["draft"].to(dev), h_in["target"].to(dev)
-    logits = None
-    if args.config == 4:
-        logits = W.draw_logits(wl, glob, device=str(dev))
-        if logits.shape[0] < cap:
-            logits = torch.cat([logits, torch.zeros(cap - logits.shape[0], logits.shape[1], dtype=logits.dtype, device=dev)])
-    root_logits = u_acc = u_bon = None
-    if logits is not None and args.temperature > 0:  # acceptance at temperature > 0 (NEXT-2) instead of the argmax
-        gen = torch.Generator(device=dev).manual_seed(W.SEED_BASE + 7)
-        root_logits = torch.randn(wl.R, logits.shape[1], generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
-        root_logits[torch.arange(wl.R, device=dev), d(wl.prev_token).long()] += 8.0
-        u_acc = torch.rand(cap, generator=gen, device=dev)
-        u_bon = torch.rand(wl.R, generator=gen, device=dev)
-    bytes_alg, flops_alg = algorithmic_bytes(wl, sel_h)
-    if heads:
-        bytes_alg, flops_alg = bytes_alg // world, flops_alg // world
-
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-    attn_ev = [(ev(), ev()) for _ in range(args.steps)]
-    gate_ev = [(ev(), ev()) for _ in range(args.steps)]
-    acc_ev = [ev() for _ in range(args.steps)]
-
-    def step(din, i=None, qq=q, bufs=None):
-        sel_, acc_, out_, lse_ = bufs or (sel, acc, out, lse)
-        if i is not None:
-            gate_ev[i][0].record()
-        gate(din, sel_)
-        if i is not None:
-            gate_ev[i][1].record(); attn_ev[i][0].record()
-        ctx.verify_attn(sel_, kv, qq, SM_SCALE, out=out_, lse=lse_)
-        if i is not None:
-            attn_ev[i][1].record()
-        if logits is not None and args.temperature > 0:
-            ctx.accept_stochastic(sel_, kv, din["draft"], logits, root_logits, wl.vocab, args.temperature, u_acc, u_bon,
-                                  out=acc_)
-        elif logits is not None:
-            ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=logits, vocab=wl.vocab, out=acc_)
-        else:
-            ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=din["target"], out=acc_)
-        if i is not None:
-            acc_ev[i].record()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step(d_in)
+    mk = lambda cfg, static=False, **kw: Case(ctx, echo, sharding, W, torch, dev, cfg, rank=rank, world=world, static=static,
+                                              dist=dist, **kw)
+    case = mk(args.config, args.static, gating=args.gating, schedule=args.schedule, heads=heads,
+              global_budget=args.global_budget, temperature=args.temperature, attn_path=args.attn_path,
+              splits=args.splits, kv_pools=4 if args.config == 1 else 1)
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    barrier()
-    e0, e1 = ev(), ev()
-    e0.record()
-    for i in range(args.steps):
-        step(d_in, i)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    sampler.stop_flag = True
-    t_attn = float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
-    t_gate = float(np.mean([a.elapsed_time(b) for a, b in gate_ev]))
-    t_acc = float(np.mean([attn_ev[i][1].elapsed_time(acc_ev[i]) for i in range(args.steps)]))
-    t_attn_min = float(np.min([a.elapsed_time(b) for a, b in attn_ev]))
-    accepted = int(acc.accept_len[:wl.R].sum().item())
+    sampler.mark("burst0")
+    t = timed_steps(case, args.steps, args.warmup, barrier)
+    sampler.mark("burst1")
+    r = dict(torch=torch, dist=dist, dev=dev, ctx=ctx, case=case, wl=case.wl, heads=heads, barrier=barrier, sampler=sampler,
+             ms=t["ms"], t_attn=float(np.mean(t["attn"])), t_attn_min=float(np.min(t["attn"])),
+             t_gate=float(np.mean(t["gate"])), t_acc=float(np.mean(t["acc"])), mhz=t["mhz"], launches=t["launches"],
+             n_sel=case.n_sel, accepted=int(case.acc.accept_len[:case.wl.R].sum().item()), sustained=None, sub={},
+             calib_us=None, draft_us=None)
+    # ---- second leg: the same step back to back for >= --sustained-seconds: the regime a serving loop runs in (the
+    # part reaches its power cap after ~100 ms and the SM clock drops; MEASURED_PEAKS.json keeps a sustained matmul
+    # figure for the same reason)
+    if args.sustained_seconds > 0:
+        n = int(min(20000, max(200, args.sustained_seconds * 1e3 / max(1e-3, t["ms"] / args.steps))))
+        sampler.mark("sus0")
+        ts = timed_steps(case, n, 0, barrier, probe_every=max(1, n // 16))
+        sampler.mark("sus1")
+        tail = ts["attn"][len(ts["attn"]) // 2:]          # second half: the clocks have settled
+        roof = case.roofline(float(np.mean(tail)), sustained=True)
+        roof.update(steps=n, seconds=ts["ms"] * 1e-3, ms_per_step=ts["ms"] / n, sm_mhz=float(np.median(ts["mhz"][len(ts["mhz"]) // 2:])),
+                    attn_ms_first_100=float(np.mean(ts["attn"][:100])),
+                    value=sharding.job_throughput(case.n_sel, n, ts["ms"]))
+        r["sustained"] = roof
+    # ---- the other shapes north_star names, one sub-record each (rank 0's view; not part of `value`)
+    if rank == 0 and args.subrecords and world == 1:
+        for name, cfg, static in (("cfg1", 1, False), ("cfg3", 3, False), ("cfg2_static60", 2, True), ("cfg4", 4, False)):
+            if cfg == args.config and static == args.static:
+                continue
+            try:
+                c = mk(cfg, static, kv_pools=4 if cfg == 1 else 1)
+                tt = timed_steps(c, 30 if cfg != 4 else 12, 5, barrier)
+                rec = c.roofline(float(np.mean(tt["attn"])))
+                rec.update(workload=WORKLOADS[cfg] + (" static-60 trees" if static else ""), steps=len(tt["attn"]),
+                           ms_per_step=tt["ms"] / len(tt["attn"]), attn_ms_min=float(np.min(tt["attn"])),
+                           gate_ms=float(np.mean(tt["gate"])), accept_ms=float(np.mean(tt["acc"])),
+                           verified_nodes_per_step=c.n_sel, value=c.n_sel * len(tt["attn"]) / (tt["ms"] * 1e-3),
+                           sm_mhz=float(np.median(tt["mhz"])), kv_pools=len(c.kvs))
+                r["sub"][name] = rec
+                del c
+                torch.cuda.empty_cache()
+            except Exception as e:  # a sub-record must never take the headline number down with it
+                r["sub"][name] = {"error": repr(e)[:200]}
+        # back to the headline case's options (the sub-cases share the context)
+        ctx.set_option(echo.OPT_ATTN_PATH, args.attn_path)
+        ctx.set_option(echo.OPT_FORCE_SPLITS, args.splits)
+        ctx.ensure_workspace(case.wl.R, case.wl.N, case.cap, case.wl.Hq, case.wl.Hkv)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    wl = case.wl
     # the step before the path: warm-up calibration of the gates, timed outside the step
-    calib_us = None
     if rank == 0 and args.calibrate_samples > 0:
         tr = W.draw_calibration_traces(np.random.default_rng(W.SEED_BASE), args.calibrate_samples)
         d_tr = [d(a) for a in tr]
@@ -312,10 +421,8 @@ def run_gpu(args, rank, world, local_rank):
             ctx.calibrate(*d_tr, 0.65)
         c1.record()
         torch.cuda.synchronize()
-        calib_us = c0.elapsed_time(c1) * 100.0
-    # the step on the other side of the path (NEXT-4): the candidate trees built on the device, level by level
-    draft_us = None
-    if rank == 0 and args.calibrate_samples > 0:
+        r["calib_us"] = c0.elapsed_time(c1) * 100.0
+        # the step on the other side of the path (NEXT-4): the candidate trees built on the device, level by level
         rng = np.random.default_rng(W.SEED_BASE + 1)
         Ld, kd = 8, 10
         lv = [W.draw_draft_level(rng, wl.R, 1 if l_ == 0 else kd, kd) for l_ in range(Ld)]
@@ -340,10 +447,9 @@ def run_gpu(args, rank, world, local_rank):
             build_tree()
         c1.record()
         torch.cuda.synchronize()
-        draft_us = c0.elapsed_time(c1) * 100.0
-    return dict(calib_us=calib_us, draft_us=draft_us, heads=heads, t_acc=t_acc, t_attn_min=t_attn_min, torch=torch, dist=dist, wl=wl, ctx=ctx, dev=dev, ms=ms, t_attn=t_attn, t_gate=t_gate, n_sel=n_sel,
-                accepted=accepted, bytes_alg=bytes_alg, flops_alg=flops_alg, step=step, h_in=h_in, d_in=d_in, q=q,
-                out=out, lse=lse, acc=acc, sel=sel, sampler=sampler, barrier=barrier, cap=cap, logits=logits)
+        r["draft_us"] = c0.elapsed_time(c1) * 100.0
+        ctx.ensure_workspace(case.wl.R, case.wl.N, case.cap, case.wl.Hq, case.wl.Hkv)
+    return r
 
 
 def run_e2e(r, args):
@@ -352,16 +458,16 @@ def run_e2e(r, args):
     is resident serving state and is not re-uploaded.  Three streams and two sets of device
     buffers: the upload of step i+1 and the download of step i-1 overlap the kernels of step i (PCIe is full
     duplex); each step still moves all of its own bytes."""
-    torch, dev, ctx, wl = r["torch"], r["dev"], r["ctx"], r["wl"]
-    h_in = r["h_in"]
-    h_q = r["q"].cpu().pin_memory()
+    torch, dev, ctx, case = r["torch"], r["dev"], r["ctx"], r["case"]
+    wl, h_in = case.wl, case.h_in
+    h_q = case.q.cpu().pin_memory()
     sets = []
     for n in range(2):
         d_in = {k_: t.to(dev) for k_, t in h_in.items()}
-        q = torch.empty_like(r["q"])
-        sel = ctx.alloc_selection(wl.R, wl.N, r["cap"])
-        acc = ctx.alloc_accept(wl.R, r["cap"])
-        out, lse = torch.zeros_like(r["out"]), torch.zeros_like(r["lse"])
+        q = torch.empty_like(case.q)
+        sel = ctx.alloc_selection(wl.R, wl.N, case.cap)
+        acc = ctx.alloc_accept(wl.R, case.cap)
+        out, lse = torch.zeros_like(case.out), torch.zeros_like(case.lse)
         outs = [out, lse, acc.accept_len, acc.accept_idx, acc.bonus_token, acc.new_len, sel.n_selected]
         h_outs = [torch.empty_like(t, device="cpu").pin_memory() for t in outs]
         ev = [torch.cuda.Event() for _ in range(3)]  # upload done, kernels done, download done
@@ -382,7 +488,7 @@ def run_e2e(r, args):
         with torch.cuda.stream(s_run):
             s_run.wait_event(up)
             s_run.wait_event(down)        # the results of step i-2 have left this set's output buffers
-            r["step"](st["d_in"], None, st["q"], st["bufs"])
+            case.step(st["d_in"], None, st["q"], st["bufs"])
             run.record(s_run)
         with torch.cuda.stream(s_down):
             s_down.wait_event(run)
@@ -406,7 +512,7 @@ def run_e2e(r, args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=300, help="timed steps of the headline leg (default: ~100 ms at cfg2)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: BS=128)")
     ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
@@ -415,6 +521,10 @@ def main():
     ap.add_argument("--ref-nodes", type=int, default=32, help="--impl reference: packed nodes of oracle attention per step (~0.75 s)")
     ap.add_argument("--baseline-nodes", type=int, default=512, help="cpu_baseline leg: packed nodes of oracle attention (~12 s once)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0,
+                    help="length of the second timed leg (back-to-back steps under the power cap); 0 = skip")
+    ap.add_argument("--no-subrecords", dest="subrecords", action="store_false",
+                    help="skip the per-shape sub-records (cfg1, cfg3, cfg2 static-60, cfg4)")
     ap.add_argument("--schedule", default="topb", choices=["topb", "alg1"],
                     help="topb: global top-B (north_star); alg1: Algorithm 1 as printed (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--gating", default="sparse", choices=["sparse", "dense", "fixed"],
@@ -443,50 +553,48 @@ def main():
         [r["ms"], e2e_dt], [r["n_sel"] / (world if r["heads"] else 1), r["accepted"] / (world if r["heads"] else 1)],
         world, r["dev"], dist)
     if rank == 0:
-        peak, peak_src = peaks()
-        achieved = r["bytes_alg"] / (r["t_attn"] * 1e-3) / 1e9
-        tpeak, tpeak_src = tensor_peak()
-        # the static-60 run has ~400 FLOP per byte, above the ridge of the measured peaks: its roof is the tensor pipe
-        tensor_bound = r["flops_alg"] / r["bytes_alg"] > tpeak * 1e12 / (peak * 1e9)
-        tflops = r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.csv")  # measured DRAM bytes per launch from the ncu --set full capture
-        if os.path.exists(tp):
+        case, wl, sampler = r["case"], r["wl"], r["sampler"]
+        sampler.stop()
+        roof = case.roofline(r["t_attn"])
+        traffic, traffic_src = None, None
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")  # DRAM bytes per launch from the committed ncu --set full capture
+        if os.path.exists(tp) and not args.static:
             for ln in open(tp).read().splitlines()[1:]:
                 f = ln.split(",")
                 if f and f[0] == f"cfg{args.config}":
-                    traffic = int(f[1])
-        wl = r["wl"]
-        units = wl.R * wl.Hkv
-        splits = args.splits or 1
-        if not args.splits:  # the library's split policy (csrc/verify_attn.cu), to count launches
-            sms = torch.cuda.get_device_properties(0).multi_processor_count
-            while splits < 8 and units * splits < sms:
-                splits *= 2
-        launches = 3 + 2 + (1 if splits > 1 else 0) + 1 + (1 if args.config == 4 else 0)  # gate 3, plan + attn, merge, accept, argmax
+                    traffic, traffic_src = int(f[1]), "not measured in this run: " + ",".join(f[3:])
+        splits = int(r["ctx"].lib.echo_attn_splits(r["ctx"]._h, wl.R, wl.Hkv)) if not args.splits else args.splits
+        roofline = {k_: roof[k_] for k_ in ("bound", "achieved", "peak", "unit", "frac")}
+        roofline.update(traffic=traffic, traffic_source=traffic_src, peak_source=roof["peak_source"],
+                        kernel="echo_verify_attn (k_plan + k_verify_attn_tc" + (" + k_lse_merge)" if splits > 1 else ")"),
+                        bytes_per_launch=case.bytes_alg, flops_per_launch=case.flops_alg)
+        cfg_name = (WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
+                    + (" global-budget" if args.global_budget else "")
+                    + (f" temperature={args.temperature}" if args.temperature > 0 and args.config == 4 else "")
+                    + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"))
         line = {"metric": "verified draft tokens/s", "value": sharding.job_throughput(n_sel_all, args.steps, ms), "unit": "tokens/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "strong" if r["heads"] else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": {"workload": WORKLOADS[args.config] + (" static-60 trees" if args.static else "")
-                           + (" global-budget" if args.global_budget else "")
-                           + (f" temperature={args.temperature}" if args.temperature > 0 and args.config == 4 else "") + ("" if args.schedule == "topb" else " schedule=alg1") + ("" if args.gating == "sparse" else f" gating={args.gating}"),
-                           "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
-                           "accepted_per_step": r["accepted"], "l2": "inputs larger than L2 (KV pool >> 126 MB)"
-                           if r["bytes_alg"] > 4e8 else "working set near L2 size: KV not flushed",
+                "config": {"workload": cfg_name, "requests": wl.R, "verified_nodes_per_step": r["n_sel"],
+                           "accepted_per_step": r["accepted"],
+                           "l2": "inputs larger than L2 (KV pool >> 126 MB)" if case.bytes_alg * len(case.kvs) > 4e8
+                           else "working set near L2 size: KV not flushed",
+                           "kv_pools_rotated": len(case.kvs),
                            "attn_ms": r["t_attn"], "attn_ms_min": r["t_attn_min"], "gate_ms": r["t_gate"], "accept_ms": r["t_acc"],
-                           "yield": r["accepted"] / max(1, r["n_sel"]), "attn_flops": r["flops_alg"],
-                           "attn_tflops": r["flops_alg"] / (r["t_attn"] * 1e-3) / 1e12,
+                           "yield": r["accepted"] / max(1, r["n_sel"]), "attn_flops": case.flops_alg,
+                           "attn_tflops": case.flops_alg / (r["t_attn"] * 1e-3) / 1e12,
                            "calibrate_us": r["calib_us"], "calibrate_samples": args.calibrate_samples,
                            "draft_tree_8x10_us": r["draft_us"]},
                 "accepted_tokens_per_s": acc_all * args.steps / (ms * 1e-3),
-                "roofline": {"bound": "tensor" if tensor_bound else "hbm", "achieved": tflops if tensor_bound else achieved,
-                             "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",
-                             "frac": tflops / tpeak if tensor_bound else achieved / peak,
-                             "traffic": None if args.static else traffic, "peak_source": tpeak_src if tensor_bound else peak_src, "kernel": "echo_verify_attn (plan + k_verify_attn_tc"
-                             + (" + k_lse_merge)" if splits > 1 else ")"), "bytes_per_launch": r["bytes_alg"], "flops_per_launch": r["flops_alg"]},
+                "roofline": roofline,
+                "roofline_sustained": r["sustained"],
+                "configs": r["sub"],
                 "e2e": {"value": n_sel_all * args.steps / e2e_dt, "unit": "tokens/s", "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h},
-                "gpu_launches": launches * args.steps, "clocks": r["sampler"].summary()}
+                "gpu_launches": r["launches"],
+                "clocks": sampler.summary(sampler.window("burst0", "burst1"), r["mhz"])}
+        if r["sustained"] is not None:
+            line["clocks_sustained"] = sampler.summary(sampler.window("sus0", "sus1"), [r["sustained"]["sm_mhz"]])
         if not args.no_cpu_baseline:
             try:
                 v, desc, cores = oracle_sample(wl, n_attn_nodes=args.baseline_nodes)

@@ -90,6 +90,12 @@ const char* echo_last_error(EchoCtx* ctx);  /* text of the last ECHO_ERR_CUDA on
 /* Copies the device status word to *flags with a blocking 4-byte copy on `stream` and clears it. */
 int echo_device_status(EchoCtx* ctx, uint32_t* flags, echo_stream_t stream);
 int echo_set_option(EchoCtx* ctx, int key, int64_t value);
+/* Measurement helpers (bench.py).  echo_launch_count: kernels this library has launched in this process so far (a
+ * host-side counter).  echo_probe_sm_clock: queues a one-thread kernel on `stream` that spins ~20 us and writes the SM
+ * clock it ran at, in MHz, to the DEVICE float *mhz_dev (cycle counter / global timer): the clock under load, which
+ * NVML does not show for kernels shorter than its sampling period. */
+uint64_t echo_launch_count(void);
+int echo_probe_sm_clock(EchoCtx* ctx, float* mhz_dev, echo_stream_t stream);
 
 /* ---- problem statement ----------------------------------- */
 /* Candidate draft trees G_i with parent function pa(j) and draft log-probabilities (Eq. 5). */

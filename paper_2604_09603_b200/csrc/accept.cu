@@ -208,6 +208,7 @@ int launch_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult
     if (!out->target_token_out && (size_t)sel->capacity * sizeof(int32_t) > ctx->workspace_bytes)
       return ECHO_ERR_WORKSPACE;
     if (sel->capacity > 0)
+      ECHO_COUNT_LAUNCH();
       k_argmax_bf16<<<sel->capacity, AM_THREADS, 0, st>>>(
           sel->n_selected, reinterpret_cast<const __nv_bfloat16*>(res->target_logits), res->ld, res->vocab, tout);
     tt = tout;

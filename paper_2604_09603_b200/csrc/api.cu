@@ -18,7 +18,31 @@ struct DeviceGuard {
   }
 };
 
+// SM clock seen by a kernel right now: one thread spins ~20 us and divides its cycle counter by the global timer.
+// NVML / nvidia-smi sample every 20-100 ms at best and read 1965 MHz between kernels; under the verify step the SMs
+// run at 1.25-1.5 GHz, and a kernel bound by SM cycles scales with that.
+__global__ void k_clock_probe(float* out) {
+  unsigned long long t0, t1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  const long long c0 = clock64();
+  do {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+  } while (t1 - t0 < 20000ull);
+  const long long c1 = clock64();
+  *out = (float)((double)(c1 - c0) * 1000.0 / (double)(t1 - t0));
+}
+
 extern "C" {
+
+uint64_t echo_launch_count(void) { return g_echo_launches.load(std::memory_order_relaxed); }
+
+int echo_probe_sm_clock(EchoCtx* ctx, float* mhz_dev, echo_stream_t stream) {
+  if (!ctx || !mhz_dev) return ECHO_ERR_INVALID_ARG;
+  DeviceGuard dg(ctx);
+  k_clock_probe<<<1, 1, 0, reinterpret_cast<cudaStream_t>(stream)>>>(mhz_dev);
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}
 
 const char* echo_strerror(int code) {
   switch (code) {

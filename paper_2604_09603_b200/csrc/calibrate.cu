@@ -198,13 +198,16 @@ int launch_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibr
   if (M > 0) {
     const long long blocks = (M + 255) / 256;
     if (blocks > 0x7fffffffll) return ECHO_ERR_UNSUPPORTED;
+    ECHO_COUNT_LAUNCH();
     k_calib_partition<<<(unsigned)blocks, 256, 0, st>>>(t->depth, t->conf, t->accepted, M, g_cnt, seg, ctx->dev_status);
   }
   if (!ctx->calib_attr_set) {  // per context: the attribute is a per-device property of the function
     ECHO_CUDA_TRY(ctx, cudaFuncSetAttribute(k_calib_depth, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL));
     ctx->calib_attr_set = true;
   }
+  ECHO_COUNT_LAUNCH();
   k_calib_depth<<<ECHO_MAX_DEPTH, NT, SM_TOTAL, st>>>(g_cnt, seg, o->auc, o->tau, o->n_pos, o->n_neg);
+  ECHO_COUNT_LAUNCH();
   k_calib_finish<<<1, 32, 0, st>>>(o->auc, o->n_pos, o->n_neg, delta, o->depth_mask);
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

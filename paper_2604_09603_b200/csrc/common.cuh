@@ -48,6 +48,12 @@ static inline int attn_split_policy(const EchoCtx* ctx, long R, long Hkv) {
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// kernels launched by this library in this process (echo_launch_count): bench.py's `gpu_launches` is this counter's
+// increase over the timed region, not arithmetic
+#include <atomic>
+inline std::atomic<uint64_t> g_echo_launches{0};
+#define ECHO_COUNT_LAUNCH() (g_echo_launches.fetch_add(1, std::memory_order_relaxed))
+
 // launchers implemented by the .cu files
 // Programmatic dependent launch: the kernel may start while its predecessor on the stream is still running; it
 // must call pdl_wait() before touching anything the predecessor writes (or reads and this kernel overwrites).
@@ -64,6 +70,7 @@ static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 b
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  ECHO_COUNT_LAUNCH();
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 #ifdef __CUDACC__

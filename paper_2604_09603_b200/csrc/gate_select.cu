@@ -6,7 +6,9 @@
 //                   counts and CSR offsets.
 //   k_pack        : one CTA per request -- Flatten & Pack (Fig. 3(3)) with local parents and 128-bit
 //                   ancestor masks.
-// These steps move < 1 MB and are latency-bound: three launches, no host sync.
+// These steps move < 1 MB and are latency-bound: three launches, no host sync.  (Tried in
+// round 2: scoring in CTAs of eight requests whose last one, by a ticket, runs the select -- and the packing too: no
+// gain, 30 us against 28; packing by that one CTA is a chain of dependent loads per eight requests, 58 us.)
 #include "common.cuh"
 
 namespace {
@@ -43,36 +45,39 @@ __device__ __forceinline__ uint64_t make_key_alg1(int phase, int depth, int requ
   return ((uint64_t)phase << 63) | ((uint64_t)depth << 56) | ((uint64_t)(uint32_t)request << 16) | (uint64_t)rank;
 }
 
-__global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
-    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent, const float* __restrict__ logq,
-    const __grid_constant__ GateParams gp, float* __restrict__ path_score, uint8_t* __restrict__ cand_depth,
-    int32_t* __restrict__ cut_depth, uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
-  __shared__ int s_par[ECHO_MAX_CAND];
-  __shared__ float s_lq[ECHO_MAX_CAND];
-  __shared__ float s_S[ECHO_MAX_CAND];
-  __shared__ int s_d[ECHO_MAX_CAND];
-  __shared__ uint32_t s_lvlmax[ECHO_MAX_DEPTH];
-  __shared__ int s_cut;
+// Shared memory of one request's scoring (one 128-thread group)
+struct ScoreSmem {
+  int par[ECHO_MAX_CAND];
+  float lq[ECHO_MAX_CAND];
+  float S[ECHO_MAX_CAND];
+  int d[ECHO_MAX_CAND];
+  uint32_t lvlmax[ECHO_MAX_DEPTH];
+  int cut;
+};
 
-  pdl_launch_dependents();
-  const int i = blockIdx.x;
-  const int b = cand_offsets[i];
-  const int C_all = cand_offsets[i + 1] - b;
+// S1-S2 and the selection keys of request i; j = candidate = thread in the request's 128-thread group.  `active` is
+// false for a group without a request (it still takes part in the CTA-wide barriers).
+__device__ __forceinline__ void score_gate_request(
+    bool active, int i, int j, ScoreSmem& sm, const int32_t* __restrict__ cand_offsets,
+    const int32_t* __restrict__ parent, const float* __restrict__ logq, const GateParams& gp,
+    float* __restrict__ path_score, uint8_t* __restrict__ cand_depth, int32_t* __restrict__ cut_depth,
+    uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
+  int b = 0, C_all = 0;
+  if (active) { b = cand_offsets[i]; C_all = cand_offsets[i + 1] - b; }
   const int C = min(C_all, ECHO_MAX_CAND);
-  const int j = threadIdx.x;
   uint32_t bad = 0;
   if (C_all > ECHO_MAX_CAND) {  // more candidates than a request may have (R:G-14): flag, and make the excess
-    bad |= ECHO_DEV_CAND_OVERFLOW;  // ineligible so that k_select never reads an unwritten key
+    bad |= ECHO_DEV_CAND_OVERFLOW;  // ineligible so that the select never reads an unwritten key
     for (int t = ECHO_MAX_CAND + j; t < C_all; t += ECHO_MAX_CAND) keys[b + t] = KEY_INELIGIBLE;
   }
-  if (j < ECHO_MAX_DEPTH) s_lvlmax[j] = 0u;
+  if (j < ECHO_MAX_DEPTH) sm.lvlmax[j] = 0u;
   if (j < C) {
     int p = parent[b + j];
     float lq = logq[b + j];
     if (p >= j || p < -1) { bad |= ECHO_DEV_BAD_PARENT; p = -1; }
     if (!(lq <= 0.0f)) bad |= ECHO_DEV_BAD_LOGQ;
-    s_par[j] = p;
-    s_lq[j] = lq;
+    sm.par[j] = p;
+    sm.lq[j] = lq;
   }
   __syncthreads();
 
@@ -83,43 +88,43 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
     // bit-identical to the sequential recurrence (R:G-3); __fadd_rn forbids contraction.
     int chain[ECHO_MAX_DEPTH];
     int n = 0, c = j;
-    while (c >= 0 && n < ECHO_MAX_DEPTH) { chain[n++] = c; c = s_par[c]; }
+    while (c >= 0 && n < ECHO_MAX_DEPTH) { chain[n++] = c; c = sm.par[c]; }
     if (c >= 0) bad |= ECHO_DEV_DEPTH_OVERFLOW;
-    for (int k = n - 1; k >= 0; --k) S = __fadd_rn(S, s_lq[chain[k]]);
+    for (int k = n - 1; k >= 0; --k) S = __fadd_rn(S, sm.lq[chain[k]]);
     d = n - 1;
-    s_S[j] = S;
-    s_d[j] = d;
+    sm.S[j] = S;
+    sm.d[j] = d;
     path_score[b + j] = S;
     cand_depth[b + j] = (uint8_t)d;
-    atomicMax(&s_lvlmax[d], f32_ordered(S));  // S2: m[i][d] (Eq. 6 in the log domain)
+    atomicMax(&sm.lvlmax[d], f32_ordered(S));  // S2: m[i][d] (Eq. 6 in the log domain)
   }
   if (bad) atomicOr(status, bad);
   __syncthreads();
 
-  if (j == 0) {
+  if (j == 0 && active) {
     int cut = ECHO_CUT_NEVER;
     if (gp.static_k <= 0) {
       for (int dd = 0; dd < ECHO_MAX_DEPTH; ++dd) {
-        if (!((gp.depth_mask >> dd) & 1u) || s_lvlmax[dd] == 0u) continue;  // ungated or absent level (R:G-5)
-        if (!(f32_unordered(s_lvlmax[dd]) > gp.log_tau[dd])) { cut = dd; break; }  // Eq. 7, strict (R:G-4)
+        if (!((gp.depth_mask >> dd) & 1u) || sm.lvlmax[dd] == 0u) continue;  // ungated or absent level (R:G-5)
+        if (!(f32_unordered(sm.lvlmax[dd]) > gp.log_tau[dd])) { cut = dd; break; }  // Eq. 7, strict (R:G-4)
       }
     }
-    s_cut = cut;
+    sm.cut = cut;
     cut_depth[i] = cut;
   }
   __syncthreads();
 
   if (j < C) {
-    const int cut = s_cut;
+    const int cut = sm.cut;
     uint64_t key = KEY_INELIGIBLE;
     if (gp.static_k > 0) {
       int rank = 0;  // per-request top-static_k by (S desc, node asc) (R:G-15)
-      for (int t = 0; t < C; ++t) rank += (s_S[t] > S) || (s_S[t] == S && t < j);
+      for (int t = 0; t < C; ++t) rank += (sm.S[t] > S) || (sm.S[t] == S && t < j);
       if (rank < gp.static_k) key = make_key(0, 0.0f, gp.cand_base + b + j);
     } else if (gp.schedule == ECHO_SCHED_ALG1) {
       if (d <= cut) {
         int rank = 0;  // position in the level by (S desc, node asc)
-        for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
+        for (int t = 0; t < C; ++t) rank += (sm.d[t] == d) && ((sm.S[t] > S) || (sm.S[t] == S && t < j));
         if (d < cut) key = make_key_alg1(0, d, gp.req_base + i, rank);
         else if (rank < gp.w_max) key = make_key_alg1(1, d, gp.req_base + i, rank);
       }
@@ -127,11 +132,21 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
       key = make_key(0, S, gp.cand_base + b + j);  // tier 0: depth extension
     } else if (d == cut) {
       int rank = 0;  // tier 1: the w_max best nodes of the truncation level (R:G-7, G-8)
-      for (int t = 0; t < C; ++t) rank += (s_d[t] == d) && ((s_S[t] > S) || (s_S[t] == S && t < j));
+      for (int t = 0; t < C; ++t) rank += (sm.d[t] == d) && ((sm.S[t] > S) || (sm.S[t] == S && t < j));
       if (rank < gp.w_max) key = make_key(1, S, gp.cand_base + b + j);
     }
     keys[b + j] = key;
   }
+}
+
+__global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent, const float* __restrict__ logq,
+    const __grid_constant__ GateParams gp, float* __restrict__ path_score, uint8_t* __restrict__ cand_depth,
+    int32_t* __restrict__ cut_depth, uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
+  __shared__ ScoreSmem sm;
+  pdl_launch_dependents();
+  score_gate_request(true, blockIdx.x, threadIdx.x, sm, cand_offsets, parent, logq, gp, path_score, cand_depth, cut_depth,
+                     keys, status);
 }
 
 constexpr int SEL_THREADS = 1024;
@@ -146,21 +161,30 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   return v;
 }
 
-__global__ void __launch_bounds__(SEL_THREADS) k_select(
-    const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ local_keys, int R,
+struct SelectSmem {
+  int hist[256];
+  int warp[32];
+  uint64_t prefix;
+  int k;
+  int eligible;
+  int done;
+};
+
+// S3 + the CSR offsets of S4 by one CTA of SEL_THREADS threads.  Returns (in every thread) the threshold: keys below it
+// are selected (0 = nothing).
+__device__ __forceinline__ uint64_t select_body(
+    SelectSmem& sm, const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ local_keys, int R,
     const uint64_t* __restrict__ keys, int N, int budget, int32_t* __restrict__ n_selected,
-    int32_t* __restrict__ sel_offsets, uint64_t* __restrict__ threshold) {
+    int32_t* __restrict__ sel_offsets) {
   // `keys` [N] is the whole key population the budget is drawn from (this call's own keys, or the keys of every rank
   // that shares the budget); `local_keys` are this call's candidates, indexed like cand_offsets.
-  __shared__ int s_hist[256];
-  __shared__ int s_warp[32];
-  __shared__ uint64_t s_prefix;
-  __shared__ int s_k;
-  __shared__ int s_eligible;
-  __shared__ int s_done;
+  int (&s_hist)[256] = sm.hist;
+  int (&s_warp)[32] = sm.warp;
+  uint64_t& s_prefix = sm.prefix;
+  int& s_k = sm.k;
+  int& s_eligible = sm.eligible;
+  int& s_done = sm.done;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  pdl_launch_dependents();
-  pdl_wait();  // keys come from k_score_gate
 
   // ---- S3: threshold T = budget-th smallest key (keys are unique => no ties to break) ----
   // Keys stay in registers across the passes when N <= SEL_THREADS * SEL_KPT (every config of BASELINE.json),
@@ -287,55 +311,68 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(
     for (int r = lo; r < hi; ++r) { run += sel_offsets[r + 1]; sel_offsets[r + 1] = run; }
     if (tid == SEL_THREADS - 1) *n_selected = s_warp[31];
   }
-  if (tid == 0) *threshold = none ? 0ull : T + 1ull;  // k_pack selects keys < threshold (0 = nothing; T < 2^64 - 1)
+  __syncthreads();  // the offsets are complete for whoever packs next
+  return none ? 0ull : T + 1ull;  // keys < threshold are selected (0 = nothing; T < 2^64 - 1)
 }
 
-// S4/S5: packed arrays, local parents, ancestor-or-self masks.  One CTA per request, thread = candidate.
-__global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
-    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent,
-    const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys,
-    const uint64_t* __restrict__ threshold, int capacity, const int32_t* __restrict__ sel_offsets,
-    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
-    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
-  __shared__ int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks below are chains of dependent reads
-  __shared__ uint32_t s_bal[4];
-  const int r = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__global__ void __launch_bounds__(SEL_THREADS) k_select(
+    const int32_t* __restrict__ cand_offsets, const uint64_t* __restrict__ local_keys, int R,
+    const uint64_t* __restrict__ keys, int N, int budget, int32_t* __restrict__ n_selected,
+    int32_t* __restrict__ sel_offsets, uint64_t* __restrict__ threshold) {
+  __shared__ SelectSmem sm;
   pdl_launch_dependents();
-  pdl_wait();  // threshold and offsets come from k_select
+  pdl_wait();  // keys come from k_score_gate
+  const uint64_t thr = select_body(sm, cand_offsets, local_keys, R, keys, N, budget, n_selected, sel_offsets);
+  if (threadIdx.x == 0) *threshold = thr;
+}
+
+// S4/S5: packed arrays, local parents, ancestor-or-self masks of request r.  One 128-thread group per request, tid =
+// candidate; `active` is false for a group without a request (it still takes part in the CTA-wide barriers).
+struct PackSmem {
+  int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks below are chains of dependent reads
+  uint32_t bal[4];
+};
+__device__ __forceinline__ void pack_request(
+    bool active, int r, int tid, PackSmem& sm, const int32_t* __restrict__ cand_offsets,
+    const int32_t* __restrict__ parent, const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys,
+    uint64_t thr, int capacity, const int32_t* __restrict__ sel_offsets, int32_t* __restrict__ sel_node,
+    int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local, uint8_t* __restrict__ sel_depth,
+    uint32_t* __restrict__ anc_mask) {
+  const int lane = tid & 31, warp = tid >> 5;
+  int b = 0, C = 0, base = 0;
+  if (active) {
+    b = cand_offsets[r];
+    C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
+    base = sel_offsets[r];
+  }
   {
-    const int b = cand_offsets[r], C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
-    const int base = sel_offsets[r];
-    const uint64_t thr = *threshold;
-    {
-      const int j = tid;
-      const uint32_t mine = __ballot_sync(0xffffffffu, j < C && keys[b + j] < thr);
-      if (lane == 0) s_bal[warp] = mine;
-      if (j < C) {
-        const int pj = parent[b + j];
-        par[j] = pj >= j ? -1 : pj;
-      }
+    const int j = tid;
+    const uint32_t mine = __ballot_sync(0xffffffffu, j < C && keys[b + j] < thr);
+    if (lane == 0) sm.bal[warp] = mine;
+    if (j < C) {
+      const int pj = parent[b + j];
+      sm.par[j] = pj >= j ? -1 : pj;
     }
-    __syncthreads();
-    uint32_t bal[4];
+  }
+  __syncthreads();
+  uint32_t bal[4];
 #pragma unroll
-    for (int w = 0; w < 4; ++w) bal[w] = s_bal[w];
-    auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
-      int l = 0;
+  for (int w = 0; w < 4; ++w) bal[w] = sm.bal[w];
+  auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
+    int l = 0;
 #pragma unroll
-      for (int w = 0; w < 4; ++w) {
-        if (w < (c >> 5)) l += __popc(bal[w]);
-        else if (w == (c >> 5)) l += __popc(bal[w] & ((1u << (c & 31)) - 1u));
-      }
-      return l;
-    };
-    {
-      const int w = warp;
-      const int j = tid;
-      if (!((bal[w] >> lane) & 1u)) return;
-      const int l = local_of(j);
-      const int k = base + l;
-      if (k >= capacity) return;
-      const int p = par[j];
+    for (int w = 0; w < 4; ++w) {
+      if (w < (c >> 5)) l += __popc(bal[w]);
+      else if (w == (c >> 5)) l += __popc(bal[w] & ((1u << (c & 31)) - 1u));
+    }
+    return l;
+  };
+  const int j = tid;
+  if ((bal[warp] >> lane) & 1u) {
+    const int l = local_of(j);
+    const int k = base + l;
+    if (k < capacity) {
+      const int p = sm.par[j];
       uint32_t m[4] = {0u, 0u, 0u, 0u};
       m[l >> 5] |= 1u << (l & 31);
       int pl = -1;
@@ -345,7 +382,7 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
         int la = local_of(c);
         if (step == 0) pl = la;
         m[la >> 5] |= 1u << (la & 31);
-        c = par[c];
+        c = sm.par[c];
       }
       sel_node[k] = j;
       sel_req[k] = r;
@@ -354,6 +391,20 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
       reinterpret_cast<uint4*>(anc_mask)[k] = make_uint4(m[0], m[1], m[2], m[3]);
     }
   }
+  __syncthreads();  // the group's shared memory may be reused for its next request
+}
+
+__global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent,
+    const uint8_t* __restrict__ cand_depth, const uint64_t* __restrict__ keys,
+    const uint64_t* __restrict__ threshold, int capacity, const int32_t* __restrict__ sel_offsets,
+    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
+    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
+  __shared__ PackSmem sm;
+  pdl_launch_dependents();
+  pdl_wait();  // threshold and offsets come from k_select
+  pack_request(true, blockIdx.x, threadIdx.x, sm, cand_offsets, parent, cand_depth, keys, *threshold, capacity,
+               sel_offsets, sel_node, sel_req, parent_local, sel_depth, anc_mask);
 }
 
 }  // namespace
@@ -373,6 +424,7 @@ static GateParams gate_params(const EchoGate* g) {
 int launch_gate_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, uint64_t* keys,
                      cudaStream_t st) {
   if (t->num_requests > 0) {
+    ECHO_COUNT_LAUNCH();
     k_score_gate<<<t->num_requests, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g),
                                                             o->path_score, o->cand_depth, o->cut_depth, keys,
                                                             ctx->dev_status);
@@ -406,6 +458,7 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
   if (keys_bytes + 256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
   uint64_t* threshold = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(ctx->workspace) + keys_bytes);
   if (R > 0) {
+    ECHO_COUNT_LAUNCH();
     k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g), o->path_score,
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);
   }
@@ -413,9 +466,9 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
   ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, keys, N, budget,
                                 o->n_selected, o->sel_offsets, threshold));
   if (R > 0) {
-    ECHO_CUDA_TRY(ctx, launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent, o->cand_depth, keys, threshold, o->capacity,
-                                        o->sel_offsets, o->sel_node, o->sel_req, o->parent_local, o->sel_depth,
-                                        o->anc_mask));
+    ECHO_CUDA_TRY(ctx, launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent, o->cand_depth,
+                                  keys, threshold, o->capacity, o->sel_offsets, o->sel_node, o->sel_req, o->parent_local,
+                                  o->sel_depth, o->anc_mask));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

@@ -183,6 +183,7 @@ int launch_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV
   } else {
     if (G > 32) return ECHO_ERR_UNSUPPORTED;
     dim3 grid(cap, Hkv, splits);
+    ECHO_COUNT_LAUNCH();
     k_attn_smallrow<<<grid, G * 32, G * D * sizeof(float), st>>>(
         sel->n_selected, sel->sel_offsets, sel->sel_req, sel->anc_mask, kp, vp, kv->page_table, kv->prefix_len,
         kv->max_pages_per_req, Hkv, Hq, reinterpret_cast<const __nv_bfloat16*>(q),
@@ -191,6 +192,7 @@ int launch_verify_attn(EchoCtx* ctx, const EchoSelection* sel, const EchoPagedKV
   if (splits > 1) {
     const int wpb = 8;
     const unsigned blocks = (unsigned)((n_rows + wpb - 1) / wpb);
+    ECHO_COUNT_LAUNCH();
     k_lse_merge<<<blocks, wpb * 32, 0, st>>>(sel->n_selected, sel->sel_req, sel->sel_offsets, kv->prefix_len, Hq,
                                              n_rows, splits, part_o, part_lse,
                                              reinterpret_cast<__nv_bfloat16*>(out), lse);

@@ -1092,6 +1092,7 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    ECHO_COUNT_LAUNCH();
     ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_verify_attn_tc, tq, tk, tv, p));
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());

@@ -26,7 +26,8 @@ CUT_NEVER = 0x7FFFFFFF
 DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
-           "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_gate_select", "echo_verify_attn", "echo_accept",
+           "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_launch_count", "echo_probe_sm_clock",
+           "echo_gate_select", "echo_verify_attn", "echo_accept",
            "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand",
            "echo_accept_stochastic"]
 
@@ -113,6 +114,10 @@ def load_library():
     lib.echo_workspace_bytes.argtypes = [C.c_int32] * 5
     lib.echo_attn_splits.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
     lib.echo_attn_splits.restype = C.c_int
+    lib.echo_launch_count.argtypes = []
+    lib.echo_launch_count.restype = C.c_uint64
+    lib.echo_probe_sm_clock.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.echo_probe_sm_clock.restype = C.c_int
     lib.echo_workspace_bytes.restype = C.c_size_t
     lib.echo_strerror.argtypes = [C.c_int]
     lib.echo_strerror.restype = C.c_char_p
@@ -295,6 +300,14 @@ class EchoContext:
         if rc < 0:
             self._check(rc)
         return buf[:rc]
+
+    def launch_count(self) -> int:
+        """kernels libecho.so has launched in this process so far"""
+        return int(self.lib.echo_launch_count())
+
+    def probe_sm_clock(self, out):
+        """queues the SM clock probe; `out` = a float32 device tensor element (MHz, written when the stream gets there)"""
+        self._check(self.lib.echo_probe_sm_clock(self._h, _ptr(out), self._stream()))
 
     def device_status(self) -> int:
         f = C.c_uint32(0)
