@@ -56,6 +56,7 @@ static_assert(SMEM_TOTAL <= 232448, "shared memory budget");
 constexpr int NTHREADS = 512;
 constexpr int W_EPI = 8, W_PROD_K = 12, W_MMA_QK = 13, W_PROD_V = 14, W_MMA_PV = 15;
 constexpr int REGS_SOFTMAX = 192, REGS_EPILOGUE = 80, REGS_AUX = 40;  // 128 * (2 * 192 + 80 + 40) <= 512 * 128, the launch allocation
+static_assert(NSTAGE == 3, "K / V stage g % NSTAGE and S buffer g % NSBUF must be the same index");
 constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
 constexpr int TMEM_O = NSBUF * TILE_N;
 constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
@@ -81,8 +82,8 @@ constexpr uint32_t IDESC_QK = tc::idesc_bf16(TILE_M, TILE_N, 0, 0);
 constexpr uint32_t IDESC_PV = tc::idesc_bf16(TILE_M, D, 0, 1);
 
 // barrier indices (8 bytes each)
-enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_KEMPTY = 5, B_VFULL = 8, B_VEMPTY = 11, B_SFULL = 14, B_PFULL = 17,
-       B_SFREE = 20, B_OFULL = 23, B_OFREE = 24, B_STATS = 25, B_STATFREE = 26, B_PHASE = 27, B_COUNT = 28 };
+enum { B_QFULL = 0, B_QEMPTY = 1, B_KFULL = 2, B_VFULL = 5, B_SFULL = 8, B_PFULL = 11, B_SFREE = 14, B_OFULL = 17,
+       B_OFREE = 18, B_STATS = 19, B_STATFREE = 20, B_PHASE = 21, B_COUNT = 22 };
 static_assert(B_COUNT * 8 <= BAR_BYTES, "barrier region");
 
 struct AttnParams {
@@ -148,7 +149,6 @@ __device__ __forceinline__ Item decode(const int4 v, const int4 w) {
   it.P = w.x; it.off = w.y; it.Ki = w.z;
   return it;
 }
-__device__ __forceinline__ Item load_item(const int4* items, int idx) { return decode(items[2 * idx], items[2 * idx + 1]); }
 // snake order over the length-sorted work list: round k of CTA c takes k*G+c (k even) or (k+1)*G-1-c (k odd)
 __device__ __forceinline__ int item_index(int k, int cta, int grid) {
   return (k & 1) ? (k + 1) * grid - 1 - cta : k * grid + cta;
@@ -264,9 +264,6 @@ __device__ __forceinline__ void weights_chunk(const uint32_t (&sc)[32], uint64_t
   for (int e = 0; e < 32; e += 2) {
     const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
     float p0, p1;
-#ifdef ECHO_EXP_NOEXP
-    tc::unpack_f32x2(x2, p0, p1);
-#else
     if (((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
       ex2_poly_x2(x2, p0, p1);
     } else {
@@ -275,11 +272,8 @@ __device__ __forceinline__ void weights_chunk(const uint32_t (&sc)[32], uint64_t
       p0 = tc::ex2(x0);
       p1 = tc::ex2(x1);
     }
-#endif
     pk[e >> 1] = tc::pack_bf16(p0, p1);
-#ifndef ECHO_EXP_NOSUM
     acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
-#endif
   }
 }
 
@@ -287,40 +281,6 @@ __device__ __forceinline__ float acc_total(const uint64_t (&acc)[4]) {
   float a0, a1;
   tc::unpack_f32x2(tc::add_f32x2(tc::add_f32x2(acc[0], acc[1]), tc::add_f32x2(acc[2], acc[3])), a0, a1);
   return a0 + a1;
-}
-
-// One chunk of a row, S registers -> P in TMEM.  In a tile that touches the tree or the ragged end (`masked`, uniform
-// over the CTA) a vote over the warp's rows sorts the chunk: all keys visible -> nothing to do; none visible -> zeros;
-// else the invisible keys are set to -inf and the chunk's share of the normaliser becomes the sum of the bf16-ROUNDED
-// weights (few visible keys: O must stay an exact convex combination of V rows; lse always takes the exact sum).
-// One body for both kinds of tile, on purpose: the masked tile runs once per item, and code that runs once per item
-// is fetched from L2 every time -- the separate masked instantiation cost ~2000 cycles per item in instruction misses.
-__device__ __forceinline__ void chunk_to_p(uint32_t (&sc)[32], uint32_t vis, bool masked, uint64_t sc2, uint64_t nm2,
-                                           uint32_t tP, uint64_t (&acc)[4], float& tr_adj) {
-  uint32_t pk[16];
-  bool partial = false;
-  if (masked && !__all_sync(0xffffffffu, vis == 0xffffffffu)) {
-    if (__all_sync(0xffffffffu, vis == 0u)) {
-#pragma unroll
-      for (int e = 0; e < 16; ++e) pk[e] = 0u;
-      tc::tmem_st16(tP, pk);
-      return;
-    }
-    mask_chunk(sc, vis);
-    partial = true;
-  }
-  const float before = partial ? acc_total(acc) : 0.f;
-  weights_chunk(sc, sc2, nm2, pk, acc);
-  if (partial) {  // (rounded - exact) sum of this chunk's weights
-    float r0 = 0.f, r1 = 0.f;
-#pragma unroll
-    for (int e = 0; e < 16; ++e) {
-      r0 += __uint_as_float(pk[e] << 16);
-      r1 += __uint_as_float(pk[e] & 0xffff0000u);
-    }
-    tr_adj += (r0 + r1) - (acc_total(acc) - before);
-  }
-  tc::tmem_st16(tP, pk);
 }
 
 // One S row (128 fp32 columns in TMEM at tS) -> bf16 P over its first 64 columns, four 32-column chunks, the load of
@@ -343,46 +303,60 @@ __device__ __forceinline__ void tile_weights_fast(uint32_t tS, float scale_log2,
   ts = acc_total(acc);
 }
 
-// The same for a tile that touches the tree or the ragged end (once or twice per item) and for the safe form: the
-// loop is rolled over chunk pairs and shares one body for all kinds of chunk -- compact rather than fast, because
-// code that runs once per item is fetched from L2 every time.  tr = the normaliser's share.
-__device__ __forceinline__ void tile_weights_masked(uint32_t tS, const uint32_t (&vis)[4], float scale_log2, float neg_m,
-                                                    float& ts, float& tr) {
-  const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
-  uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};
-  float tr_adj = 0.f;
-  uint32_t s0[32], s1[32];
-  tc::tmem_ld32(tS, s0);
+// A tile that touches the tree or the ragged end (once or twice per item) goes through the SAME hot loop: first the
+// invisible keys of the row are overwritten with -inf in TMEM (chunks every row of the warp sees whole are skipped),
+// afterwards the bf16 weights just stored are summed for the normaliser (few visible keys: O must stay an exact convex
+// combination of V rows; lse always takes the exact sum).  Both passes are small rolled loops on purpose: code that
+// runs once per item is fetched from L2 every time, and a separate unrolled masked instantiation of the tile body
+// cost ~3000 cycles per item in instruction misses (event trace, round 2).
+__device__ __forceinline__ void mask_tile_in_tmem(uint32_t tS, const uint32_t (&vis)[4]) {
 #pragma unroll 1
-  for (int cc = 0; cc < 2; ++cc) {
+  for (int c = 0; c < 4; ++c) {
+    const uint32_t v = c == 0 ? vis[0] : c == 1 ? vis[1] : c == 2 ? vis[2] : vis[3];
+    if (__all_sync(0xffffffffu, v == 0xffffffffu)) continue;  // warp-uniform
+    uint32_t s[32];
+    tc::tmem_ld32(tS + 32 * c, s);
     tc::tmem_wait_ld();
-    tc::reg_fence32(s0);
-    tc::tmem_ld32(tS + 64 * cc + 32, s1);
-    chunk_to_p(s0, cc ? vis[2] : vis[0], true, sc2, nm2, tS + 32 * cc, acc, tr_adj);  // P columns [32cc, 32cc+16)
-    tc::tmem_wait_ld();
-    tc::reg_fence32(s1);
-    if (cc == 0) tc::tmem_ld32(tS + 64, s0);
-    chunk_to_p(s1, cc ? vis[3] : vis[1], true, sc2, nm2, tS + 32 * cc + 16, acc, tr_adj);
+    tc::reg_fence32(s);
+    mask_chunk(s, v);
+    tc::tmem_st32(tS + 32 * c, s);
   }
-  ts = acc_total(acc);
-  tr = ts + tr_adj;
+  tc::tmem_wait_st();
+}
+__device__ __forceinline__ float rounded_sum_of_p(uint32_t tS) {  // P = bf16 pairs in columns [0,64)
+  float r0 = 0.f, r1 = 0.f;
+  tc::tmem_wait_st();
+#pragma unroll 1
+  for (int c = 0; c < 2; ++c) {
+    uint32_t pk[32];
+    tc::tmem_ld32(tS + 32 * c, pk);
+    tc::tmem_wait_ld();
+    tc::reg_fence32(pk);
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+      r0 += __uint_as_float(pk[e] << 16);
+      r1 += __uint_as_float(pk[e] & 0xffff0000u);
+    }
+  }
+  return r0 + r1;
 }
 
-__device__ __forceinline__ float row_max_pass(uint32_t tS, const uint32_t (&vis)[4]) {
-  float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-  uint32_t s[2][32];
-  tc::tmem_ld32(tS, s[0]);
-#pragma unroll
+// row maximum of S (masked keys already hold -inf), for the safe form
+__device__ __forceinline__ float row_max_pass(uint32_t tS) {
+  float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll 1
   for (int c = 0; c < 4; ++c) {
+    uint32_t s[32];
+    tc::tmem_ld32(tS + 32 * c, s);
     tc::tmem_wait_ld();
-    tc::reg_fence32(s[c & 1]);
-    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
-    mask_chunk(s[c & 1], vis[c]);
+    tc::reg_fence32(s);
 #pragma unroll
-    for (int e = 0; e < 32; e += 2)
-      mx[(e >> 1) & 3] = tc::max3(mx[(e >> 1) & 3], __uint_as_float(s[c & 1][e]), __uint_as_float(s[c & 1][e + 1]));
+    for (int e = 0; e < 32; e += 4) {
+      mx0 = tc::max3(mx0, __uint_as_float(s[e]), __uint_as_float(s[e + 1]));
+      mx1 = tc::max3(mx1, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
+    }
   }
-  return fmaxf(fmaxf(mx[0], mx[1]), fmaxf(mx[2], mx[3]));
+  return fmaxf(mx0, mx1);
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_constant__ CUtensorMap tmap_q,
@@ -438,7 +412,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const bool is_k = warp == W_PROD_K;
       const uint32_t s_dst = is_k ? sK : sV;
       const CUtensorMap* tmap = is_k ? &tmap_k : &tmap_v;
-      const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
+      // "stage empty" is not a barrier of its own: K stage g % 3 is free when QK^T of tile g has completed, which is
+      // what B_SFULL[g % 3] says, and V stage g % 3 when PV of tile g has, which is B_SFREE[g % 3] (NSTAGE == NSBUF, one
+      // tile counter).  Every tcgen05.commit costs the issuing thread ~150 cycles in the queue it shares with the MMAs
+      // (`mio` stalls on UTCBAR, ncu source page): two commits per tile less.
+      const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_SFULL : B_SFREE;
       int g = 0, itc = 0;
       PROF_DECL(3);
       PROF_T0();
@@ -569,8 +547,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
               const uint32_t k16 = ((kk & 3) * 32 + (kk >> 2) * 1024) >> 4;
               tc::mma_ss(tmem_u + b * TILE_N, qdesc + q16, kdesc + k16, IDESC_QK, kk > 0);
             }
-            tc::mma_commit(bar(B_SFULL + b));
-            tc::mma_commit(bar(B_KEMPTY + slot));
+            tc::mma_commit(bar(B_SFULL + b));  // S_b is complete and K stage `slot` (== b) is free
             if (j == n - 1) tc::mma_commit(bar(B_QEMPTY));
           }
           __syncwarp();
@@ -608,8 +585,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 #pragma unroll
             for (int kk = 0; kk < TILE_N / 16; ++kk)
               tc::mma_ts(tO, tmem_u + b * TILE_N + kk * 8, vdesc + ((kk * 2 * GROUP_BYTES) >> 4), IDESC_PV, (j > 0) || (kk > 0));
-            tc::mma_commit(bar(B_VEMPTY + slot));
-            tc::mma_commit(bar(B_SFREE + b));
+            tc::mma_commit(bar(B_SFREE + b));  // P_b has been read and V stage `slot` (== b) is free
             if (j == n - 1) tc::mma_commit(bar(B_OFULL));
           }
           __syncwarp();
@@ -667,15 +643,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
           for (int c = 0; c < 4; ++c) vis[c] = visible_word(mk, P, tile0 + 32 * c);
         }
         float ts = 0.f, tr = 0.f;  // this tile's exact weight sum / share of the normaliser
-        if (!safe && !masked) {
-          tile_weights_fast(tS, p.scale_log2, 0.f, ts);
-          tr = ts;
-        } else if (!safe) {
-          tile_weights_masked(tS, vis, p.scale_log2, 0.f, ts, tr);
-        } else {
+        if (masked) mask_tile_in_tmem(tS, vis);
+        float neg_ref = 0.f;
+        if (safe) {
           // safe form: row maximum first, O rescaled in TMEM when the reference moves (all lanes take the same path:
           // the TMEM instructions are warp-wide)
-          const float mx = row_max_pass(tS, vis);
+          const float mx = row_max_pass(tS);
           const float m_new = fmaxf(m_used, mx * p.scale_log2);
           float alpha = 1.f;
           if (m_new > m_used) {
@@ -691,7 +664,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             // rescaled under a running PV.
             PROF_WAIT(3, bar(B_SFREE + (g - 1) % NSBUF), ((g - 1) / NSBUF) & 1);
             tc::tc_fence_after();
-#pragma unroll
+#pragma unroll 1
             for (int c = 0; c < 4; ++c) {
               uint32_t o[32];
               tc::tmem_ld32(tO + c * 32, o);
@@ -703,9 +676,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
             }
             tc::tmem_wait_st();
           }
-          const float m_eff = (m_used == -INFINITY) ? 0.f : m_used;
-          tile_weights_masked(tS, vis, p.scale_log2, -m_eff, ts, tr);
+          neg_ref = (m_used == -INFINITY) ? 0.f : -m_used;
         }
+        tile_weights_fast(tS, p.scale_log2, neg_ref, ts);
+        tr = (masked || safe) ? rounded_sum_of_p(tS) : ts;
         lsum += ts;
         lnorm += tr;
         tc::tmem_wait_st();
@@ -806,25 +780,25 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
       const float m_ref = stats[ST_M0 * TILE_M + row];
       tc::mbar_arrive(bar(B_STATFREE));
       if (!safe) {
-#ifdef ECHO_EXP_NOCHECK
-        const bool bad = false;
-#else
         const bool bad = valid && !(lsum >= SUM_LO && lsum <= SUM_HI);
-#endif
         if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(const_cast<uint32_t*>(redo) + (k >> 5), 1u << (k & 31));
       }
       const float inv = lnorm > 0.f ? 1.f / lnorm : 0.f;
       const float lse_v = lsum > 0.f ? (m_ref + log2f(lsum)) * LN2 : -INFINITY;
       PROF_WAIT(2, bar(B_OFULL), itc & 1);
       tc::tc_fence_after();
-      uint32_t o[2][32];
-      tc::tmem_ld32(tO, o[0]);
-#pragma unroll
+      // rolled on purpose (this code runs once per item and is fetched from L2 every time); O is handed back to the
+      // PV issuer as soon as its last chunk is in registers, before that chunk is converted and stored
+#pragma unroll 1
       for (int c = 0; c < 4; ++c) {
+        uint32_t oc[32];
+        tc::tmem_ld32(tO + c * 32, oc);
         tc::tmem_wait_ld();
-        tc::reg_fence32(o[c & 1]);
-        if (c < 3) tc::tmem_ld32(tO + (c + 1) * 32, o[(c + 1) & 1]);
-        uint32_t(&oc)[32] = o[c & 1];
+        tc::reg_fence32(oc);
+        if (c == 3) {
+          tc::tc_fence_before();
+          tc::mbar_arrive(bar(B_OFREE));
+        }
         if (valid) {
           if (p.splits == 1) {
             uint4* dst = reinterpret_cast<uint4*>(p.out + rowg * D + c * 32);
@@ -850,8 +824,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         if (p.splits == 1) p.lse[rowg] = lse_v;
         else p.part_lse[(size_t)it.split * p.n_rows_cap + rowg] = lse_v;
       }
-      tc::tc_fence_before();
-      tc::mbar_arrive(bar(B_OFREE));
       ++itc;
     };
     // between the phases: the bitmap is final (release); every role, this one included, then reads it
