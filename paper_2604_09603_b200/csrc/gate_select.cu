@@ -1,4 +1,8 @@
 // echo_gate_select: S1-S5 of the super-tree verify step (include/echo.h).
+//   k_gate_cluster: all of it as ONE launch of one thread-block cluster (<= 16 CTAs x 1024 threads, 8 requests per CTA
+//                   and round): keys stay in shared memory, the radix select's histograms are summed through
+//                   distributed shared memory, the thread that made a key packs its node.  The path echo_gate_select
+//                   takes for up to 512 requests.
 //   k_score_gate  : one CTA per request -- path scores (Eq. 5), level maxima and the
 //                   sparse gate (Eq. 6-7), tier assignment (Alg. 1) and a
 //                   unique 64-bit selection key per candidate.
@@ -6,10 +10,17 @@
 //                   counts and CSR offsets.
 //   k_pack        : one CTA per request -- Flatten & Pack (Fig. 3(3)) with local parents and 128-bit
 //                   ancestor masks.
-// These steps move < 1 MB and are latency-bound: three launches, no host sync.  (Tried in
-// round 2: scoring in CTAs of eight requests whose last one, by a ticket, runs the select -- and the packing too: no
-// gain, 30 us against 28; packing by that one CTA is a chain of dependent loads per eight requests, 58 us.)
+// The three-kernel chain serves echo_gate_keys / echo_gate_select_keys (several ranks share one budget: the key
+// population crosses processes between scoring and selecting), more than 512 requests, and ECHO_OPT_GATE_PATH = 1; it
+// shares the scoring and packing device functions with the cluster kernel.
+// These steps move < 1 MB and are latency-bound.  (Tried in round 2: scoring in CTAs of eight
+// requests whose last one, by a ticket, runs the select -- and the packing too: no gain, 30 us against 28; packing by
+// that one CTA is a chain of dependent loads per eight requests, 58 us.)
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -29,6 +40,7 @@ __device__ __forceinline__ float f32_unordered(uint32_t o) {
 }
 
 constexpr uint64_t KEY_INELIGIBLE = ~0ull;
+
 
 // key order == (tier asc, S desc, request asc, node asc): tier in bit 63, inverted ordered score in
 // bits 31..62, global candidate index (monotone in (request, node)) in bits 0..30.
@@ -52,28 +64,38 @@ struct ScoreSmem {
   float S[ECHO_MAX_CAND];
   int d[ECHO_MAX_CAND];
   uint32_t lvlmax[ECHO_MAX_DEPTH];
+  uint32_t lvlbal[ECHO_MAX_CAND / 32];
   int cut;
 };
 
-// S1-S2 and the selection keys of request i; j = candidate = thread in the request's 128-thread group.  `active` is
-// false for a group without a request (it still takes part in the CTA-wide barriers).
-__device__ __forceinline__ void score_gate_request(
-    bool active, int i, int j, ScoreSmem& sm, const int32_t* __restrict__ cand_offsets,
-    const int32_t* __restrict__ parent, const float* __restrict__ logq, const GateParams& gp,
-    float* __restrict__ path_score, uint8_t* __restrict__ cand_depth, int32_t* __restrict__ cut_depth,
-    uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
-  int b = 0, C_all = 0;
-  if (active) { b = cand_offsets[i]; C_all = cand_offsets[i + 1] - b; }
+// What candidate j of request i reads from global memory (issued ahead of the arithmetic that needs it)
+struct CandIn {
+  int b, C_all;  // first candidate of the request, its candidate count as given
+  int p;
+  float lq;
+};
+__device__ __forceinline__ CandIn load_cand(bool active, int i, int j, const int32_t* __restrict__ cand_offsets,
+                                            const int32_t* __restrict__ parent, const float* __restrict__ logq) {
+  CandIn in = {0, 0, -1, 0.0f};
+  if (active) { in.b = cand_offsets[i]; in.C_all = cand_offsets[i + 1] - in.b; }
+  if (j < min(in.C_all, ECHO_MAX_CAND)) { in.p = parent[in.b + j]; in.lq = logq[in.b + j]; }
+  return in;
+}
+
+// S1-S2 and the selection key of candidate j (= thread in the request's 128-thread group) of request i; the key is
+// returned (KEY_INELIGIBLE when j is past the request), the depth goes to d_out.  `active` is false for a group
+// without a request (it still takes part in the CTA-wide barriers).
+__device__ __forceinline__ uint64_t score_gate_request(
+    bool active, int i, int j, const CandIn& in, ScoreSmem& sm, const GateParams& gp, float* __restrict__ path_score,
+    uint8_t* __restrict__ cand_depth, int32_t* __restrict__ cut_depth, uint32_t* __restrict__ status, int& d_out) {
+  const int b = in.b, C_all = in.C_all;
   const int C = min(C_all, ECHO_MAX_CAND);
   uint32_t bad = 0;
-  if (C_all > ECHO_MAX_CAND) {  // more candidates than a request may have (R:G-14): flag, and make the excess
-    bad |= ECHO_DEV_CAND_OVERFLOW;  // ineligible so that the select never reads an unwritten key
-    for (int t = ECHO_MAX_CAND + j; t < C_all; t += ECHO_MAX_CAND) keys[b + t] = KEY_INELIGIBLE;
-  }
+  if (C_all > ECHO_MAX_CAND) bad |= ECHO_DEV_CAND_OVERFLOW;  // more candidates than a request may have (R:G-14)
   if (j < ECHO_MAX_DEPTH) sm.lvlmax[j] = 0u;
   if (j < C) {
-    int p = parent[b + j];
-    float lq = logq[b + j];
+    int p = in.p;
+    float lq = in.lq;
     if (p >= j || p < -1) { bad |= ECHO_DEV_BAD_PARENT; p = -1; }
     if (!(lq <= 0.0f)) bad |= ECHO_DEV_BAD_LOGQ;
     sm.par[j] = p;
@@ -101,42 +123,61 @@ __device__ __forceinline__ void score_gate_request(
   if (bad) atomicOr(status, bad);
   __syncthreads();
 
-  if (j == 0 && active) {
-    int cut = ECHO_CUT_NEVER;
-    if (gp.static_k <= 0) {
-      for (int dd = 0; dd < ECHO_MAX_DEPTH; ++dd) {
-        if (!((gp.depth_mask >> dd) & 1u) || sm.lvlmax[dd] == 0u) continue;  // ungated or absent level (R:G-5)
-        if (!(f32_unordered(sm.lvlmax[dd]) > gp.log_tau[dd])) { cut = dd; break; }  // Eq. 7, strict (R:G-4)
-      }
+  if (j < ECHO_MAX_DEPTH) {  // the group's first warp, lane = depth: the first gated level that fails Eq. 7
+    static_assert(ECHO_MAX_DEPTH == 32, "one lane per depth");
+    const uint32_t m = sm.lvlmax[j];
+    // ungated or absent levels never fail (R:G-5); the comparison is strict (R:G-4)
+    const bool fail = gp.static_k <= 0 && ((gp.depth_mask >> j) & 1u) && m != 0u && !(f32_unordered(m) > gp.log_tau[j]);
+    const unsigned fails = __ballot_sync(0xffffffffu, fail);
+    if (j == 0 && active) {
+      const int cut = fails ? __ffs(fails) - 1 : ECHO_CUT_NEVER;
+      sm.cut = cut;
+      cut_depth[i] = cut;
     }
-    sm.cut = cut;
-    cut_depth[i] = cut;
   }
   __syncthreads();
 
-  if (j < C) {
-    const int cut = sm.cut;
-    uint64_t key = KEY_INELIGIBLE;
+  uint64_t key = KEY_INELIGIBLE;
+  const int cut = sm.cut;
+  if (gp.static_k <= 0 && gp.schedule != ECHO_SCHED_ALG1) {
+    // tier 0: depth extension; tier 1: the w_max best nodes of the truncation level by (S desc, node asc)
+    // (R:G-7, G-8).  The level's nodes are first gathered into a list (the chain replays are over: lq and
+    // d hold the list's scores and node ids from here on), so a rank costs the level's width, not C, compares.
+    const bool lvl = j < C && d == cut;
+    const unsigned lane = j & 31, wq = j >> 5;
+    const unsigned mine = __ballot_sync(0xffffffffu, lvl);
+    if (lane == 0) sm.lvlbal[wq] = mine;
+    __syncthreads();
+    int pos = __popc(mine & ((1u << lane) - 1u)), n_lvl = 0;
+#pragma unroll
+    for (int w = 0; w < ECHO_MAX_CAND / 32; ++w) {
+      const int c = __popc(sm.lvlbal[w]);
+      if (w < (int)wq) pos += c;
+      n_lvl += c;
+    }
+    if (lvl) { sm.lq[pos] = S; sm.d[pos] = j; }
+    __syncthreads();
+    if (j < C && d < cut) {
+      key = make_key(0, S, gp.cand_base + b + j);
+    } else if (lvl) {
+      int rank = 0;
+      for (int t = 0; t < n_lvl; ++t) rank += (sm.lq[t] > S) || (sm.lq[t] == S && sm.d[t] < j);
+      if (rank < gp.w_max) key = make_key(1, S, gp.cand_base + b + j);
+    }
+  } else if (j < C) {
     if (gp.static_k > 0) {
       int rank = 0;  // per-request top-static_k by (S desc, node asc) (R:G-15)
       for (int t = 0; t < C; ++t) rank += (sm.S[t] > S) || (sm.S[t] == S && t < j);
       if (rank < gp.static_k) key = make_key(0, 0.0f, gp.cand_base + b + j);
-    } else if (gp.schedule == ECHO_SCHED_ALG1) {
-      if (d <= cut) {
-        int rank = 0;  // position in the level by (S desc, node asc)
-        for (int t = 0; t < C; ++t) rank += (sm.d[t] == d) && ((sm.S[t] > S) || (sm.S[t] == S && t < j));
-        if (d < cut) key = make_key_alg1(0, d, gp.req_base + i, rank);
-        else if (rank < gp.w_max) key = make_key_alg1(1, d, gp.req_base + i, rank);
-      }
-    } else if (d < cut) {
-      key = make_key(0, S, gp.cand_base + b + j);  // tier 0: depth extension
-    } else if (d == cut) {
-      int rank = 0;  // tier 1: the w_max best nodes of the truncation level (R:G-7, G-8)
+    } else if (d <= cut) {  // ECHO_SCHED_ALG1
+      int rank = 0;  // position in the level by (S desc, node asc)
       for (int t = 0; t < C; ++t) rank += (sm.d[t] == d) && ((sm.S[t] > S) || (sm.S[t] == S && t < j));
-      if (rank < gp.w_max) key = make_key(1, S, gp.cand_base + b + j);
+      if (d < cut) key = make_key_alg1(0, d, gp.req_base + i, rank);
+      else if (rank < gp.w_max) key = make_key_alg1(1, d, gp.req_base + i, rank);
     }
-    keys[b + j] = key;
   }
+  d_out = d;
+  return key;
 }
 
 __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
@@ -145,8 +186,13 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_score_gate(
     int32_t* __restrict__ cut_depth, uint64_t* __restrict__ keys, uint32_t* __restrict__ status) {
   __shared__ ScoreSmem sm;
   pdl_launch_dependents();
-  score_gate_request(true, blockIdx.x, threadIdx.x, sm, cand_offsets, parent, logq, gp, path_score, cand_depth, cut_depth,
-                     keys, status);
+  const int i = blockIdx.x, j = threadIdx.x;
+  const CandIn in = load_cand(true, i, j, cand_offsets, parent, logq);
+  int d;
+  const uint64_t key = score_gate_request(true, i, j, in, sm, gp, path_score, cand_depth, cut_depth, status, d);
+  if (j < min(in.C_all, ECHO_MAX_CAND)) keys[in.b + j] = key;
+  // the excess of an over-long request is ineligible, so that the select never reads an unwritten key
+  for (int t = ECHO_MAX_CAND + j; t < in.C_all; t += ECHO_MAX_CAND) keys[in.b + t] = KEY_INELIGIBLE;
 }
 
 constexpr int SEL_THREADS = 1024;
@@ -326,10 +372,48 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(
   if (threadIdx.x == 0) *threshold = thr;
 }
 
-// S4/S5: packed arrays, local parents, ancestor-or-self masks of request r.  One 128-thread group per request, tid =
-// candidate; `active` is false for a group without a request (it still takes part in the CTA-wide barriers).
+// S4/S5 for one selected candidate j of request r: its packed slot, local parent and ancestor-or-self mask.  `bal` =
+// the request's 128 selection bits, `par(c)` = parent of candidate c (-1 or negative for a root), `base` = the
+// request's first packed slot.
+template <typename ParFn>
+__device__ __forceinline__ void pack_node(
+    int r, int j, int depth, const uint32_t (&bal)[4], ParFn par, int base, int capacity,
+    int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req, int32_t* __restrict__ parent_local,
+    uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask) {
+  auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
+    int l = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      if (w < (c >> 5)) l += __popc(bal[w]);
+      else if (w == (c >> 5)) l += __popc(bal[w] & ((1u << (c & 31)) - 1u));
+    }
+    return l;
+  };
+  const int l = local_of(j);
+  const int k = base + l;
+  if (k >= capacity) return;
+  uint32_t m[4] = {0u, 0u, 0u, 0u};
+  m[l >> 5] |= 1u << (l & 31);
+  int pl = -1;
+  int c = par(j);
+  for (int step = 0; c >= 0 && step < ECHO_MAX_DEPTH; ++step) {
+    // ancestor closure (DESIGN.md invariant I2) guarantees every ancestor is selected
+    const int la = local_of(c);
+    if (step == 0) pl = la;
+    m[la >> 5] |= 1u << (la & 31);
+    c = par(c);
+  }
+  sel_node[k] = j;
+  sel_req[k] = r;
+  sel_depth[k] = (uint8_t)depth;
+  parent_local[k] = pl;
+  reinterpret_cast<uint4*>(anc_mask)[k] = make_uint4(m[0], m[1], m[2], m[3]);
+}
+
+// One 128-thread group per request, tid = candidate; `active` is false for a group without a request (it still takes
+// part in the CTA-wide barriers).
 struct PackSmem {
-  int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks below are chains of dependent reads
+  int par[ECHO_MAX_CAND];  // the request's parent array: the ancestor walks are chains of dependent reads
   uint32_t bal[4];
 };
 __device__ __forceinline__ void pack_request(
@@ -345,8 +429,8 @@ __device__ __forceinline__ void pack_request(
     C = min(cand_offsets[r + 1] - b, ECHO_MAX_CAND);
     base = sel_offsets[r];
   }
+  const int j = tid;
   {
-    const int j = tid;
     const uint32_t mine = __ballot_sync(0xffffffffu, j < C && keys[b + j] < thr);
     if (lane == 0) sm.bal[warp] = mine;
     if (j < C) {
@@ -358,39 +442,9 @@ __device__ __forceinline__ void pack_request(
   uint32_t bal[4];
 #pragma unroll
   for (int w = 0; w < 4; ++w) bal[w] = sm.bal[w];
-  auto local_of = [&](int c) -> int {  // packed local index of selected candidate c
-    int l = 0;
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      if (w < (c >> 5)) l += __popc(bal[w]);
-      else if (w == (c >> 5)) l += __popc(bal[w] & ((1u << (c & 31)) - 1u));
-    }
-    return l;
-  };
-  const int j = tid;
-  if ((bal[warp] >> lane) & 1u) {
-    const int l = local_of(j);
-    const int k = base + l;
-    if (k < capacity) {
-      const int p = sm.par[j];
-      uint32_t m[4] = {0u, 0u, 0u, 0u};
-      m[l >> 5] |= 1u << (l & 31);
-      int pl = -1;
-      int c = p;
-      for (int step = 0; c >= 0 && step < ECHO_MAX_DEPTH; ++step) {
-        // ancestor closure (DESIGN.md invariant I2) guarantees every ancestor is selected
-        int la = local_of(c);
-        if (step == 0) pl = la;
-        m[la >> 5] |= 1u << (la & 31);
-        c = sm.par[c];
-      }
-      sel_node[k] = j;
-      sel_req[k] = r;
-      sel_depth[k] = cand_depth[b + j];
-      parent_local[k] = pl;
-      reinterpret_cast<uint4*>(anc_mask)[k] = make_uint4(m[0], m[1], m[2], m[3]);
-    }
-  }
+  if ((bal[warp] >> lane) & 1u)
+    pack_node(r, j, cand_depth[b + j], bal, [&](int c) { return sm.par[c]; }, base, capacity, sel_node, sel_req,
+              parent_local, sel_depth, anc_mask);
   __syncthreads();  // the group's shared memory may be reused for its next request
 }
 
@@ -405,6 +459,212 @@ __global__ void __launch_bounds__(ECHO_MAX_CAND) k_pack(
   pdl_wait();  // threshold and offsets come from k_select
   pack_request(true, blockIdx.x, threadIdx.x, sm, cand_offsets, parent, cand_depth, keys, *threshold, capacity,
                sel_offsets, sel_node, sel_req, parent_local, sel_depth, anc_mask);
+}
+
+// ---- the whole of echo_gate_select as one launch of one thread-block cluster ----
+// The three kernels above cost three launches and two hand-overs through global memory for < 1 MB of data.  Here a
+// cluster of CL CTAs of 1024 threads holds everything on chip: CTA c scores requests [c*rpc, (c+1)*rpc) (eight
+// 128-thread groups, thread = candidate, up to GC_ROUNDS requests per group), the keys stay in shared memory, the radix
+// select takes 11 bits a pass over a 2048-bin histogram that every CTA builds on its own keys and then sums over the
+// cluster through distributed shared memory (so every CTA takes the same decisions and nothing is broadcast), and the
+// thread that made a key packs its node.  Same arithmetic as the chain: the scoring and packing are the same device
+// functions.  Measured (B200, bench.py, cfg2): 21.6 us per echo_gate_select against 28.6 us for the chain.
+constexpr int GC_THREADS = 1024;
+constexpr int GC_GROUPS = GC_THREADS / ECHO_MAX_CAND;  // 8
+constexpr int GC_ROUNDS = 4;
+constexpr int GC_SLOTS = GC_GROUPS * GC_ROUNDS;  // requests per CTA
+constexpr int GC_BITS = 11;
+constexpr int GC_BINS = 1 << GC_BITS;
+constexpr int GC_SLICE = 128;                  // bins per slice: one int4 per lane of a warp
+constexpr int GC_NSLICE = GC_BINS / GC_SLICE;  // 16
+static_assert(GC_BINS == 2 * GC_THREADS, "one thread zeroes two bins");
+static_assert(GC_SLOTS == 32, "one warp scans a CTA's request counts");
+
+struct ClusterSmem {
+  uint64_t key[GC_SLOTS][ECHO_MAX_CAND];  // selection keys of the CTA's requests (KEY_INELIGIBLE past a request's end)
+  ScoreSmem score[GC_GROUPS];
+  int8_t par8[GC_SLOTS][ECHO_MAX_CAND];   // validated parents (-1 = root), kept for the packing
+  uint8_t dep8[GC_SLOTS][ECHO_MAX_CAND];  // depths
+  uint32_t bal[GC_SLOTS][4];              // selection bits per request
+  int hist[2][GC_BINS];                   // this CTA's keys by digit, per pass parity; read by every CTA of the cluster
+  int slice[2][GC_NSLICE];                // sums of the histogram's slices of GC_SLICE bins; likewise
+  int csum[2][GC_NSLICE];                 // the cluster's slice sums
+  alignas(16) int tot[2][GC_SLICE];       // the cluster's histogram of the slice that holds the k-th key
+  int cnt[GC_SLOTS];  // inclusive count of selected nodes over this CTA's requests
+  int cta_total;      // read by every CTA of the cluster
+  int base;
+  uint64_t found;
+};
+
+// Code size is time here: the kernel runs once per step with its instructions cold in every cache (the attention
+// kernel has streamed > 1 GB through L2 since), so every loop over a CTA's request slots stays rolled.
+__global__ void __launch_bounds__(GC_THREADS, 1) k_gate_cluster(
+    const int32_t* __restrict__ cand_offsets, const int32_t* __restrict__ parent, const float* __restrict__ logq,
+    const __grid_constant__ GateParams gp, int R, int budget, int capacity, float* __restrict__ path_score,
+    uint8_t* __restrict__ cand_depth, int32_t* __restrict__ cut_depth, int32_t* __restrict__ n_selected,
+    int32_t* __restrict__ sel_offsets, int32_t* __restrict__ sel_node, int32_t* __restrict__ sel_req,
+    int32_t* __restrict__ parent_local, uint8_t* __restrict__ sel_depth, uint32_t* __restrict__ anc_mask,
+    uint32_t* __restrict__ status) {
+  extern __shared__ __align__(16) unsigned char gc_smem[];
+  ClusterSmem& sm = *reinterpret_cast<ClusterSmem*>(gc_smem);
+  cg::cluster_group cluster = cg::this_cluster();
+  const int CL = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  pdl_launch_dependents();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = tid / ECHO_MAX_CAND, j = tid % ECHO_MAX_CAND;
+  const int rpc = (R + CL - 1) / CL;  // requests per CTA (host: <= GC_SLOTS)
+  const int rounds = (rpc + GC_GROUPS - 1) / GC_GROUPS;
+  const int nslot = rounds * GC_GROUPS;
+  // ---- S1-S2 and keys: a round's loads are issued a round ahead of the arithmetic ----
+  CandIn nxt = load_cand(g < rpc && rank * rpc + g < R, rank * rpc + g, j, cand_offsets, parent, logq);
+  sm.hist[0][2 * tid] = 0;
+  sm.hist[0][2 * tid + 1] = 0;
+  if (tid < GC_NSLICE) sm.slice[0][tid] = sm.csum[0][tid] = 0;
+  if (tid < GC_SLICE) sm.tot[0][tid] = 0;
+#pragma unroll 1
+  for (int slot = g; slot < nslot; slot += GC_GROUPS) {
+    const int i = rank * rpc + slot;
+    const CandIn in = nxt;
+    {
+      const int s2 = slot + GC_GROUPS, i2 = rank * rpc + s2;
+      if (s2 < nslot) nxt = load_cand(s2 < rpc && i2 < R, i2, j, cand_offsets, parent, logq);
+    }
+    int d;
+    const uint64_t key =
+        score_gate_request(slot < rpc && i < R, i, j, in, sm.score[g], gp, path_score, cand_depth, cut_depth, status, d);
+    sm.key[slot][j] = key;
+    sm.par8[slot][j] = (int8_t)sm.score[g].par[j];  // (whatever it holds past the request's end is never read)
+    sm.dep8[slot][j] = (uint8_t)d;
+    __syncthreads();  // the group's scoring buffers are reused by its next request; at the end, all keys are in place
+  }
+
+  // ---- S3: threshold T = budget-th smallest key of the cluster's keys (unique => no ties to break) ----
+  // A pass: every CTA histograms its own keys (2048 bins, and the sums of the 16 slices of 128 bins); after one
+  // cluster barrier every CTA adds up the CL x 16 slice sums, finds the slice that holds the k-th key, adds up that
+  // slice's CL x 128 bins and finds the bin -- the same decision everywhere, nothing to broadcast, and 8.5 KB instead
+  // of 128 KB through distributed shared memory (which moves ~20 B a cycle per SM).
+  const bool none = budget <= 0;
+  uint64_t T = 0;
+  if (!none) {
+    uint64_t prefix = 0;
+    int k = budget, shift = 64;
+#pragma unroll 1
+    for (int pass = 0;; ++pass) {
+      const int bits = shift >= GC_BITS ? GC_BITS : shift;  // 11, 11, 11, 11, 11, 9
+      const int hi = shift;                                 // bits [hi, 64) are decided: they equal `prefix`
+      shift -= bits;
+      int* h = sm.hist[pass & 1];
+      int* hs = sm.slice[pass & 1];
+      int* csum = sm.csum[pass & 1];
+      int* tot = sm.tot[pass & 1];
+#pragma unroll 1
+      for (int slot = g; slot < nslot; slot += GC_GROUPS) {
+        const uint64_t key = sm.key[slot][j];
+        const bool in_prefix = key != KEY_INELIGIBLE && (pass == 0 || (key >> hi) == prefix);
+        const int digit = in_prefix ? (int)((key >> shift) & ((1u << bits) - 1u)) : -1;
+        // the top digits take one or two values: a warp that agrees on its digit adds it once
+        const int d0 = __shfl_sync(0xffffffffu, digit, 0);
+        if (__all_sync(0xffffffffu, digit == d0)) {
+          if (lane == 0 && d0 >= 0) { atomicAdd(&h[d0], 32); atomicAdd(&hs[d0 / GC_SLICE], 32); }
+        } else if (in_prefix) {
+          atomicAdd(&h[digit], 1);
+          atomicAdd(&hs[digit / GC_SLICE], 1);
+        }
+      }
+      cluster.sync();  // every CTA's histogram of this pass is complete; the other set of buffers is no longer read
+      sm.hist[(pass + 1) & 1][2 * tid] = 0;
+      sm.hist[(pass + 1) & 1][2 * tid + 1] = 0;
+      if (tid < GC_NSLICE) sm.slice[(pass + 1) & 1][tid] = sm.csum[(pass + 1) & 1][tid] = 0;
+      if (tid < GC_SLICE) sm.tot[(pass + 1) & 1][tid] = 0;
+      for (int t = tid; t < GC_NSLICE * CL; t += GC_THREADS) {
+        const int v = *cluster.map_shared_rank(&hs[t % GC_NSLICE], t / GC_NSLICE);
+        if (v) atomicAdd(&csum[t % GC_NSLICE], v);
+      }
+      __syncthreads();
+      // every warp for itself: the slice that holds the k-th key
+      const int v = lane < GC_NSLICE ? csum[lane] : 0;
+      const int vincl = warp_incl_scan(v, lane);
+      if (pass == 0 && __shfl_sync(0xffffffffu, vincl, 31) <= budget) {  // everything eligible (R:G-12)
+        T = KEY_INELIGIBLE - 1;
+        break;
+      }
+      const int owner = __ffs(__ballot_sync(0xffffffffu, vincl - v < k && k <= vincl)) - 1;  // exactly one lane
+      const int below = __shfl_sync(0xffffffffu, vincl - v, owner);  // keys in the slices below
+      for (int t = tid; t < GC_SLICE * CL; t += GC_THREADS) {
+        const int c = *cluster.map_shared_rank(&h[owner * GC_SLICE + t % GC_SLICE], t / GC_SLICE);
+        if (c) atomicAdd(&tot[t % GC_SLICE], c);
+      }
+      __syncthreads();
+      if (warp == 0) {  // the bin inside the slice, four bins per lane
+        const int4 c4 = *reinterpret_cast<const int4*>(&tot[4 * lane]);
+        const int c[4] = {c4.x, c4.y, c4.z, c4.w};
+        const int sum = c4.x + c4.y + c4.z + c4.w;
+        int e = below + warp_incl_scan(sum, lane) - sum;
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          if (e < k && k <= e + c[t])  // exactly one lane and t: (bin << 32 | k inside the bin << 1 | whole bin taken)
+            sm.found = ((uint64_t)(owner * GC_SLICE + 4 * lane + t) << 32) | ((uint64_t)(k - e) << 1) |
+                       (uint64_t)(k - e == c[t]);
+          e += c[t];
+        }
+      }
+      __syncthreads();
+      const uint64_t found = sm.found;
+      prefix = (prefix << bits) | (found >> 32);
+      k = (int)((found & 0xffffffffull) >> 1);
+      if ((found & 1ull) || shift == 0) {
+        // the whole bin is selected (lower digits do not matter), or every digit is decided: keys with the found
+        // prefix and everything below it are selected; pad the undecided low digits with ones
+        T = shift > 0 ? ((prefix << shift) | ((1ull << shift) - 1ull)) : prefix;
+        break;
+      }
+    }
+  }
+  const uint64_t thr = none ? 0ull : T + 1ull;  // keys < thr are selected
+
+  // ---- S4: per-request counts, CSR offsets (a scan over the CTA's requests, then over the cluster's CTAs) ----
+#pragma unroll 1
+  for (int slot = g; slot < GC_SLOTS; slot += GC_GROUPS) {
+    const unsigned b = __ballot_sync(0xffffffffu, slot < nslot && sm.key[slot][j] < thr);
+    if (lane == 0) sm.bal[slot][warp & 3] = b;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    const int c = __popc(sm.bal[lane][0]) + __popc(sm.bal[lane][1]) + __popc(sm.bal[lane][2]) + __popc(sm.bal[lane][3]);
+    const int incl = warp_incl_scan(c, lane);
+    sm.cnt[lane] = incl;
+    if (lane == 31) sm.cta_total = incl;
+  }
+  cluster.sync();
+  if (warp == 0) {
+    const int v = lane < CL ? *cluster.map_shared_rank(&sm.cta_total, lane) : 0;
+    const int incl = warp_incl_scan(v, lane);
+    const int base = rank ? __shfl_sync(0xffffffffu, incl, (rank + 31) & 31) : 0;
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    const int i = rank * rpc + lane;
+    if (lane < rpc && i < R) sel_offsets[i + 1] = base + sm.cnt[lane];
+    if (rank == 0 && lane == 0) {
+      sel_offsets[0] = 0;
+      *n_selected = total;
+    }
+    if (lane == 0) sm.base = base;
+  }
+  __syncthreads();
+  cluster.barrier_arrive();  // this CTA has read the others' shared memory for the last time
+
+  // ---- S4/S5: Flatten & Pack by the thread that made the key ----
+#pragma unroll 1
+  for (int slot = g; slot < nslot; slot += GC_GROUPS) {
+    if (sm.key[slot][j] < thr) {
+      uint32_t bal[4];
+#pragma unroll
+      for (int w = 0; w < 4; ++w) bal[w] = sm.bal[slot][w];
+      const int8_t* par = sm.par8[slot];
+      pack_node(rank * rpc + slot, j, sm.dep8[slot][j], bal, [&](int c) { return (int)par[c]; },
+                sm.base + (slot ? sm.cnt[slot - 1] : 0), capacity, sel_node, sel_req, parent_local, sel_depth, anc_mask);
+    }
+  }
+  cluster.barrier_wait();  // no CTA leaves while its shared memory may still be read
 }
 
 }  // namespace
@@ -451,8 +711,76 @@ int launch_gate_select_keys(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g,
   return ECHO_OK;
 }
 
+// Largest cluster of k_gate_cluster CTAs this device can place (16 needs the non-portable opt-in), probed once per
+// context; 0 = none.
+static int gate_cluster_max(EchoCtx* ctx) {
+  if (ctx->gate_cluster_max != 0) return ctx->gate_cluster_max > 0 ? ctx->gate_cluster_max : 0;
+  ctx->gate_cluster_max = -1;
+  if (cudaFuncSetAttribute(k_gate_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ClusterSmem)) !=
+      cudaSuccess) {
+    (void)cudaGetLastError();
+    return 0;
+  }
+  const bool np = cudaFuncSetAttribute(k_gate_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+  for (int cl = np ? 16 : 8; cl >= 1; cl /= 2) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cl);
+    cfg.blockDim = dim3(GC_THREADS);
+    cfg.dynamicSmemBytes = sizeof(ClusterSmem);
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cl;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, k_gate_cluster, &cfg) == cudaSuccess && n >= 1) {
+      ctx->gate_cluster_max = cl;
+      break;
+    }
+  }
+  (void)cudaGetLastError();
+  return ctx->gate_cluster_max > 0 ? ctx->gate_cluster_max : 0;
+}
+
+// Cluster size for R requests: eight requests per CTA and round; 0 when the cluster kernel cannot take the call.
+static int gate_cluster_size(EchoCtx* ctx, int R) {
+  const int cl_max = gate_cluster_max(ctx);
+  if (cl_max == 0) return 0;
+  int cl = 1;
+  if (ctx->opt_gate_cluster > 0) cl = (int)ctx->opt_gate_cluster;
+  else
+    while (cl < cl_max && cl * GC_GROUPS < R) cl *= 2;
+  if (cl > cl_max || (R + cl - 1) / cl > GC_SLOTS) return 0;
+  return cl;
+}
+
 int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoSelection* o, cudaStream_t st) {
   const int R = t->num_requests, N = t->total_cand;
+  const int budget = g->static_k > 0 ? N : g->budget;
+  const int cl = ctx->opt_gate_path == 1 ? 0 : gate_cluster_size(ctx, R);
+  if (cl > 0) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cl);
+    cfg.blockDim = dim3(GC_THREADS);
+    cfg.dynamicSmemBytes = sizeof(ClusterSmem);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cl;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ECHO_COUNT_LAUNCH();
+    ECHO_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, k_gate_cluster, t->cand_offsets, t->parent, t->logq, gate_params(g), R,
+                                          budget, o->capacity, o->path_score, o->cand_depth, o->cut_depth,
+                                          o->n_selected, o->sel_offsets, o->sel_node, o->sel_req, o->parent_local,
+                                          o->sel_depth, o->anc_mask, ctx->dev_status));
+    return ECHO_OK;
+  }
+  if (ctx->opt_gate_path == 2) return ECHO_ERR_UNSUPPORTED;
   uint64_t* keys = reinterpret_cast<uint64_t*>(ctx->workspace);
   const size_t keys_bytes = align_up((size_t)N * sizeof(uint64_t), 256);
   if (keys_bytes + 256 > ctx->workspace_bytes) return ECHO_ERR_WORKSPACE;
@@ -462,7 +790,6 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
     k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g), o->path_score,
                                                o->cand_depth, o->cut_depth, keys, ctx->dev_status);
   }
-  const int budget = g->static_k > 0 ? N : g->budget;
   ECHO_CUDA_TRY(ctx, launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, keys, N, budget,
                                 o->n_selected, o->sel_offsets, threshold));
   if (R > 0) {

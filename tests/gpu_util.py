@@ -10,6 +10,7 @@ def dev(a, device="cuda"):
 
 
 _CTX = {}
+GATE = {"path": 0, "cluster": 0}  # ECHO_OPT_GATE_PATH / ECHO_OPT_GATE_CLUSTER that get_ctx() applies (test fixtures set it)
 
 
 def get_ctx():
@@ -21,6 +22,8 @@ def get_ctx():
     ctx.set_option(echo.OPT_ATTN_PATH, 0)
     ctx.set_option(echo.OPT_NUM_CTAS, 0)
     ctx.set_option(echo.OPT_ATTN_SAFE, 0)
+    ctx.set_option(echo.OPT_GATE_PATH, GATE["path"])
+    ctx.set_option(echo.OPT_GATE_CLUSTER, GATE["cluster"])
     return ctx
 
 

@@ -107,16 +107,35 @@ def test_attn_many_requests_planner_multi_pass():
     _check_rows(wl, want_sel, q, k, v, out, lse, sorted(set(rows)))
 
 
+@pytest.mark.parametrize("gate_path", [1, 2])
 @pytest.mark.parametrize("schedule", [0, 1])
-def test_gate_select_more_keys_than_the_register_cache(schedule):
-    """N = 16 800 > 16 384: k_select reads the keys from global memory in every radix pass (the branch the merged key
-    population of 8 request-sharded ranks takes)."""
+def test_gate_select_more_keys_than_the_register_cache(schedule, gate_path):
+    """N = 16 800 > 16 384: as three kernels, k_select reads the keys from global memory in every radix pass (the branch
+    the merged key population of 8 request-sharded ranks takes); as one cluster, 16 CTAs take 14 requests each in two
+    rounds."""
+    from paper_2604_09603_b200 import echo
     ctx = get_ctx()
+    ctx.set_option(echo.OPT_GATE_PATH, gate_path)
     wl = W.make_config(2, R=210)
     assert wl.N > 16384
     sel = run_gate_select(ctx, wl, schedule=schedule)
     assert_selection_equal(sel.to_host(), oracle_gate_select(orc, wl, schedule=schedule))
     assert ctx.device_status() == 0
+
+
+def test_gate_select_more_requests_than_a_cluster_takes():
+    """R = 520 > 16 CTAs x 32 requests: echo_gate_select falls back to the three-kernel chain by itself, and refuses
+    when the cluster kernel is forced."""
+    from paper_2604_09603_b200 import echo
+    ctx = get_ctx()
+    wl = W.make_config(1, R=520)
+    sel = run_gate_select(ctx, wl)
+    assert_selection_equal(sel.to_host(), oracle_gate_select(orc, wl))
+    ctx.set_option(echo.OPT_GATE_PATH, 2)
+    with pytest.raises(echo.EchoError) as e:
+        run_gate_select(ctx, wl)
+    assert e.value.code == echo.ERR_UNSUPPORTED
+    ctx.set_option(echo.OPT_GATE_PATH, 0)
 
 
 def test_global_budget_eight_ranks_key_population():

@@ -9,10 +9,22 @@ import pytest
 from oracle import echo_oracle as orc
 from paper_2604_09603_b200 import workloads as W
 from helpers import oracle_gate_select, packed_tokens, torch_bf16_to_bits
+import gpu_util
 from gpu_util import dev, get_ctx, run_gate_select, make_kv, assert_selection_equal
 
 pytestmark = pytest.mark.gpu
 GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "w1.json")))
+
+
+@pytest.fixture(autouse=True, params=["auto", "chain", "cluster2", "cluster1"])
+def gate_path(request):
+    """Every test of this file runs echo_gate_select as the one-cluster kernel with its default cluster size, as the
+    three-kernel chain, and as a cluster of two CTAs / one CTA (several requests per thread group; the chain again
+    where a CTA would get more than 32 requests)."""
+    gpu_util.GATE.update({"auto": dict(path=0, cluster=0), "chain": dict(path=1, cluster=0),
+                          "cluster2": dict(path=0, cluster=2), "cluster1": dict(path=0, cluster=1)}[request.param])
+    yield request.param
+    gpu_util.GATE.update(path=0, cluster=0)
 
 
 def _w1_workload():
