@@ -123,6 +123,7 @@ __device__ long long g_trace[256][8];
 #define PROF_SPAN_END(slot) prof_[slot] += clock64() - span_t_
 #define PROF_COUNT(slot) prof_[slot] += 1
 #define TRACE(gg, ev) do { if (blockIdx.x == 0 && (gg) < 256 && lane == 0) g_trace[gg][ev] = clock64(); } while (0)
+#define TRACE_K(ev) do { if (blockIdx.x == 0 && threadIdx.x == 0) g_trace[255][ev] = clock64(); } while (0)
 #define PROF_SPAN2_BEGIN() const long long span2_t_ = clock64()
 #define PROF_SPAN2_END(slot) prof_[slot] += clock64() - span2_t_
 #else
@@ -139,6 +140,7 @@ __device__ long long g_trace[256][8];
 #define PROF_SPAN2_BEGIN() do {} while (0)
 #define PROF_SPAN2_END(slot) do {} while (0)
 #define TRACE(gg, ev) do {} while (0)
+#define TRACE_K(ev) do {} while (0)
 #endif
 
 // work item record written by k_plan: two int4 = {req, kvh | rt<<8 | split<<16, jt0, jt1} {P_i, sel_offsets[i], K_i, 0}
@@ -289,16 +291,23 @@ __device__ __forceinline__ float acc_total(const uint64_t (&acc)[4]) {
 __device__ __forceinline__ void tile_weights_fast(uint32_t tS, float scale_log2, float neg_m, float& ts) {
   const uint64_t sc2 = tc::pack_f32x2(scale_log2, scale_log2), nm2 = tc::pack_f32x2(neg_m, neg_m);
   uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};  // 8 independent fp32 partial sums
-  uint32_t s[2][32];
-  tc::tmem_ld32(tS, s[0]);
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    tc::tmem_wait_ld();
-    tc::reg_fence32(s[c & 1]);
-    if (c < 3) tc::tmem_ld32(tS + 32 * (c + 1), s[(c + 1) & 1]);
+  uint32_t s0[32], s1[32];
+  tc::tmem_ld32(tS, s0);
+  // two chunks per trip (the two register buffers by name), the loop itself rolled: half the code of the kernel's
+  // hottest path -- the whole kernel has to live in a 32 KB instruction cache next to the per-item code
+#pragma unroll 1
+  for (int c = 0; c < 4; c += 2) {
     uint32_t pk[16];
-    weights_chunk(s[c & 1], sc2, nm2, pk, acc);
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s0);
+    tc::tmem_ld32(tS + 32 * (c + 1), s1);
+    weights_chunk(s0, sc2, nm2, pk, acc);
     tc::tmem_st16(tS + 16 * c, pk);  // P columns [16c, 16c+16) lie inside S chunks already read (c/2 <= c)
+    tc::tmem_wait_ld();
+    tc::reg_fence32(s1);
+    if (c == 0) tc::tmem_ld32(tS + 64, s0);
+    weights_chunk(s1, sc2, nm2, pk, acc);
+    tc::tmem_st16(tS + 16 * (c + 1), pk);
   }
   ts = acc_total(acc);
 }
@@ -374,6 +383,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cta = blockIdx.x, grid = gridDim.x;
+  TRACE_K(0);
   pdl_launch_dependents();  // echo_accept's kernel may queue behind this one (it waits for our completion itself)
 
   if (threadIdx.x == 0) {
@@ -395,9 +405,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem = *tmem_slot;
+  TRACE_K(1);
   // Programmatic dependent launch: everything above (barrier init, TMEM allocation, descriptor prefetch) overlaps
   // k_plan; the work list is read only after k_plan has completed.
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  TRACE_K(2);
   const int n_items = *p.n_items;
   const bool force_safe = p.force_safe != 0;
 
@@ -619,6 +631,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
 #endif
     auto do_item = [&](const Item& it, const uint4& mk, const bool safe) {
       const int P = it.P, total = it.P + it.Ki;
+      // A warp none of whose 32 rows belongs to a node (the last row tile of a request is ragged: a quarter to a third
+      // of all row-warps at the configs of BASELINE.json) computes nothing -- whatever its TMEM lanes hold goes through
+      // PV into O rows that are never stored -- but keeps every barrier's pace: it waits for S like the others (so it
+      // cannot run a phase ahead of P-full), helps zero the ragged V rows, and arrives.
+      const bool idle = ((it.rt * TILE_M + wq * 32) >> p.log2G) >= it.Ki;
       float m_used = safe ? -INFINITY : 0.f, lsum = 0.f, lnorm = 0.f;
       const uint32_t tO = tmem + TMEM_O + lane_addr;
       // fast form: warpgroup w takes the tiles with g & 1 == w; safe form: warpgroup 0 takes all of them
@@ -634,8 +651,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         PROF_WAIT(1, bar(B_SFULL + b), (g / NSBUF) & 1);
         PROF_SPAN_BEGIN();
         if (wq == 0) TRACE(g, 2);
-        tc::tc_fence_after();
         const int tile0 = j * TILE_N;
+        if (!idle) {
+        tc::tc_fence_after();
         const bool masked = tile0 + TILE_N > P;  // the tile touches tree positions or the ragged end
         uint32_t vis[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
         if (masked) {
@@ -683,6 +701,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
         lsum += ts;
         lnorm += tr;
         tc::tmem_wait_st();
+        }
         if (tile0 + TILE_N > total) {  // ragged end: V rows past the last token may hold anything (R:A-7)
           const int slot = g % NSTAGE;
           PROF_WAIT(4, bar(B_VFULL + slot), (g / NSTAGE) & 1);
@@ -835,6 +854,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   // ---- teardown ----
   tc::tc_fence_before();
   __syncthreads();
+  TRACE_K(3);
   if (warp == W_MMA_QK) tc::tmem_dealloc(tmem, TMEM_COLS);
 }
 
