@@ -40,7 +40,8 @@ typedef void* echo_stream_t;     /* a cudaStream_t, e.g. torch.cuda.current_stre
 typedef enum {
   ECHO_OK = 0,
   ECHO_ERR_INVALID_ARG = -1, /* NULL pointer, negative size, capacity too small, misaligned pointer */
-  ECHO_ERR_UNSUPPORTED = -2, /* head_dim != 128, page_size != 16, Hq % Hkv != 0, max_cand_per_req > 128 */
+  ECHO_ERR_UNSUPPORTED = -2, /* head_dim != 128, page_size != 16, Hq % Hkv != 0, max_cand_per_req > 128, ECHO_SCHED_ALG1 with more
+                                than 2^24 requests over the ranks sharing a budget */
   ECHO_ERR_WORKSPACE = -3,   /* ctx workspace smaller than echo_workspace_bytes(...) for this call */
   ECHO_ERR_ARCH = -4,        /* device is not sm_100 */
   ECHO_ERR_CUDA = -5         /* a CUDA runtime / driver call failed; text via echo_last_error */

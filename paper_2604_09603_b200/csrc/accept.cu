@@ -93,24 +93,37 @@ __global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
     int32_t* __restrict__ accept_idx, int32_t* __restrict__ slot_src, int32_t* __restrict__ slot_dst) {
   __shared__ int s_L;
   __shared__ int s_src[ECHO_MAX_ACCEPT], s_dst[ECHO_MAX_ACCEPT];
-  pdl_wait();  // the attention kernel before this one reads the pools this kernel compacts in place
   const int i = blockIdx.x;
-  const int b = sel_offsets[i], Ki = min(sel_offsets[i + 1] - b, ECHO_MAX_CAND);
+  // what the caller owns (not written by this step's kernels) is loaded while the attention kernel drains
   const int P = prefix_len[i];
+  const int prev = prev_token[i];
+  pdl_wait();  // the attention kernel before this one reads the pools this kernel compacts in place
+  const int b = sel_offsets[i], Ki = min(sel_offsets[i + 1] - b, ECHO_MAX_CAND);
   const int32_t* pt = page_table + (size_t)i * max_pages;
   if (threadIdx.x < 32) {
     const int lane = threadIdx.x;
-    const int prev = prev_token[i];
+    // every load of the decision is issued before the first one is used: one memory round trip, then one more for
+    // the parents' target tokens
+    int pl[4], dr[4], dep[4];
+    uint4 am[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int l = w * 32 + lane;
+      pl[w] = -1; dr[w] = 0; dep[w] = 0; am[w] = make_uint4(0u, 0u, 0u, 0u);
+      if (l < Ki) {
+        pl[w] = parent_local[b + l];
+        dr[w] = draft_token[b + l];
+        dep[w] = sel_depth[b + l];
+        am[w] = reinterpret_cast<const uint4*>(anc_mask)[b + l];
+      }
+    }
     // match[l]: draft token equals the target's greedy token after the parent (roots: prev_token)
     uint32_t match[4];
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
       const int l = w * 32 + lane;
       bool mt = false;
-      if (l < Ki) {
-        const int pl = parent_local[b + l];
-        mt = draft_token[b + l] == (pl < 0 ? prev : target_token[b + pl]);
-      }
+      if (l < Ki) mt = dr[w] == (pl[w] < 0 ? prev : target_token[b + pl[w]]);
       match[w] = __ballot_sync(0xffffffffu, mt);
     }
     // acc[l] <=> every ancestor-or-self matches; best = max depth, then lowest l (R:C-4)
@@ -119,9 +132,9 @@ __global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
     for (int w = 0; w < 4; ++w) {
       const int l = w * 32 + lane;
       if (l < Ki) {
-        const uint4 m = reinterpret_cast<const uint4*>(anc_mask)[b + l];
+        const uint4 m = am[w];
         const bool acc = !((m.x & ~match[0]) | (m.y & ~match[1]) | (m.z & ~match[2]) | (m.w & ~match[3]));
-        if (acc) best_key = max(best_key, ((int)sel_depth[b + l] << 8) | (ECHO_MAX_CAND - 1 - l));
+        if (acc) best_key = max(best_key, (dep[w] << 8) | (ECHO_MAX_CAND - 1 - l));
       }
     }
 #pragma unroll
@@ -129,7 +142,9 @@ __global__ void __launch_bounds__(AC_THREADS) k_accept_compact(
     int L = 0;
     if (best_key >= 0) {
       const int best = ECHO_MAX_CAND - 1 - (best_key & 0xff);
-      const uint4 m = reinterpret_cast<const uint4*>(anc_mask)[b + best];
+      uint4 m = (best >> 5) == 0 ? am[0] : (best >> 5) == 1 ? am[1] : (best >> 5) == 2 ? am[2] : am[3];  // warp-uniform
+      m.x = __shfl_sync(0xffffffffu, m.x, best & 31); m.y = __shfl_sync(0xffffffffu, m.y, best & 31);
+      m.z = __shfl_sync(0xffffffffu, m.z, best & 31); m.w = __shfl_sync(0xffffffffu, m.w, best & 31);
       const uint32_t mw[4] = {m.x, m.y, m.z, m.w};
       L = min(__popc(m.x) + __popc(m.y) + __popc(m.z) + __popc(m.w), ECHO_MAX_ACCEPT);
       // lane t finds the t-th set bit (path order = ascending local index, R:P-1)

@@ -165,6 +165,8 @@ static int check_gate(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, EchoS
   if (g->cand_index_base < 0 || g->request_base < 0) return ECHO_ERR_INVALID_ARG;
   if (g->schedule != ECHO_SCHED_TOPB && g->schedule != ECHO_SCHED_ALG1) return ECHO_ERR_INVALID_ARG;
   if (t->max_cand_per_req > ECHO_MAX_CAND) return ECHO_ERR_UNSUPPORTED;
+  // ECHO_SCHED_ALG1 keys carry the global request index in 24 bits
+  if (g->schedule == ECHO_SCHED_ALG1 && (int64_t)g->request_base + t->num_requests > (1 << 24)) return ECHO_ERR_UNSUPPORTED;
   if (!t->cand_offsets || !o->cut_depth) return ECHO_ERR_INVALID_ARG;
   if (t->total_cand > 0 && (!t->parent || !t->logq || !o->path_score || !o->cand_depth)) return ECHO_ERR_INVALID_ARG;
   if (!need_packed) return ECHO_OK;

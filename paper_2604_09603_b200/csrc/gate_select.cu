@@ -53,8 +53,10 @@ __device__ __forceinline__ uint64_t make_key(int tier, float S, int g) {
 // truncated, the W_max best nodes of the truncation level) are, read as one sequence, the eligible nodes sorted by
 // (phase, depth, request, rank in level); taking the first K_max of that order is the algorithm, including the
 // level that only partly fits (readings R:L-1..L-4).
+// The fields sit at the top of the key (1 + 5 + 24 + 8 bits: depth < 32, request < 2^24 -- checked by the host --,
+// rank < 128), so the radix select is through after the first 38 bits.
 __device__ __forceinline__ uint64_t make_key_alg1(int phase, int depth, int request, int rank) {
-  return ((uint64_t)phase << 63) | ((uint64_t)depth << 56) | ((uint64_t)(uint32_t)request << 16) | (uint64_t)rank;
+  return ((uint64_t)phase << 63) | ((uint64_t)depth << 58) | ((uint64_t)(uint32_t)request << 34) | ((uint64_t)rank << 26);
 }
 
 // Shared memory of one request's scoring (one 128-thread group)

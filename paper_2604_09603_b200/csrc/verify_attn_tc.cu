@@ -869,14 +869,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) k_plan(const int32_t* __restrict
   __shared__ int s_cnt[PLAN_BUCKETS];
   __shared__ int s_warp[32];
   pdl_launch_dependents();  // let k_verify_attn_tc set itself up meanwhile
-  pdl_wait();               // sel_offsets come from echo_gate_select's kernels
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int b = tid; b < PLAN_BUCKETS; b += PLAN_THREADS) s_cnt[b] = 0;
   if (tid < 32) s_warp[tid] = 0;
+  const int P_first = tid < R ? prefix_len[tid] : 0;  // the caller's: loaded while the kernel before this one drains
+  pdl_wait();                                        // sel_offsets come from echo_gate_select's kernels
   __syncthreads();
   auto for_items = [&](auto&& fn) {
     for (int r = tid; r < R; r += PLAN_THREADS) {
-      const int off = sel_offsets[r], P = prefix_len[r];
+      const int off = sel_offsets[r], P = r == tid ? P_first : prefix_len[r];
       int Ki = sel_offsets[r + 1] - off;
       if (Ki <= 0) continue;
       if (Ki > ECHO_MAX_CAND) {  // more packed nodes than a request can have: clamp and flag (never silently truncate)

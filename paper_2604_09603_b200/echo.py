@@ -180,11 +180,20 @@ class Selection:
     cand_depth: "torch.Tensor"
     cut_depth: "torch.Tensor"
 
+    def __setattr__(self, name, value):  # a field that changes drops the marshalled struct
+        self.__dict__.pop("_cs", None)
+        object.__setattr__(self, name, value)
+
     def c_struct(self) -> EchoSelection:
-        return EchoSelection(self.capacity, _ptr(self.n_selected), _ptr(self.sel_offsets), _ptr(self.sel_node),
-                             _ptr(self.sel_req), _ptr(self.parent_local), _ptr(self.sel_depth),
-                             _ptr(self.anc_mask), _ptr(self.path_score), _ptr(self.cand_depth),
-                             _ptr(self.cut_depth))
+        """the C struct of these tensors, marshalled once (per-call marshalling is what bounds small batches)"""
+        cs = self.__dict__.get("_cs")
+        if cs is None:
+            cs = EchoSelection(self.capacity, _ptr(self.n_selected), _ptr(self.sel_offsets), _ptr(self.sel_node),
+                               _ptr(self.sel_req), _ptr(self.parent_local), _ptr(self.sel_depth),
+                               _ptr(self.anc_mask), _ptr(self.path_score), _ptr(self.cand_depth),
+                               _ptr(self.cut_depth))
+            self.__dict__["_cs"] = cs
+        return cs
 
     def to_host(self) -> dict:
         """numpy copies trimmed to n_selected (synchronises)."""
@@ -204,10 +213,20 @@ class PagedKV:
     page_table: "torch.Tensor"  # int32 [R][max_pages]
     prefix_len: "torch.Tensor"  # int32 [R]
 
-    def c_struct(self) -> EchoPagedKV:
-        L, NP, Hkv, PS, Dh = self.k_pool.shape
-        return EchoPagedKV(Hkv, Dh, PS, NP, self.page_table.shape[1], L, _ptr(self.k_pool), _ptr(self.v_pool),
-                           _ptr(self.page_table), _ptr(self.prefix_len))
+    def __setattr__(self, name, value):  # a field that changes drops the marshalled structs
+        self.__dict__.pop("_cs", None)
+        object.__setattr__(self, name, value)
+
+    def c_struct(self, with_pools: bool = True) -> EchoPagedKV:
+        """the C struct of these tensors (pool pointers NULL if not with_pools), marshalled once"""
+        cs = self.__dict__.get("_cs")
+        if cs is None:
+            L, NP, Hkv, PS, Dh = self.k_pool.shape
+            args = (Hkv, Dh, PS, NP, self.page_table.shape[1], L)
+            tail = (_ptr(self.page_table), _ptr(self.prefix_len))
+            cs = (EchoPagedKV(*args, None, None, *tail), EchoPagedKV(*args, _ptr(self.k_pool), _ptr(self.v_pool), *tail))
+            self.__dict__["_cs"] = cs
+        return cs[1 if with_pools else 0]
 
 
 @dataclass
@@ -220,6 +239,20 @@ class Acceptance:
     slot_src: "torch.Tensor"
     slot_dst: "torch.Tensor"
     target_token: Optional["torch.Tensor"]
+
+    def __setattr__(self, name, value):  # a field that changes drops the marshalled structs
+        self.__dict__.pop("_cs", None)
+        object.__setattr__(self, name, value)
+
+    def c_struct(self, with_target: bool) -> EchoAccept:
+        """the C struct of these tensors (target_token_out NULL unless with_target), marshalled once"""
+        cs = self.__dict__.get("_cs")
+        if cs is None:
+            head = (_ptr(self.accept_len), _ptr(self.last_node), _ptr(self.bonus_token), _ptr(self.new_len),
+                    _ptr(self.accept_idx), _ptr(self.slot_src), _ptr(self.slot_dst))
+            cs = (EchoAccept(*head, None), EchoAccept(*head, _ptr(self.target_token)))
+            self.__dict__["_cs"] = cs
+        return cs[1 if with_target else 0]
 
     def to_host(self) -> dict:
         return {k: getattr(self, k).cpu().numpy() for k in
@@ -268,6 +301,15 @@ class EchoContext:
         return C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
 
     def ensure_workspace(self, R: int, N: int, capacity: int, Hq: int, Hkv: int = 0):
+        key = (R, N, capacity, Hq, Hkv, self._opts.get(OPT_FORCE_SPLITS, 0) if hasattr(self, "_opts") else 0)
+        if key in self.__dict__.setdefault("_ws_ok", set()):
+            return
+        self._ensure_workspace(R, N, capacity, Hq, Hkv)
+        if len(self._ws_ok) > 1024:
+            self._ws_ok.clear()
+        self._ws_ok.add(key)
+
+    def _ensure_workspace(self, R: int, N: int, capacity: int, Hq: int, Hkv: int = 0):
         splits = int(self.lib.echo_attn_splits(self._h, R, Hkv)) if Hq > 0 and Hkv > 0 else 1
         need = int(self.lib.echo_workspace_bytes(R, N, capacity, Hq, splits))
         if need > self.workspace_bytes:
@@ -337,18 +379,28 @@ class EchoContext:
         self.ensure_workspace(R, N, capacity, 0)
         sel = out if out is not None else self.alloc_selection(R, N, capacity)
         trees = EchoTrees(R, N, max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
-        g = EchoGate()
-        g.depth_mask = int(depth_mask) & 0xFFFFFFFF
-        lt = np.asarray(log_tau, np.float32)
-        for d in range(32):
-            g.log_tau[d] = float(lt[d])
-        g.w_max, g.budget, g.static_k, g.schedule = int(w_max), int(budget), int(static_k), int(schedule)
+        g = self._gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, 0, 0)
         cs = sel.c_struct()
         self._check(self.lib.echo_gate_select(self._h, C.byref(trees), C.byref(g), C.byref(cs), self._stream()))
         return sel
 
+    _gate_cache: dict = {}
+
+    @classmethod
+    def _gate_struct(cls, depth_mask, log_tau, w_max, budget, static_k, schedule, cand_index_base, request_base):
+        """EchoGate of these settings, marshalled once per distinct setting (the structs are read-only to the library)"""
+        lt = np.ascontiguousarray(log_tau, np.float32)
+        key = (int(depth_mask), lt.tobytes(), int(w_max), int(budget), int(static_k), int(schedule), int(cand_index_base),
+               int(request_base))
+        g = cls._gate_cache.get(key)
+        if g is None:
+            if len(cls._gate_cache) > 256:
+                cls._gate_cache.clear()
+            g = cls._gate_cache[key] = cls._make_gate_struct(*key[:1], lt, *key[2:])
+        return g
+
     @staticmethod
-    def _gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, cand_index_base, request_base):
+    def _make_gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, cand_index_base, request_base):
         g = EchoGate()
         g.depth_mask = int(depth_mask) & 0xFFFFFFFF
         lt = np.asarray(log_tau, np.float32)
@@ -421,12 +473,8 @@ class EchoContext:
         assert target_logits.stride(0) == root_logits.stride(0)
         inp = EchoSampleInputs(_ptr(draft_token), _ptr(target_logits), _ptr(root_logits), int(vocab),
                                int(root_logits.stride(0)), float(temperature), _ptr(u_accept), _ptr(u_bonus))
-        ck = kv.c_struct()
-        if not compact:
-            ck.k_pool = None
-            ck.v_pool = None
-        oa = EchoAccept(_ptr(acc.accept_len), _ptr(acc.last_node), _ptr(acc.bonus_token), _ptr(acc.new_len),
-                        _ptr(acc.accept_idx), _ptr(acc.slot_src), _ptr(acc.slot_dst), None)
+        ck = kv.c_struct(with_pools=compact)
+        oa = acc.c_struct(with_target=False)
         cs = sel.c_struct()
         self._check(self.lib.echo_accept_stochastic(self._h, C.byref(cs), C.byref(inp), sel.R, C.byref(ck), C.byref(oa),
                                                     self._stream()))
@@ -475,13 +523,8 @@ class EchoContext:
         self.ensure_workspace(sel.R, 0, sel.capacity, 0)
         res = EchoVerifyResult(_ptr(draft_token), _ptr(prev_token), _ptr(target_token), _ptr(target_logits),
                                int(vocab), int(target_logits.stride(0)) if target_logits is not None else 0)
-        ck = kv.c_struct()
-        if not compact:
-            ck.k_pool = None
-            ck.v_pool = None
-        oa = EchoAccept(_ptr(acc.accept_len), _ptr(acc.last_node), _ptr(acc.bonus_token), _ptr(acc.new_len),
-                        _ptr(acc.accept_idx), _ptr(acc.slot_src), _ptr(acc.slot_dst),
-                        _ptr(acc.target_token) if target_logits is not None else None)
+        ck = kv.c_struct(with_pools=compact)
+        oa = acc.c_struct(with_target=target_logits is not None)
         cs = sel.c_struct()
         self._check(self.lib.echo_accept(self._h, C.byref(cs), C.byref(res), sel.R, C.byref(ck), C.byref(oa),
                                          self._stream()))
