@@ -1015,7 +1015,17 @@ static int encode_pool(EchoCtx* ctx, CUtensorMap* m, const void* pool, uint64_t 
 }
 
 #ifdef ECHO_WAIT_PROF
+static const int4* g_dbg_items = nullptr;     // the last launch's work list (debug build only)
+static const int32_t* g_dbg_n_items = nullptr;
 extern "C" int echo_debug_wait_prof(EchoCtx* ctx, uint64_t* host_out, int32_t n_ctas) {
+  if (ctx && host_out && n_ctas <= -3) {  // the work list of the last launch: up to -n_ctas records of 8 int32; returns n_items
+    int32_t n = 0;
+    ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
+    ECHO_CUDA_TRY(ctx, cudaMemcpy(&n, g_dbg_n_items, 4, cudaMemcpyDeviceToHost));
+    const int m = n < -n_ctas ? n : -n_ctas;
+    ECHO_CUDA_TRY(ctx, cudaMemcpy(host_out, g_dbg_items, (size_t)m * 32, cudaMemcpyDeviceToHost));
+    return n;
+  }
   if (ctx && host_out && n_ctas == -1) {  // event trace of CTA 0: [256 tiles][8 events] clock64
     ECHO_CUDA_TRY(ctx, cudaDeviceSynchronize());
     ECHO_CUDA_TRY(ctx, cudaMemcpyFromSymbol(host_out, g_trace, sizeof(long long) * 256 * 8));
@@ -1057,6 +1067,10 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   uint8_t* plan = reinterpret_cast<uint8_t*>(ctx->workspace) + part_bytes;
   int32_t* n_items = reinterpret_cast<int32_t*>(plan);
   int4* items = reinterpret_cast<int4*>(plan + 256);
+#ifdef ECHO_WAIT_PROF
+  g_dbg_items = items;
+  g_dbg_n_items = n_items;
+#endif
   ECHO_CUDA_TRY(ctx, launch_pdl(k_plan, dim3(1), dim3(PLAN_THREADS), 0, st, sel->sel_offsets, kv->prefix_len, R, Hkv, G,
                                 splits, (int)max_items, max_rt, items, n_items, ctx->dev_status));
 

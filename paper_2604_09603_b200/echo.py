@@ -24,6 +24,7 @@ ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
 MAX_ACCEPT = 32
 CUT_NEVER = 0x7FFFFFFF
 DEV_BAD_PARENT, DEV_BAD_LOGQ, DEV_DEPTH_OVERFLOW, DEV_PAGE_OVERFLOW = 1, 2, 4, 8
+DEV_BAD_TRACE, DEV_CALIB_OVERFLOW, DEV_TREE_OVERFLOW, DEV_CAND_OVERFLOW, DEV_INTERNAL = 16, 32, 64, 128, 256
 
 EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror", "echo_last_error",
            "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_launch_count", "echo_probe_sm_clock",

@@ -125,6 +125,49 @@ def test_device_status_flags_bad_inputs():
     assert ctx.device_status() == 0
 
 
+def test_gate_select_empty_batch_and_requests_without_candidates():
+    """R = 0 selects nothing and writes sel_offsets[0] = n_selected = 0; requests without candidates (equal
+    offsets) sit between requests that have some, first and last included."""
+    import torch
+    ctx = get_ctx()
+    z32 = lambda n: torch.zeros(n, dtype=torch.int32, device="cuda")
+    sel = ctx.gate_select(z32(1), z32(0), torch.zeros(0, device="cuda"), 0, np.zeros(32, np.float32), 0, 8, capacity=8)
+    torch.cuda.synchronize()
+    assert int(sel.n_selected.item()) == 0 and int(sel.sel_offsets[0].item()) == 0
+    assert ctx.device_status() == 0
+    wl = W.make_config(0, gated=True)
+    sizes = np.diff(wl.cand_offsets)
+    keep = np.ones(wl.R, bool)
+    keep[[0, wl.R // 2, wl.R - 1]] = False
+    offs = np.concatenate([[0], np.cumsum(np.where(keep, sizes, 0))]).astype(np.int32)
+    rows = np.concatenate([np.arange(wl.cand_offsets[i], wl.cand_offsets[i + 1]) for i in range(wl.R) if keep[i]])
+    parent, logq = wl.parent[rows], wl.logq[rows]
+    g = wl.gate
+    for budget in (5, g.budget):
+        sel = ctx.gate_select(dev(offs), dev(parent), dev(logq), g.depth_mask, g.log_tau, g.w_max, budget,
+                              capacity=max(1, budget))
+        want = orc.gate_select(offs, parent, logq, g.depth_mask, g.log_tau, g.w_max, budget)
+        assert_selection_equal(sel.to_host(), want)
+    assert ctx.device_status() == 0
+
+
+def test_device_status_flags_overflows():
+    """a request with more than 128 candidates (declared as 128) and a chain deeper than 31: flagged, never a trap,
+    and the well-formed request next to them is still selected from"""
+    from paper_2604_09603_b200 import echo
+    ctx = get_ctx()
+    n_big = 140
+    offs = np.asarray([0, n_big, n_big + 40, n_big + 43], np.int32)
+    parent = np.concatenate([np.full(n_big, -1), np.arange(-1, 39), [-1, 0, 0]]).astype(np.int32)   # roots; one chain; a tree
+    logq = np.full(len(parent), -0.1, np.float32)
+    sel = ctx.gate_select(dev(offs), dev(parent), dev(logq), 0, np.zeros(32, np.float32), 0, 16, capacity=16, max_cand=128)
+    got = sel.to_host()
+    f = ctx.device_status()
+    assert f & echo.DEV_CAND_OVERFLOW and f & echo.DEV_DEPTH_OVERFLOW
+    assert got["n_selected"] <= 16 and got["sel_offsets"][-1] == got["n_selected"]
+    assert ctx.device_status() == 0
+
+
 def test_error_codes_on_gpu():
     from paper_2604_09603_b200 import echo
     ctx = get_ctx()
