@@ -550,7 +550,9 @@ def run_e2e(r, args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300, help="timed steps of the headline leg (default: ~100 ms at cfg2)")
+    ap.add_argument("--steps", type=int, default=100,
+                    help="timed steps of the headline leg (default: ~30 ms at cfg2, inside the burst-clock window that "
+                         "MEASURED_PEAKS.json's copy figure was taken in; the sustained leg follows)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: BS=128)")
     ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
