@@ -60,14 +60,6 @@ static_assert(NSTAGE == 3, "K / V stage g % NSTAGE and S buffer g % NSBUF must b
 constexpr int NSBUF = 3;        // S / P buffers in TMEM: the QK^T of tile j+2 is issued before the PV of tile j
 constexpr int TMEM_O = NSBUF * TILE_N;
 constexpr int TMEM_COLS = 512;  // S_b [128 b, 128 b + 128) for b < 3, O [384,512); P_b aliases S_b[0,64)
-// of every POLY_PERIOD weight pairs in a prefix tile, POLY_COUNT take 2^x on the FMA pipe, the rest on MUFU
-#ifndef ECHO_POLY_COUNT
-#define ECHO_POLY_COUNT 1
-#endif
-#ifndef ECHO_POLY_PERIOD
-#define ECHO_POLY_PERIOD 4
-#endif
-constexpr int POLY_PERIOD = ECHO_POLY_PERIOD, POLY_COUNT = ECHO_POLY_COUNT;
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 // The fast form takes every weight as 2^(s * scale * log2e) with no reference subtracted.  fp32 sums and bf16 weights
@@ -233,47 +225,19 @@ __device__ __forceinline__ void mask_chunk(uint32_t (&s)[32], uint32_t vis) {
     if (!((vis >> e) & 1u)) s[e] = 0xff800000u;  // -inf
 }
 
-// 2^x for a pair of finite x on the FMA pipe instead of MUFU (16 ex2 per clock per SM, the busiest pipe of the
-// softmax): n = round(x) by the 1.5*2^23 trick, f = x - n in [-0.5, 0.5], 2^f by a degree-3 minimax polynomial
-// (relative error 7.5e-5, far below the bf16 rounding of P), then n is added to the exponent field.  x is clamped
-// to [-125, 126]: 2^-125 instead of less is far below the window's lower end (so this form is used only where no
-// key is masked), and 2^126 puts the row sum above the window: the item is redone in the safe form.
-__device__ __forceinline__ void ex2_poly_x2(uint64_t x2, float& p0, float& p1) {
-  float x0, x1;
-  tc::unpack_f32x2(x2, x0, x1);
-  x2 = tc::pack_f32x2(fminf(fmaxf(x0, -125.f), 126.f), fminf(fmaxf(x1, -125.f), 126.f));
-  const uint64_t magic = tc::pack_f32x2(12582912.f, 12582912.f), nmagic = tc::pack_f32x2(-12582912.f, -12582912.f);
-  const uint64_t t = tc::add_f32x2(x2, magic);
-  const uint64_t n = tc::add_f32x2(t, nmagic);
-  const uint64_t f = tc::fma_f32x2(n, tc::pack_f32x2(-1.f, -1.f), x2);
-  uint64_t q = tc::fma_f32x2(f, tc::pack_f32x2(0x1.c3f76p-5f, 0x1.c3f76p-5f), tc::pack_f32x2(0x1.f0de1ap-3f, 0x1.f0de1ap-3f));
-  q = tc::fma_f32x2(q, f, tc::pack_f32x2(0x1.62f31ap-1f, 0x1.62f31ap-1f));
-  q = tc::fma_f32x2(q, f, tc::pack_f32x2(0x1.fff692p-1f, 0x1.fff692p-1f));
-  float q0, q1, t0, t1;
-  tc::unpack_f32x2(q, q0, q1);
-  tc::unpack_f32x2(t, t0, t1);
-  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
-  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
-}
-
 // weights p = 2^(s*scale_log2 + neg_m) of one 32-column chunk of a row: packed to bf16 in pk, added to the exact fp32
-// partial sums in acc.  Packed f32x2 FMA / ADD halve the issue slots: straight-line FFMA2 / MUFU / F2FP / FADD2, 2.5
-// issue slots per weight.  A masked key arrives as -inf: MUFU turns it into 0, the polynomial form (which clamps at
-// -125) into 2^-125, which is below anything the row-sum window lets through.
+// partial sums in acc.  Packed f32x2 FMA / ADD halve the issue slots: straight-line FFMA2 / MUFU.EX2 / F2FP / FADD2.  A
+// masked key arrives as -inf and MUFU turns it into 0.  (Round 1-2 took every fourth pair's 2^x on the FMA pipe by a
+// degree-3 polynomial to relieve MUFU; with the present structure that costs 2.5 % -- A/B on one box, cfg2 0.2630 vs
+// 0.2563 ms, static-60 0.656 vs 0.642 -- XU is at 42 % of its peak without it.)
 __device__ __forceinline__ void weights_chunk(const uint32_t (&sc)[32], uint64_t sc2, uint64_t nm2, uint32_t (&pk)[16],
                                               uint64_t (&acc)[4]) {
 #pragma unroll
   for (int e = 0; e < 32; e += 2) {
     const uint64_t x2 = tc::fma_f32x2(tc::pack_f32x2(__uint_as_float(sc[e]), __uint_as_float(sc[e + 1])), sc2, nm2);
-    float p0, p1;
-    if (((e >> 1) % POLY_PERIOD) < POLY_COUNT) {
-      ex2_poly_x2(x2, p0, p1);
-    } else {
-      float x0, x1;
-      tc::unpack_f32x2(x2, x0, x1);
-      p0 = tc::ex2(x0);
-      p1 = tc::ex2(x1);
-    }
+    float x0, x1;
+    tc::unpack_f32x2(x2, x0, x1);
+    const float p0 = tc::ex2(x0), p1 = tc::ex2(x1);
     pk[e >> 1] = tc::pack_bf16(p0, p1);
     acc[(e >> 1) & 3] = tc::add_f32x2(acc[(e >> 1) & 3], tc::pack_f32x2(p0, p1));
   }
