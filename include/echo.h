@@ -44,7 +44,8 @@ typedef enum {
                                 than 2^24 requests over the ranks sharing a budget */
   ECHO_ERR_WORKSPACE = -3,   /* ctx workspace smaller than echo_workspace_bytes(...) for this call */
   ECHO_ERR_ARCH = -4,        /* device is not sm_100 */
-  ECHO_ERR_CUDA = -5         /* a CUDA runtime / driver call failed; text via echo_last_error */
+  ECHO_ERR_CUDA = -5,        /* a CUDA runtime / driver call failed; text via echo_last_error */
+  ECHO_ERR_TOO_LARGE = -6    /* echo_gate_select_noalloc: total_cand > ECHO_NOALLOC_MAX_CAND (its fixed scratch array) */
 } EchoStatus;
 
 /* bits of the device status word */
@@ -218,6 +219,29 @@ int echo_gate_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, E
                    echo_stream_t stream);
 int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, const uint64_t* local_keys,
                           const uint64_t* all_keys, int64_t n_all, EchoSelection* out, echo_stream_t stream);
+
+/* ---- a call that allocates nothing -------------------------------------------------------- */
+/* echo_gate_select for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): no context, no workspace.  The scratch the selection needs -- the 64-bit selection keys
+ * [total_cand] and the threshold, which echo_gate_select keeps in the context's workspace -- lives in a fixed array of
+ * ECHO_NOALLOC_SCRATCH_BYTES (256 + 8 * ECHO_NOALLOC_MAX_CAND = 512.25 KB) that is part of the library image: every
+ * GPU that loads libecho.so holds it until the process exits.  The call makes no cudaMalloc / cudaFree and calls no
+ * allocating library routine; it runs the three-kernel form of the step (score + keys, radix select, pack), results
+ * identical to echo_gate_select.
+ *   - Runs on the calling thread's CURRENT device (compute capability 10.0, else ECHO_ERR_ARCH); `stream` and every
+ *     dev pointer must belong to it.  The first call on a device looks up the array's device address (once per
+ *     device): make that first call outside stream capture.
+ *   - trees / gate / out: as for echo_gate_select; out->capacity >= min(budget, total_cand) (static_k: num_requests *
+ *     static_k).  `status`: dev [1], caller-owned; the ECHO_DEV_* bits of data-dependent violations are OR-ed into it
+ *     (the caller zeroes it when it wants to).
+ *   - total_cand > ECHO_NOALLOC_MAX_CAND -> ECHO_ERR_TOO_LARGE, nothing is launched.
+ *   - Every call on a device shares the one array, which keeps the last call's contents; nothing in it has to start
+ *     at zero (every word a call reads it has written before).  Calls that overlap on the GPU -- two streams, two
+ *     threads, two processes' worth of graphs replayed at once -- RACE on it: serialise them on one stream. */
+#define ECHO_NOALLOC_MAX_CAND 65536
+#define ECHO_NOALLOC_SCRATCH_BYTES (256 + 8 * (size_t)ECHO_NOALLOC_MAX_CAND)
+int echo_gate_select_noalloc(const EchoTrees* trees, const EchoGate* gate, EchoSelection* out, uint32_t* status,
+                             echo_stream_t stream);
 
 /* ---- acceptance at temperature > 0 ----------------------------------- */
 typedef struct {

@@ -52,6 +52,7 @@ const char* echo_strerror(int code) {
     case ECHO_ERR_WORKSPACE: return "workspace too small";
     case ECHO_ERR_ARCH: return "device is not sm_100 (B200)";
     case ECHO_ERR_CUDA: return "CUDA error (see echo_last_error)";
+    case ECHO_ERR_TOO_LARGE: return "more candidates than the fixed scratch of echo_gate_select_noalloc holds (ECHO_NOALLOC_MAX_CAND)";
     default: return "unknown error";
   }
 }

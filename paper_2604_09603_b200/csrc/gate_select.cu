@@ -802,3 +802,99 @@ int launch_gate_select(EchoCtx* ctx, const EchoTrees* t, const EchoGate* g, Echo
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;
 }
+
+// ---- echo_gate_select_noalloc (include/echo.h): the three-kernel chain with its scratch in the library image ----
+// Scratch layout: [0, 8) the select threshold, [256, 256 + 8 N) the selection keys.  File-scope device array: every
+// GPU that loads the library holds ECHO_NOALLOC_SCRATCH_BYTES until the process exits.  In HOST code the name below is
+// a host-side stand-in, not a device address: the address a kernel may use comes from cudaGetSymbolAddress, looked up
+// once per device with that device current.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[ECHO_NOALLOC_SCRATCH_BYTES];
+
+#include <mutex>
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+struct NoallocDevice {
+  std::atomic<int> state{0};  // 0 = not set up, 1 = ready, < 0 = the EchoStatus the set-up ended with
+  unsigned char* scratch = nullptr;
+};
+NoallocDevice g_noalloc_dev[NOALLOC_MAX_DEVICES];
+std::mutex g_noalloc_mutex;
+
+// Set-up of the current device `dev`: architecture check and the scratch array's device address.  No allocation.
+int noalloc_setup(int dev, unsigned char** scratch) {
+  NoallocDevice& d = g_noalloc_dev[dev];
+  int st = d.state.load(std::memory_order_acquire);
+  if (st == 0) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    st = d.state.load(std::memory_order_acquire);
+    if (st == 0) {
+      int major = 0, minor = 0;
+      void* ptr = nullptr;
+      if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+          cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess) {
+        st = ECHO_ERR_CUDA;
+      } else if (major != 10 || minor != 0) {
+        st = ECHO_ERR_ARCH;
+      } else if (cudaGetSymbolAddress(&ptr, g_noalloc_scratch) != cudaSuccess || ptr == nullptr) {
+        st = ECHO_ERR_CUDA;
+      } else {
+        d.scratch = static_cast<unsigned char*>(ptr);
+        st = 1;
+      }
+      (void)cudaGetLastError();
+      if (st != ECHO_ERR_CUDA) d.state.store(st, std::memory_order_release);  // a CUDA failure may be transient: retried
+    }
+  }
+  if (st != 1) return st;
+  *scratch = d.scratch;
+  return ECHO_OK;
+}
+}  // namespace
+
+extern "C" int echo_gate_select_noalloc(const EchoTrees* t, const EchoGate* g, EchoSelection* o, uint32_t* status,
+                                        echo_stream_t stream) {
+  // the checks of echo_gate_select (api.cu), plus the scratch limit; nothing below allocates
+  if (!t || !g || !o || !status) return ECHO_ERR_INVALID_ARG;
+  if (t->num_requests < 0 || t->total_cand < 0 || t->max_cand_per_req < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->budget < 0 || g->w_max < 0 || g->static_k < 0 || o->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->cand_index_base < 0 || g->request_base < 0) return ECHO_ERR_INVALID_ARG;
+  if (g->schedule != ECHO_SCHED_TOPB && g->schedule != ECHO_SCHED_ALG1) return ECHO_ERR_INVALID_ARG;
+  if (t->max_cand_per_req > ECHO_MAX_CAND) return ECHO_ERR_UNSUPPORTED;
+  if (g->schedule == ECHO_SCHED_ALG1 && (int64_t)g->request_base + t->num_requests > (1 << 24)) return ECHO_ERR_UNSUPPORTED;
+  if (!t->cand_offsets || !o->cut_depth || !o->n_selected || !o->sel_offsets) return ECHO_ERR_INVALID_ARG;
+  if (t->total_cand > 0 && (!t->parent || !t->logq || !o->path_score || !o->cand_depth)) return ECHO_ERR_INVALID_ARG;
+  long need = g->static_k > 0 ? (long)t->num_requests * g->static_k : (long)g->budget;
+  if (need > t->total_cand) need = t->total_cand;
+  if (o->capacity < need) return ECHO_ERR_INVALID_ARG;
+  if (o->capacity > 0 && (!o->sel_node || !o->sel_req || !o->parent_local || !o->sel_depth || !o->anc_mask))
+    return ECHO_ERR_INVALID_ARG;
+  if (reinterpret_cast<uintptr_t>(o->anc_mask) & 15u) return ECHO_ERR_INVALID_ARG;
+  if (t->total_cand > ECHO_NOALLOC_MAX_CAND) return ECHO_ERR_TOO_LARGE;
+
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) return ECHO_ERR_CUDA;
+  unsigned char* scratch = nullptr;
+  const int rc = noalloc_setup(dev, &scratch);
+  if (rc != ECHO_OK) return rc;
+  uint64_t* threshold = reinterpret_cast<uint64_t*>(scratch);
+  uint64_t* keys = reinterpret_cast<uint64_t*>(scratch + 256);
+
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const int R = t->num_requests, N = t->total_cand;
+  const int budget = g->static_k > 0 ? N : g->budget;
+  if (R > 0) {
+    ECHO_COUNT_LAUNCH();
+    k_score_gate<<<R, ECHO_MAX_CAND, 0, st>>>(t->cand_offsets, t->parent, t->logq, gate_params(g), o->path_score,
+                                               o->cand_depth, o->cut_depth, keys, status);
+  }
+  if (launch_pdl(k_select, dim3(1), dim3(SEL_THREADS), 0, st, t->cand_offsets, keys, R, keys, N, budget, o->n_selected,
+                 o->sel_offsets, threshold) != cudaSuccess)
+    return ECHO_ERR_CUDA;
+  if (R > 0 &&
+      launch_pdl(k_pack, dim3(R), dim3(ECHO_MAX_CAND), 0, st, t->cand_offsets, t->parent, o->cand_depth, keys, threshold,
+                 o->capacity, o->sel_offsets, o->sel_node, o->sel_req, o->parent_local, o->sel_depth, o->anc_mask) !=
+          cudaSuccess)
+    return ECHO_ERR_CUDA;
+  return cudaGetLastError() == cudaSuccess ? ECHO_OK : ECHO_ERR_CUDA;
+}

@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libecho.so")
 
 ECHO_OK = 0
-ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5
+ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA, ERR_TOO_LARGE = -1, -2, -3, -4, -5, -6
+NOALLOC_MAX_CAND = 65536  # ECHO_NOALLOC_MAX_CAND: candidates echo_gate_select_noalloc's fixed scratch holds
 OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS, OPT_ATTN_SAFE, OPT_GATE_PATH, OPT_GATE_CLUSTER = 1, 2, 3, 4, 5, 6
 SCHED_TOPB, SCHED_ALG1 = 0, 1  # EchoGate.schedule: global top-B (north_star) / Algorithm 1 as printed
 ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
@@ -30,7 +31,7 @@ EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror
            "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_launch_count", "echo_probe_sm_clock",
            "echo_gate_select", "echo_verify_attn", "echo_accept",
            "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand",
-           "echo_accept_stochastic"]
+           "echo_accept_stochastic", "echo_gate_select_noalloc"]
 
 
 class EchoTrees(C.Structure):
@@ -145,6 +146,8 @@ def load_library():
     lib.echo_calibrate.restype = C.c_int
     lib.echo_gate_select.argtypes = [C.c_void_p, P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p]
     lib.echo_gate_select.restype = C.c_int
+    lib.echo_gate_select_noalloc.argtypes = [P(EchoTrees), P(EchoGate), P(EchoSelection), C.c_void_p, C.c_void_p]
+    lib.echo_gate_select_noalloc.restype = C.c_int
     lib.echo_verify_attn.argtypes = [C.c_void_p, P(EchoSelection), P(EchoPagedKV), C.c_int32, C.c_int32,
                                      C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
     lib.echo_verify_attn.restype = C.c_int
@@ -258,6 +261,25 @@ class Acceptance:
     def to_host(self) -> dict:
         return {k: getattr(self, k).cpu().numpy() for k in
                 ("accept_len", "last_node", "bonus_token", "new_len", "accept_idx", "slot_src", "slot_dst")}
+
+
+def gate_select_noalloc(cand_offsets, parent, logq, depth_mask: int, log_tau, w_max: int, budget: int, sel: "Selection",
+                        status, static_k: int = 0, schedule: int = 0, max_cand: int = 128) -> "Selection":
+    """echo_gate_select_noalloc: echo_gate_select without a context or workspace and without any allocation (its
+    scratch is a fixed array in the library; at most NOALLOC_MAX_CAND candidates).  Runs on torch's current device
+    and stream; `sel` (e.g. from EchoContext.alloc_selection) and `status` (int32 device tensor [1], flags are OR-ed
+    in) are the caller's.  Calls that overlap on the GPU race on the scratch."""
+    import torch
+    lib = load_library()
+    R, N = cand_offsets.numel() - 1, parent.numel()
+    trees = EchoTrees(R, N, max_cand, _ptr(cand_offsets), _ptr(parent), _ptr(logq))
+    g = EchoContext._gate_struct(depth_mask, log_tau, w_max, budget, static_k, schedule, 0, 0)
+    cs = sel.c_struct()
+    rc = lib.echo_gate_select_noalloc(C.byref(trees), C.byref(g), C.byref(cs), _ptr(status),
+                                      C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != ECHO_OK:
+        raise EchoError(rc, lib.echo_strerror(rc).decode())
+    return sel
 
 
 class EchoContext:
