@@ -66,6 +66,8 @@ typedef enum {
 #define ECHO_OPT_ATTN_SAFE 4      /* 1: the tcgen05 kernel takes every item in its safe form (running row maximum) */
 #define ECHO_OPT_GATE_PATH 5      /* echo_gate_select: 0 = auto, 1 = three kernels (score, select, pack), 2 = one
                                      thread-block cluster (ECHO_ERR_UNSUPPORTED past 32 requests per CTA) */
+#define ECHO_OPT_ATTN_PLAN 7      /* tcgen05 kernel's work list: 0 = auto (planned inside the kernel for up to 512 (request,
+                                     split) pairs, else by a planner kernel in front of it), 1 = always the planner kernel */
 #define ECHO_OPT_GATE_CLUSTER 6   /* >0: cluster size of that kernel (1, 2, 4, 8, 16; default: one CTA per 8 requests) */
 
 #define ECHO_MAX_CAND 128   /* C_i <= 128 candidates per request (R:G-14) */

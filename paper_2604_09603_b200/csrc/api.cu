@@ -151,6 +151,10 @@ int echo_set_option(EchoCtx* ctx, int key, int64_t value) {
       if (value < 0 || value > 2) return ECHO_ERR_INVALID_ARG;
       ctx->opt_gate_path = value;
       return ECHO_OK;
+    case ECHO_OPT_ATTN_PLAN:
+      if (value < 0 || value > 1) return ECHO_ERR_INVALID_ARG;
+      ctx->opt_attn_plan = value;
+      return ECHO_OK;
     case ECHO_OPT_GATE_CLUSTER:
       if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16) return ECHO_ERR_INVALID_ARG;
       ctx->opt_gate_cluster = value;

@@ -23,6 +23,7 @@ struct EchoCtx {
   int64_t opt_num_ctas;
   int64_t opt_attn_safe;
   int64_t opt_gate_path, opt_gate_cluster;
+  int64_t opt_attn_plan;
   int gate_cluster_max;  // 0 = not probed yet, -1 = no cluster launch on this device
   TmapCache* tmaps;
   bool attn_attr_set, calib_attr_set;  // cudaFuncSetAttribute is per device, i.e. per context

@@ -96,7 +96,15 @@ struct AttnParams {
   float* part_lse;
   size_t n_rows_cap;
   uint32_t* status;
+  // in-kernel planning (plan_in_kernel != 0): every CTA builds the work list itself and writes its own records
+  int plan_in_kernel, R, max_items, max_rt;
+  int4* items_w;
+  int32_t* n_items_w;
 };
+// Up to INPLAN_MAX (request, split) entries are planned inside the attention kernel (one entry per thread, NTHREADS);
+// tile counts above INPLAN_BUCKETS - 1 share the last bucket (as in k_plan).
+constexpr int INPLAN_MAX = 512;
+constexpr int INPLAN_BUCKETS = 1024;
 
 // Optional wait-time profile (build with -DECHO_WAIT_PROF): cycles each role spends blocked on each mbarrier,
 // per CTA, read back with echo_debug_wait_prof (csrc/debug_prof.h).  Compiled out otherwise.
@@ -371,10 +379,96 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_verify_attn_tc(const __grid_con
   const uint32_t tmem = *tmem_slot;
   TRACE_K(1);
   // Programmatic dependent launch: everything above (barrier init, TMEM allocation, descriptor prefetch) overlaps
-  // k_plan; the work list is read only after k_plan has completed.
+  // the kernel before (k_plan, or the gate's); sel_offsets / the work list are read only after it has completed.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   TRACE_K(2);
-  const int n_items = *p.n_items;
+  int n_items;
+  if (p.plan_in_kernel) {
+    // The work list without a launch of its own (k_plan: ~5 us in front of every attention call, 10 % of cfg1): every
+    // CTA computes the whole placement -- entries (request, split) bucketed by tile count, longest first, ties by
+    // entry index, so that all CTAs agree -- and writes only the records the snake order gives to itself.  Scratch:
+    // the K ring, which no TMA has written yet.
+    static_assert(NTHREADS == INPLAN_MAX && INPLAN_BUCKETS == 2 * NTHREADS, "one entry and two buckets per thread");
+    int* s_bkt = reinterpret_cast<int*>(gen_base + SMEM_K);
+    int* s_cnt = s_bkt + INPLAN_MAX;
+    int* s_hist = s_cnt + INPLAN_MAX;
+    int* s_wsum = s_hist + INPLAN_BUCKETS;
+    const int t = threadIdx.x;
+    s_hist[2 * t] = 0;
+    s_hist[2 * t + 1] = 0;
+    int bkt = -1, cnt = 0, r = 0, sp = 0, j0 = 0, j1 = 0, n_rt = 1, P = 0, off = 0, Ki = 0;
+    if (t < p.R * p.splits) {
+      r = t / p.splits;
+      sp = t - r * p.splits;
+      off = p.sel_offsets[r];
+      P = p.prefix_len[r];
+      Ki = p.sel_offsets[r + 1] - off;
+      if (Ki > ECHO_MAX_CAND) {  // more packed nodes than a request can have: clamp and flag (never silently truncate)
+        if (cta == 0) atomicOr(p.status, ECHO_DEV_CAND_OVERFLOW);
+        Ki = ECHO_MAX_CAND;
+      }
+      if (Ki > 0) {
+        const int n_tiles = (P + Ki + TILE_N - 1) / TILE_N;
+        n_rt = min((Ki * p.G + TILE_M - 1) / TILE_M, p.max_rt);
+        const int tps = (n_tiles + p.splits - 1) / p.splits;
+        j0 = sp * tps;
+        j1 = min(n_tiles, j0 + tps);
+        if (j0 < n_tiles) {
+          cnt = p.Hkv * n_rt;
+          bkt = INPLAN_BUCKETS - 1 - min(j1 - j0, INPLAN_BUCKETS - 1);
+        }
+      }
+    }
+    s_bkt[t] = bkt;
+    s_cnt[t] = cnt;
+    __syncthreads();
+    if (cnt > 0) atomicAdd(&s_hist[bkt], cnt);
+    __syncthreads();
+    const int h0 = s_hist[2 * t], h1 = s_hist[2 * t + 1];
+    int incl = h0 + h1;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += v;
+    }
+    if (lane == 31) s_wsum[warp] = incl;
+    __syncthreads();  // (also: every bucket count has been read)
+    if (warp == 0) {
+      int w = lane < NTHREADS / 32 ? s_wsum[lane] : 0;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, w, o);
+        if (lane >= o) w += v;
+      }
+      s_wsum[lane] = w;
+    }
+    __syncthreads();
+    const int base = incl - (h0 + h1) + (warp ? s_wsum[warp - 1] : 0);
+    s_hist[2 * t] = base;  // first position of the bucket (bucket 0 = longest)
+    s_hist[2 * t + 1] = base + h0;
+    n_items = min(s_wsum[31], p.max_items);
+    __syncthreads();
+    if (cnt > 0) {
+      int pos = s_hist[bkt];
+      for (int e = 0; e < t; ++e)
+        if (s_bkt[e] == bkt) pos += s_cnt[e];
+      for (int q = 0; q < cnt; ++q) {
+        const int idx = pos + q;
+        const int rnd = idx / grid, pp = idx - rnd * grid;
+        if (((rnd & 1) ? grid - 1 - pp : pp) == cta && idx < p.max_items) {  // item_index(rnd, cta, grid) == idx
+          const int kvh = q / n_rt, rt = q - kvh * n_rt;
+          p.items_w[2 * idx] = make_int4(r, kvh | (rt << 8) | (sp << 16), j0, j1);
+          p.items_w[2 * idx + 1] = make_int4(P, off, Ki, 0);
+        }
+      }
+    }
+    if (cta == 0 && t == 0) *p.n_items_w = n_items;
+    tc::fence_proxy_async();  // the scratch is done with before the TMA writes the K ring
+    __threadfence_block();
+    __syncthreads();          // this CTA's records are in place for its own readers
+  } else {
+    n_items = *p.n_items;
+  }
   const bool force_safe = p.force_safe != 0;
 
   if (warp >= 12) tc::setmaxnreg_dec<REGS_AUX>();
@@ -1035,8 +1129,10 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   g_dbg_items = items;
   g_dbg_n_items = n_items;
 #endif
-  ECHO_CUDA_TRY(ctx, launch_pdl(k_plan, dim3(1), dim3(PLAN_THREADS), 0, st, sel->sel_offsets, kv->prefix_len, R, Hkv, G,
-                                splits, (int)max_items, max_rt, items, n_items, ctx->dev_status));
+  const bool plan_in_kernel = (long)R * splits <= INPLAN_MAX && ctx->opt_attn_plan != 1;
+  if (!plan_in_kernel)
+    ECHO_CUDA_TRY(ctx, launch_pdl(k_plan, dim3(1), dim3(PLAN_THREADS), 0, st, sel->sel_offsets, kv->prefix_len, R, Hkv, G,
+                                  splits, (int)max_items, max_rt, items, n_items, ctx->dev_status));
 
   if (!ctx->attn_attr_set) {  // per context, i.e. per device (the attribute is a per-device property of the function)
     ECHO_CUDA_TRY(ctx, cudaFuncSetAttribute(k_verify_attn_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL));
@@ -1050,6 +1146,8 @@ int launch_verify_attn_tc(EchoCtx* ctx, const EchoSelection* sel, const EchoPage
   p.out = reinterpret_cast<__nv_bfloat16*>(out); p.lse = lse; p.scale_log2 = sm_scale * LOG2E; p.splits = splits;
   p.force_safe = ctx->opt_attn_safe ? 1 : 0;
   p.part_o = part_o; p.part_lse = part_lse; p.n_rows_cap = n_rows; p.status = ctx->dev_status;
+  p.plan_in_kernel = plan_in_kernel ? 1 : 0; p.R = R; p.max_items = (int)max_items; p.max_rt = max_rt;
+  p.items_w = items; p.n_items_w = n_items;
   int grid = ctx->opt_num_ctas > 0 ? (int)ctx->opt_num_ctas : ctx->num_sms;
   if ((size_t)grid > max_items) grid = (int)(max_items ? max_items : 1);
   {

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libecho.so")
 ECHO_OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA, ERR_TOO_LARGE = -1, -2, -3, -4, -5, -6
 NOALLOC_MAX_CAND = 65536  # ECHO_NOALLOC_MAX_CAND: candidates echo_gate_select_noalloc's fixed scratch holds
-OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS, OPT_ATTN_SAFE, OPT_GATE_PATH, OPT_GATE_CLUSTER = 1, 2, 3, 4, 5, 6
+OPT_FORCE_SPLITS, OPT_ATTN_PATH, OPT_NUM_CTAS, OPT_ATTN_SAFE, OPT_GATE_PATH, OPT_GATE_CLUSTER, OPT_ATTN_PLAN = 1, 2, 3, 4, 5, 6, 7
 SCHED_TOPB, SCHED_ALG1 = 0, 1  # EchoGate.schedule: global top-B (north_star) / Algorithm 1 as printed
 ATTN_AUTO, ATTN_SMALLROW, ATTN_TCGEN05 = 0, 1, 2
 MAX_ACCEPT = 32

@@ -22,6 +22,7 @@ def get_ctx():
     ctx.set_option(echo.OPT_ATTN_PATH, 0)
     ctx.set_option(echo.OPT_NUM_CTAS, 0)
     ctx.set_option(echo.OPT_ATTN_SAFE, 0)
+    ctx.set_option(echo.OPT_ATTN_PLAN, 0)
     ctx.set_option(echo.OPT_GATE_PATH, GATE["path"])
     ctx.set_option(echo.OPT_GATE_CLUSTER, GATE["cluster"])
     return ctx

@@ -310,3 +310,33 @@ def test_attn_head_sharded_equals_unsharded(world):
         outs.append(o_r.clone()); lses.append(l_r.clone())
     n = want_sel["n_selected"]
     assert torch.equal(torch.cat(outs, dim=1)[:n], out[:n]) and torch.equal(torch.cat(lses, dim=1)[:n], lse[:n])
+
+
+@pytest.mark.parametrize("cfg,R,splits", [(0, None, 0), (0, None, 3), (1, None, 0), (1, 300, 1), (1, 300, 2), (2, 40, 16)])
+def test_attn_work_list_planned_in_kernel_or_by_k_plan(cfg, R, splits):
+    """The tcgen05 kernel plans its work list itself for up to 512 (request, split) pairs, else k_plan runs in front of
+    it (R x splits = 600 and 640 here; ECHO_OPT_ATTN_PLAN = 1 forces it): same items in another order, so the
+    outputs are equal bit for bit -- and right (oracle on sampled rows)."""
+    import torch
+    from paper_2604_09603_b200 import echo
+    wl = W.make_config(cfg, R=R, gated=True)
+    ctx, sel, want_sel, q, k, v = _setup(wl)
+    kv = make_kv(wl, k, v)
+    ctx.set_option(echo.OPT_ATTN_PATH, 2)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, splits)
+    res = []
+    for plan in (0, 1):
+        ctx.set_option(echo.OPT_ATTN_PLAN, plan)
+        out, lse = ctx.verify_attn(sel, kv, q, SM_SCALE)
+        torch.cuda.synchronize()
+        res.append((out, lse))
+    n = want_sel["n_selected"]
+    assert torch.equal(res[0][0][:n], res[1][0][:n]) and torch.equal(res[0][1][:n], res[1][1][:n])
+    assert ctx.device_status() == 0
+    rng = np.random.default_rng(17)
+    rows = sorted({(int(a), int(b)) for a, b in zip(rng.integers(0, n, 40), rng.integers(0, wl.Hq, 40))})
+    rows += [(0, 0), (n - 1, wl.Hq - 1)]
+    _compare(wl, want_sel, q, k, v, res[0][0], res[0][1], rows=sorted(set(rows)))
+    ctx.set_option(echo.OPT_ATTN_PLAN, 0)
+    ctx.set_option(echo.OPT_ATTN_PATH, 0)
+    ctx.set_option(echo.OPT_FORCE_SPLITS, 0)
