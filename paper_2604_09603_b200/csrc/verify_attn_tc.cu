@@ -1,10 +1,10 @@
 // S6 on the 5th-gen tensor cores: persistent, warp-specialised split-KV verify attention.
 //
 //   work item   = (request i, KV head, 128-row tile of (node, head-in-group) rows, KV split); KV tile = 128 tokens
-//   warps 12,16 = K producers, warps 14,17 = V producers (one lane each): one 4-D TMA box per page (16 tokens x 128 d
-//                 of one KV head), pages looked up in the page table; warp 12 also loads the Q tile (3-D tensor map
-//                 over [node][head][d]).  Two issuing threads per ring because one cp.async.bulk.tensor costs its
-//                 thread 110-170 cycles whatever the box size.
+//   warp 12     = K producer, warp 14 = V producer (all lanes walk the loop, one elected lane issues): one 4-D TMA
+//                 box per page (16 tokens x 128 d of one KV head), pages looked up in the page table one tile ahead.
+//                 "Stage empty" is S-full (K) / S-free (V) of the same tile index, not a barrier of its own.
+//                 The Q tile (3-D tensor map over [node][head][d]) is loaded by the QK^T issuer, warp 13.
 //   warp 13     = issuer of S = Q K^T (SS, K-major x K-major) into one of three S buffers in TMEM
 //   warp 15     = issuer of O += P V (TS: P read from TMEM where the softmax wrote it over S, V as the MN-major B
 //                 operand straight from its TMA layout); accumulators never leave TMEM
@@ -12,12 +12,12 @@
 //                 one warpgroup waits for its S tile, loads it from TMEM or hands P back, the other one computes, so
 //                 the two warps of an SM sub-partition are never stalled together.  Weights are taken against the
 //                 fixed reference 0 (fp32 and bf16 share the exponent range, so no running maximum is needed while
-//                 the row sums stay inside [2^-90, 2^100]); tree mask only in tiles that touch positions >= P_i; part
-//                 of the prefix-tile weights take 2^x on the FMA pipe; P written back to TMEM as bf16 over S.
+//                 the row sums stay inside [2^-90, 2^100]); tree mask only in tiles that touch positions >= P_i; every
+//                 2^x on MUFU (ex2.approx), packed f32x2 FMA / ADD; P written back to TMEM as bf16 over S.
 //   warps 8-11  = epilogue: O / l -> bf16 out + lse (or the fp32 split partial) while the softmax is on the next item;
 //                 it also checks the row sums: an item with a sum outside the window is flagged and redone at the end
 //                 by the same CTA in the SAFE form (running row maximum, O rescaled in TMEM; warpgroup 0 alone).
-//   setmaxnreg  : softmax 160, epilogue 80, single-lane warps 40 registers
+//   setmaxnreg  : softmax 192, epilogue 80, producer / issuer warps 40 registers
 // Each KV page is read once per (KV head, row tile) and serves all rows of the tile.
 // Operator definition: include/echo.h (paper: P:39, P:85 names it only; readings R:A-1..A-8).
 #include <cuda.h>
