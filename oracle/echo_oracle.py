@@ -20,6 +20,9 @@ scikit-learn roc_auc_score / roc_curve), `draft_expand`
 (tests/test_oracle_draft_pins.py: hand example, brute-force top-k, Eq. 5 scores of
 the built tree), `accept_stochastic` (tests/test_oracle_stochastic_pins.py: hand
 example, emitted-token distribution on a grid of uniforms, T -> 0 = `accept`).
+`argmax_shard_pairs` / `merge_argmax_pairs` (SURVEY 8(e), vocabulary-sharded S8;
+tests/test_oracle_pins.py: merged over any partition they are `argmax_bf16`, with
+ties, -0 / +0 and all -inf rows across the shard boundaries).
 The paper prints no numeric example of this path, so parity with
 "the paper's values" is unpinned; every function below is pinned by the
 mathematics listed above.
@@ -279,6 +282,30 @@ def argmax_bf16(logits_bits, vocab):
     numpy.argmax returns the first occurrence; pinned against an explicit strict-'>' scan."""
     x = (np.asarray(logits_bits)[:, :vocab].astype(np.uint32) << 16).view(np.float32)
     return np.argmax(x, axis=1).astype(np.int32)
+
+
+def argmax_shard_pairs(logits_bits, v0, v1):
+    """S8 on one vocabulary shard (tensor-parallel ranks hold columns [v0, v1) of the logits): per row
+    the shard's maximum (fp32 value of the bf16 logit, -0 taken as +0, S:C-3) and the GLOBAL index of its first
+    occurrence.  Pinned (tests/test_oracle_pins.py): merged over any partition of the vocabulary it is `argmax_bf16`."""
+    x = (np.asarray(logits_bits)[:, v0:v1].astype(np.uint32) << 16).view(np.float32)
+    j = np.argmax(x, axis=1)
+    val = x[np.arange(x.shape[0]), j] + np.float32(0.0)
+    return val.astype(np.float32), (v0 + j).astype(np.int32)
+
+
+def merge_argmax_pairs(values, indices):
+    """values / indices [W][rows] from `argmax_shard_pairs` -> token per row: the greatest value, then the lowest
+    index (the first maximum of the whole row, S:C-3)."""
+    values, indices = np.asarray(values), np.asarray(indices)
+    out = np.zeros(values.shape[1], np.int32)
+    for r in range(values.shape[1]):
+        best = 0
+        for w in range(1, values.shape[0]):
+            if values[w, r] > values[best, r] or (values[w, r] == values[best, r] and indices[w, r] < indices[best, r]):
+                best = w
+        out[r] = indices[best, r]
+    return out
 
 
 # ---------------------------------------------------------------- O9 (S9)

@@ -182,6 +182,46 @@ def test_argmax_pins():
     assert got[0] == 30 and got[1] == 0 and got[2] == V - 1
 
 
+def _partitions(V):
+    """vocabulary partitions: equal shards of 1, 2, 3, 8 ranks, a lopsided one, and one with empty shards"""
+    eq = lambda W_: [(V * r // W_, V * (r + 1) // W_) for r in range(W_)]
+    return [eq(1), eq(2), eq(3), eq(8), [(0, 1), (1, V - 1), (V - 1, V)], [(0, 8), (8, 8), (8, V)]]
+
+
+def test_sharded_argmax_is_the_argmax():
+    """SURVEY 8(e), vocabulary-sharded S8: per-shard (maximum, first index) pairs merged by (greater value, then lower
+    index) give the first maximum of the whole row -- for every partition, with the maximum duplicated across shard
+    boundaries, -0 / +0 in different shards, all-equal and all -inf rows."""
+    rng = np.random.default_rng(11)
+    V, ld = 1000, 1024
+    bits = lambda v: f32_to_bf16_bits(np.float32(v))
+    x = f32_to_bf16_bits(rng.standard_normal((8, ld)))
+    x[:, V:] = bits(100.0)                                   # padding beyond the vocabulary
+    x[0, 900] = x[0, 499] = x[0, 500] = bits(9.0)            # the same maximum in several shards: lowest index
+    x[1, :] = bits(-1.5)                                     # all equal => 0
+    x[2, :V] = 0xFF80                                        # all -inf => 0
+    x[3, :V] = bits(-2.0); x[3, 700] = 0x8000; x[3, 20] = 0x0000; x[3, 10] = 0x8000   # -0 at 10 wins over +0 at 20
+    x[4, V - 1] = bits(50.0)                                 # last column
+    x[5, :V] = 0xFF80; x[5, 640] = bits(-3.0)                # one finite logit among -inf
+    want = orc.argmax_bf16(x, V)
+    assert want[0] == 499 and want[1] == 0 and want[2] == 0 and want[3] == 10 and want[4] == V - 1 and want[5] == 640
+    for part in _partitions(V):
+        vals, idxs = [], []
+        for v0, v1 in part:
+            if v1 > v0:
+                a, b = orc.argmax_shard_pairs(x, v0, v1)
+                assert ((b >= v0) & (b < v1)).all()
+                assert (bf16_bits_to_f32(x[np.arange(8), b]) == a).all()          # the value is the logit at the index
+                assert (bf16_bits_to_f32(x[:, v0:v1]).max(axis=1) == a).all()     # and the shard's maximum
+                assert not np.signbit(a[a == 0]).any()                            # -0 reported as +0
+                vals.append(a); idxs.append(b)
+        np.testing.assert_array_equal(orc.merge_argmax_pairs(vals, idxs), want, err_msg=str(part))
+    # a wrong tie rule shows: taking the LAST shard on equal values would give 900 / V-1 style answers
+    a0, b0 = orc.argmax_shard_pairs(x, 0, 500)
+    a1, b1 = orc.argmax_shard_pairs(x, 500, V)
+    assert b0[0] == 499 and b1[0] == 500 and a0[0] == a1[0]
+
+
 # ------------------------------------------------------------------ S9 / S10
 def _all_paths(parent_local):
     n = len(parent_local)
