@@ -233,10 +233,17 @@ class Case:
         self.d_in["draft"], self.d_in["target"] = self.h_in["draft"].to(dev), self.h_in["target"].to(dev)
         self.logits = self.root_logits = self.u_acc = self.u_bon = None
         self.temperature = temperature
+        self.vocab_sharded, self.am_bufs = False, {}
         if cfg == 4:
             lg = W.draw_logits(wl, glob, device=str(dev))
             if lg.shape[0] < cap:
                 lg = torch.cat([lg, torch.zeros(cap - lg.shape[0], lg.shape[1], dtype=lg.dtype, device=dev)])
+            if heads and temperature <= 0:
+                # head-sharded ranks hold a vocabulary shard of the logits: S8 = per-rank (max, index)
+                # keys, one all-gather of capacity x 8 B, merge -- sharding.sharded_argmax
+                v0, v1 = sharding.vocab_shard(rank, world, wl.vocab)
+                lg = lg[:, v0:v1].contiguous()
+                self.vocab_sharded = True
             self.logits = lg
             if temperature > 0:  # acceptance at temperature > 0 (NEXT-2) instead of the argmax
                 gen = torch.Generator(device=dev).manual_seed(W.SEED_BASE + 7)
@@ -279,6 +286,10 @@ class Case:
         if self.logits is not None and self.temperature > 0:
             ctx.accept_stochastic(sel_, kv, din["draft"], self.logits, self.root_logits, wl.vocab, self.temperature,
                                   self.u_acc, self.u_bon, out=acc_)
+        elif self.vocab_sharded:
+            tok = self.sharding.sharded_argmax(ctx, sel_, self.logits, self.rank, self.world, wl.vocab, dist=self.dist,
+                                               bufs=self.am_bufs)
+            ctx.accept(sel_, kv, din["draft"], din["prev"], target_token=tok, out=acc_)
         elif self.logits is not None:
             ctx.accept(sel_, kv, din["draft"], din["prev"], target_logits=self.logits, vocab=wl.vocab, out=acc_)
         else:

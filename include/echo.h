@@ -9,7 +9,8 @@
  *     until the work queued on `stream` has finished.  Structs themselves are HOST memory,
  *     read during the call only.
  *   - The hot path is three calls -- echo_gate_select, echo_verify_attn, echo_accept; beside them
- *     echo_gate_keys / echo_gate_select_keys (one budget shared by several ranks),
+ *     echo_gate_keys / echo_gate_select_keys (one budget shared by several ranks), echo_argmax_shard /
+ *     echo_argmax_merge (S8 over vocabulary-sharded logits),
  *     echo_accept_stochastic (temperature > 0), echo_calibrate (warm-up calibration of the gates)
  *     and echo_draft_expand (draft-side tree construction).  Every compute call is asynchronous
  *     on `stream`, never synchronises, never reads a device result on the host (CUDA-graph
@@ -221,6 +222,25 @@ int echo_gate_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, E
                    echo_stream_t stream);
 int echo_gate_select_keys(EchoCtx* ctx, const EchoTrees* trees, const EchoGate* gate, const uint64_t* local_keys,
                           const uint64_t* all_keys, int64_t n_all, EchoSelection* out, echo_stream_t stream);
+
+/* ---- S8 over vocabulary-sharded logits (tensor-parallel ranks) ----------------- */
+/* When the ranks shard the KV heads (attention needs no collective), the target logits are sharded over the
+ * vocabulary: rank r holds logits_shard = dev bf16 [capacity][ld], columns [vocab_base, vocab_base + vocab_shard) of
+ * every packed node's row (ld >= vocab_shard, ld % 8 == 0, 16-byte aligned; vocab_base + vocab_shard < 2^31).  The
+ * greedy target token (first maximum, -0 == +0, R:C-3) then needs the one exchange this split has:
+ *   echo_argmax_shard: pairs_out[k] (dev u64 [capacity], caller-owned) = (order-preserving image of the shard's
+ *     maximum, -0 taken as +0) << 32 | (2^31 - 1 - global index of its first occurrence) for k < n_selected, 0 for
+ *     the rows behind: a greater key is a greater value, then a lower index;
+ *   the ranks all-gather their pairs (capacity x 8 B each, e.g. ncclAllGather) into pairs_all = dev u64
+ *     [world][capacity];
+ *   echo_argmax_merge: target_token_out[k] (dev i32 [capacity]) = the index in the greatest of the row's `world` keys,
+ *     k < n_selected -- what echo_accept computes from the unsharded logits -- to be handed to echo_accept as
+ *     EchoVerifyResult.target_token.
+ * A shard whose logits are all -inf reports its first index, so an all -inf row yields token 0 like echo_accept. */
+int echo_argmax_shard(EchoCtx* ctx, const EchoSelection* sel, const void* logits_shard, int64_t ld, int32_t vocab_shard,
+                      int32_t vocab_base, uint64_t* pairs_out, echo_stream_t stream);
+int echo_argmax_merge(EchoCtx* ctx, const EchoSelection* sel, const uint64_t* pairs_all, int32_t world,
+                      int32_t* target_token_out, echo_stream_t stream);
 
 /* ---- a call that allocates nothing -------------------------------------------------------- */
 /* echo_gate_select for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,

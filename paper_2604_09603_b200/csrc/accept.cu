@@ -76,6 +76,75 @@ __global__ void __launch_bounds__(AM_THREADS) k_argmax_bf16(const int32_t* __res
   }
 }
 
+// ---- S8 over vocabulary-sharded logits (tensor-parallel ranks) ----
+// Each rank holds the columns [vocab_base, vocab_base + vocab_shard) of every logits row.  Its partial result per row
+// is ONE 64-bit key = (order-preserving image of the shard's maximum, -0 canonicalised to +0) << 32 | (INT32_MAX -
+// global index of its first occurrence): the larger key is the greater value, then the lower index (R:C-3), so the
+// argmax over the whole vocabulary is the maximum of the ranks' keys -- one all-gather of rows x 8 B per rank.
+__device__ __forceinline__ uint64_t amax_key(float v, int global_index) {
+  return ((uint64_t)f32_ordered(v + 0.0f) << 32) | (uint64_t)(uint32_t)(0x7fffffff - global_index);
+}
+
+__global__ void __launch_bounds__(AM_THREADS) k_argmax_shard(const int32_t* __restrict__ n_selected,
+                                                             const __nv_bfloat16* __restrict__ logits, int64_t ld,
+                                                             int vocab_shard, int vocab_base,
+                                                             unsigned long long* __restrict__ pairs) {
+  const int row = blockIdx.x;
+  if (row >= *n_selected) {  // rows past the packed nodes: a defined value in the buffer that is gathered
+    if (threadIdx.x == 0) pairs[row] = 0ull;
+    return;
+  }
+  const __nv_bfloat16* rp = logits + (size_t)row * ld;
+  const uint4* rp4 = reinterpret_cast<const uint4*>(rp);
+  const int nvec = vocab_shard / 8;
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  int v = threadIdx.x;
+  for (; v + (AM_UNROLL - 1) * AM_THREADS < nvec; v += AM_UNROLL * AM_THREADS) {
+    uint4 u[AM_UNROLL];
+#pragma unroll
+    for (int t = 0; t < AM_UNROLL; ++t) u[t] = ldg_stream(rp4 + v + t * AM_THREADS);
+#pragma unroll
+    for (int t = 0; t < AM_UNROLL; ++t) amax_chunk(bv, bi, u[t], (v + t * AM_THREADS) * 8);
+  }
+  for (; v < nvec; v += AM_THREADS) amax_chunk(bv, bi, ldg_stream(rp4 + v), v * 8);
+  for (int c = nvec * 8 + threadIdx.x; c < vocab_shard; c += AM_THREADS) {
+    const float x = __bfloat162float(rp[c]);
+    if (x > bv) { bv = x; bi = c; }
+  }
+#pragma unroll
+  for (int ofs = 16; ofs; ofs >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, bv, ofs);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, ofs);
+    amax_upd(bv, bi, ov, oi);
+  }
+  __shared__ float s_v[AM_THREADS / 32];
+  __shared__ int s_i[AM_THREADS / 32];
+  if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = bv; s_i[threadIdx.x >> 5] = bi; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < AM_THREADS / 32; ++w) amax_upd(bv, bi, s_v[w], s_i[w]);
+    if (bi == 0x7fffffff) bi = 0;  // every logit of the shard is -inf: its first index
+    pairs[row] = amax_key(bv, vocab_base + bi);
+  }
+}
+
+// target_token[row] = index held by the largest of the `world` keys of the row (pairs_all [world][capacity])
+constexpr int MG_THREADS = 128;
+__global__ void __launch_bounds__(MG_THREADS) k_argmax_merge(const int32_t* __restrict__ n_selected,
+                                                             const unsigned long long* __restrict__ pairs_all,
+                                                             int world, int capacity,
+                                                             int32_t* __restrict__ target_token) {
+  const int row = blockIdx.x * MG_THREADS + threadIdx.x;
+  if (row >= capacity || row >= *n_selected) return;
+  unsigned long long best = 0ull;
+  for (int w = 0; w < world; ++w) {
+    const unsigned long long k = pairs_all[(size_t)w * capacity + row];
+    best = k > best ? k : best;
+  }
+  target_token[row] = 0x7fffffff - (int)(uint32_t)(best & 0xffffffffull);
+}
+
 constexpr int AC_THREADS = 128;
 
 // S9 + S10: one CTA per request.  Warp 0 decides the path; then every thread owns a column of
@@ -222,10 +291,11 @@ int launch_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult
     int32_t* tout = out->target_token_out ? out->target_token_out : reinterpret_cast<int32_t*>(ctx->workspace);
     if (!out->target_token_out && (size_t)sel->capacity * sizeof(int32_t) > ctx->workspace_bytes)
       return ECHO_ERR_WORKSPACE;
-    if (sel->capacity > 0)
+    if (sel->capacity > 0) {  // (an empty grid is a launch error)
       ECHO_COUNT_LAUNCH();
       k_argmax_bf16<<<sel->capacity, AM_THREADS, 0, st>>>(
           sel->n_selected, reinterpret_cast<const __nv_bfloat16*>(res->target_logits), res->ld, res->vocab, tout);
+    }
     tt = tout;
   }
   if (R > 0) {
@@ -236,6 +306,29 @@ int launch_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult
         have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->k_pool) : (__nv_bfloat16*)nullptr,
         have_pools ? reinterpret_cast<__nv_bfloat16*>(kv->v_pool) : (__nv_bfloat16*)nullptr, out->accept_len, out->last_node,
         out->bonus_token, out->new_len, out->accept_idx, out->slot_src, out->slot_dst));
+  }
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}
+
+int launch_argmax_shard(EchoCtx* ctx, const EchoSelection* sel, const void* logits, int64_t ld, int32_t vocab_shard,
+                        int32_t vocab_base, uint64_t* pairs, cudaStream_t st) {
+  if (sel->capacity > 0) {
+    ECHO_COUNT_LAUNCH();
+    k_argmax_shard<<<sel->capacity, AM_THREADS, 0, st>>>(sel->n_selected, reinterpret_cast<const __nv_bfloat16*>(logits), ld,
+                                                         vocab_shard, vocab_base,
+                                                         reinterpret_cast<unsigned long long*>(pairs));
+  }
+  ECHO_CUDA_TRY(ctx, cudaGetLastError());
+  return ECHO_OK;
+}
+
+int launch_argmax_merge(EchoCtx* ctx, const EchoSelection* sel, const uint64_t* pairs_all, int32_t world,
+                        int32_t* target_token, cudaStream_t st) {
+  if (sel->capacity > 0) {
+    ECHO_COUNT_LAUNCH();
+    k_argmax_merge<<<(sel->capacity + MG_THREADS - 1) / MG_THREADS, MG_THREADS, 0, st>>>(
+        sel->n_selected, reinterpret_cast<const unsigned long long*>(pairs_all), world, sel->capacity, target_token);
   }
   ECHO_CUDA_TRY(ctx, cudaGetLastError());
   return ECHO_OK;

@@ -276,6 +276,27 @@ int echo_calibrate(EchoCtx* ctx, const EchoTraces* t, double delta, EchoCalibrat
   return launch_calibrate(ctx, t, delta, o, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int echo_argmax_shard(EchoCtx* ctx, const EchoSelection* sel, const void* logits_shard, int64_t ld, int32_t vocab_shard,
+                      int32_t vocab_base, uint64_t* pairs_out, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
+  if (!ctx || !sel || !logits_shard || !pairs_out || !sel->n_selected || sel->capacity < 0) return ECHO_ERR_INVALID_ARG;
+  if (vocab_shard <= 0 || vocab_base < 0 || ld < vocab_shard || (int64_t)vocab_base + vocab_shard > INT32_MAX)
+    return ECHO_ERR_INVALID_ARG;
+  if (ld % 8 != 0) return ECHO_ERR_UNSUPPORTED;
+  if (misaligned(logits_shard, 16) || misaligned(pairs_out, 8)) return ECHO_ERR_INVALID_ARG;
+  return launch_argmax_shard(ctx, sel, logits_shard, ld, vocab_shard, vocab_base, pairs_out,
+                             reinterpret_cast<cudaStream_t>(stream));
+}
+
+int echo_argmax_merge(EchoCtx* ctx, const EchoSelection* sel, const uint64_t* pairs_all, int32_t world,
+                      int32_t* target_token_out, echo_stream_t stream) {
+  DeviceGuard dg(ctx);
+  if (!ctx || !sel || !pairs_all || !target_token_out || !sel->n_selected || sel->capacity < 0 || world < 1)
+    return ECHO_ERR_INVALID_ARG;
+  if (misaligned(pairs_all, 8)) return ECHO_ERR_INVALID_ARG;
+  return launch_argmax_merge(ctx, sel, pairs_all, world, target_token_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int echo_accept(EchoCtx* ctx, const EchoSelection* sel, const EchoVerifyResult* res, int32_t R, EchoPagedKV* kv,
                 EchoAccept* out, echo_stream_t stream) {
   DeviceGuard dg(ctx);

@@ -93,6 +93,10 @@ int launch_verify_attn(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32
                        const void* q, void* out, float* lse, float sm_scale, cudaStream_t);
 int launch_accept(EchoCtx*, const EchoSelection*, const EchoVerifyResult*, int32_t R, EchoPagedKV*, EchoAccept*,
                   cudaStream_t);
+int launch_argmax_shard(EchoCtx*, const EchoSelection*, const void* logits, int64_t ld, int32_t vocab_shard,
+                        int32_t vocab_base, uint64_t* pairs, cudaStream_t);
+int launch_argmax_merge(EchoCtx*, const EchoSelection*, const uint64_t* pairs_all, int32_t world, int32_t* target_token,
+                        cudaStream_t);
 // tcgen05 path (verify_attn_tc.cu); returns ECHO_ERR_UNSUPPORTED when the shape cannot use it
 int launch_verify_attn_tc(EchoCtx*, const EchoSelection*, const EchoPagedKV*, int32_t layer, int32_t Hq, int32_t R,
                           const void* q, void* out, float* lse, float sm_scale, int splits, float* part_o,

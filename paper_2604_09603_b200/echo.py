@@ -31,7 +31,7 @@ EXPORTS = ["echo_create", "echo_destroy", "echo_workspace_bytes", "echo_strerror
            "echo_device_status", "echo_set_option", "echo_attn_splits", "echo_launch_count", "echo_probe_sm_clock",
            "echo_gate_select", "echo_verify_attn", "echo_accept",
            "echo_calibrate", "echo_gate_keys", "echo_gate_select_keys", "echo_draft_expand",
-           "echo_accept_stochastic", "echo_gate_select_noalloc"]
+           "echo_accept_stochastic", "echo_gate_select_noalloc", "echo_argmax_shard", "echo_argmax_merge"]
 
 
 class EchoTrees(C.Structure):
@@ -151,6 +151,11 @@ def load_library():
     lib.echo_verify_attn.argtypes = [C.c_void_p, P(EchoSelection), P(EchoPagedKV), C.c_int32, C.c_int32,
                                      C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
     lib.echo_verify_attn.restype = C.c_int
+    lib.echo_argmax_shard.argtypes = [C.c_void_p, P(EchoSelection), C.c_void_p, C.c_int64, C.c_int32, C.c_int32,
+                                      C.c_void_p, C.c_void_p]
+    lib.echo_argmax_shard.restype = C.c_int
+    lib.echo_argmax_merge.argtypes = [C.c_void_p, P(EchoSelection), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.echo_argmax_merge.restype = C.c_int
     lib.echo_accept.argtypes = [C.c_void_p, P(EchoSelection), P(EchoVerifyResult), C.c_int32, P(EchoPagedKV),
                                 P(EchoAccept), C.c_void_p]
     lib.echo_accept.restype = C.c_int
@@ -536,6 +541,29 @@ class EchoContext:
         oc = EchoCalibration(_ptr(out["auc"]), _ptr(out["tau"]), _ptr(out["n_pos"]), _ptr(out["n_neg"]),
                              _ptr(out["depth_mask"]))
         self._check(self.lib.echo_calibrate(self._h, C.byref(tr), C.c_double(delta), C.byref(oc), self._stream()))
+        return out
+
+    def argmax_shard(self, sel: Selection, logits_shard, vocab_base: int, vocab_shard: Optional[int] = None, out=None):
+        """echo_argmax_shard: logits_shard bf16 [capacity][ld], this rank's columns [vocab_base, vocab_base +
+        vocab_shard) of the target logits -> int64 [capacity] (max, first index) keys to all-gather."""
+        import torch
+        if out is None:
+            out = torch.empty(max(1, sel.capacity), dtype=torch.int64, device=self.device)
+        n = int(logits_shard.shape[1] if vocab_shard is None else vocab_shard)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_argmax_shard(self._h, C.byref(cs), _ptr(logits_shard), int(logits_shard.stride(0)), n,
+                                               int(vocab_base), _ptr(out), self._stream()))
+        return out
+
+    def argmax_merge(self, sel: Selection, pairs_all, world: int, out=None):
+        """echo_argmax_merge: pairs_all int64 [world][capacity] (the ranks' gathered keys) -> int32 [capacity] target
+        tokens (rows < n_selected), to be passed to accept(target_token=...)."""
+        import torch
+        if out is None:
+            out = torch.zeros(max(1, sel.capacity), dtype=torch.int32, device=self.device)
+        cs = sel.c_struct()
+        self._check(self.lib.echo_argmax_merge(self._h, C.byref(cs), _ptr(pairs_all), int(world), _ptr(out),
+                                               self._stream()))
         return out
 
     def accept(self, sel: Selection, kv: PagedKV, draft_token, prev_token, target_token=None,

@@ -56,6 +56,46 @@ def shard_attention_inputs(q, k_pool, v_pool, rank: int, world: int):
     return q[:, hq].contiguous(), k_pool[:, :, hkv].contiguous(), v_pool[:, :, hkv].contiguous()
 
 
+def vocab_shard(rank: int, world: int, vocab: int, align: int = 8):
+    """Columns [v0, v1) of the target logits that rank `rank` of a tensor-parallel group holds (with the
+    KV heads sharded, the logits are sharded over the vocabulary): contiguous, in rank order, every boundary but the
+    last a multiple of `align` columns (16-byte rows for the streaming loads), sizes as equal as that allows.  A rank
+    may hold no columns when vocab < world * align."""
+    if world < 1 or not (0 <= rank < world) or vocab < 1 or align < 1:
+        raise ValueError(f"cannot shard a vocabulary of {vocab} over {world} ranks")
+    blocks = (vocab + align - 1) // align
+    b0 = blocks * rank // world
+    b1 = blocks * (rank + 1) // world
+    return min(vocab, b0 * align), min(vocab, b1 * align)
+
+
+def sharded_argmax(ctx, sel, logits_shard, rank: int, world: int, vocab: int, dist=None, bufs=None):
+    """S8 when the ranks hold vocabulary shards of the logits: every rank reduces its columns to one 64-bit (max, first
+    index) key per packed node (echo_argmax_shard), the ranks all-gather the keys (capacity x 8 B each -- the one
+    exchange of the head-sharded path), and every rank takes the greatest key per row (echo_argmax_merge).  Returns the
+    int32 target tokens for ctx.accept(target_token=...).  `logits_shard` = [capacity][v1 - v0] of vocab_shard(rank,
+    world, vocab); `bufs` keeps the key buffers between steps.  No host synchronisation."""
+    import torch
+    if dist is None and world > 1:
+        import torch.distributed as dist  # noqa: PLC0415
+    v0, v1 = vocab_shard(rank, world, vocab)
+    bufs = bufs if bufs is not None else {}
+    cap = max(1, sel.capacity)
+    if "pairs" not in bufs or bufs["pairs"].numel() != cap or bufs["gathered"].numel() != world * cap:
+        bufs["pairs"] = torch.zeros(cap, dtype=torch.int64, device=logits_shard.device)
+        bufs["gathered"] = torch.zeros(world * cap, dtype=torch.int64, device=logits_shard.device)
+        bufs["token"] = torch.zeros(cap, dtype=torch.int32, device=logits_shard.device)
+    if v1 > v0:
+        ctx.argmax_shard(sel, logits_shard, v0, v1 - v0, out=bufs["pairs"])
+    else:
+        bufs["pairs"].zero_()  # a rank without columns: the smallest key, never the maximum
+    if world > 1:
+        dist.all_gather_into_tensor(bufs["gathered"], bufs["pairs"])
+    else:
+        bufs["gathered"].copy_(bufs["pairs"])
+    return ctx.argmax_merge(sel, bufs["gathered"], world, out=bufs["token"])
+
+
 def rank_bases(sizes, rank: int):
     """Exclusive prefix sum of per-rank sizes (candidates or requests): the base this rank's keys carry."""
     return int(sum(int(x) for x in sizes[:rank]))

@@ -56,6 +56,8 @@ def test_null_arguments_rejected(lib):
     assert lib.echo_accept_stochastic(None, None, None, 0, None, None, None) == -1
     assert lib.echo_calibrate(None, None, C.c_double(0.5), None, None) == -1
     assert lib.echo_draft_expand(None, None, None, None, None, None) == -1
+    assert lib.echo_argmax_shard(None, None, None, 8, 8, 0, None, None) == -1
+    assert lib.echo_argmax_merge(None, None, None, 1, None, None) == -1
     assert lib.echo_destroy(None) == -1
     assert lib.echo_set_option(None, 1, 1) == -1
 

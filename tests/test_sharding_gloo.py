@@ -124,3 +124,67 @@ def test_global_budget_exchange_under_gloo():
     assert res[0]["local"] == list(range(7)) and res[1]["local"] == [7000 + i for i in range(4)]
     assert res[0]["budget"] == res[1]["budget"] == 5
     assert sharding.rank_bases([3, 4, 5], 2) == 7 and sharding.rank_bases([3, 4, 5], 0) == 0
+
+
+def test_vocab_shards_partition_the_vocabulary():
+    for V, W_ in [(151936, 1), (151936, 2), (151936, 8), (128256, 4), (1000, 3), (1003, 8), (20, 8), (5, 2)]:
+        edges = [sharding.vocab_shard(r, W_, V) for r in range(W_)]
+        assert edges[0][0] == 0 and edges[-1][1] == V
+        for (a0, a1), (b0, b1) in zip(edges, edges[1:]):
+            assert a1 == b0 and a0 <= a1                         # contiguous, in rank order
+        assert all(v0 % 8 == 0 for v0, _ in edges)               # 16-byte aligned shard starts
+        sizes = [v1 - v0 for v0, v1 in edges]
+        if V >= 8 * W_:
+            assert max(sizes) - min(sizes) <= 8 + 7              # as equal as whole 8-column blocks allow
+    with pytest.raises(ValueError):
+        sharding.vocab_shard(2, 2, 100)
+
+
+class _FakeArgmaxCtx:
+    """stands in for the two kernels of the vocabulary-sharded S8 (no GPU here): keys in the layout echo.h gives them"""
+
+    def argmax_shard(self, sel, logits_shard, vocab_base, vocab_shard=None, out=None):
+        x = logits_shard.float().numpy()
+        j = x.argmax(axis=1)
+        v = (x[np.arange(x.shape[0]), j] + np.float32(0)).astype(np.float32).view(np.uint32).astype(np.uint64)
+        o = np.where(v >> 31, ~v & 0xFFFFFFFF, v | 0x80000000)
+        key = (o << np.uint64(32)) | (np.uint64(0x7FFFFFFF) - (vocab_base + j).astype(np.uint64))
+        out.copy_(torch.from_numpy(key.view(np.int64)))
+        return out
+
+    def argmax_merge(self, sel, pairs_all, world, out=None):
+        k = pairs_all.numpy().view(np.uint64).reshape(world, -1)
+        out.copy_(torch.from_numpy((0x7FFFFFFF - (k.max(axis=0) & np.uint64(0xFFFFFFFF)).astype(np.int64)).astype(np.int32)))
+        return out
+
+
+class _Sel:
+    capacity = 5
+
+
+def _worker_vocab(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        V = 40
+        g = torch.Generator().manual_seed(3)
+        full = torch.randn(_Sel.capacity, V, generator=g).to(torch.bfloat16)
+        full[0, 7] = full[0, 33] = 9.0          # the same maximum on both ranks: rank 0's index wins
+        full[1, 39] = 9.0                       # last column, rank 1
+        v0, v1 = sharding.vocab_shard(rank, world, V)
+        tok = sharding.sharded_argmax(_FakeArgmaxCtx(), _Sel(), full[:, v0:v1], rank, world, V, dist=dist)
+        out[rank] = dict(tok=tok.tolist(), want=full.float().argmax(dim=1).tolist(), shard=(v0, v1))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sharded_argmax_exchange_under_gloo():
+    """the head-sharded path's one exchange: both ranks end with the argmax over the WHOLE vocabulary"""
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker_vocab, args=(2, _free_port(), out), nprocs=2, join=True)
+        res = {k: dict(v) for k, v in out.items()}
+    assert res[0]["shard"] == (0, 16) and res[1]["shard"] == (16, 40)
+    assert res[0]["tok"] == res[1]["tok"] == res[0]["want"]
+    assert res[0]["tok"][0] == 7 and res[0]["tok"][1] == 39
+
