@@ -23,6 +23,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 SM_SCALE = 1.0 / np.sqrt(128.0)
+NOMINAL_GBS, NOMINAL_TFLOPS = 8000.0, 2250.0  # BASELINE.json north_star: "about 8 TB/s"; dense bf16 nominal
 WORKLOADS = {1: "cfg1 LLaMA-3.1-8B shape BS=32 B=1024", 2: "cfg2 LLaMA-3.3-70B shape BS=128 B=2048",
              3: "cfg3 Qwen3-235B shape BS=128 B=1024", 4: "cfg4 stress BS=256 B=4096 logits argmax",
              0: "cfg0 tiny"}
@@ -308,6 +309,9 @@ class Case:
         return {"bound": "tensor" if tensor_bound else "hbm", "achieved": tfl if tensor_bound else gbs,
                 "peak": tpeak if tensor_bound else peak, "unit": "TFLOP/s" if tensor_bound else "GB/s",
                 "frac": tfl / tpeak if tensor_bound else gbs / peak, "peak_source": tpeak_src if tensor_bound else peak_src,
+                # the same figure against the nominal roofs north_star names (about 8 TB/s; 2.25 PFLOP/s dense bf16)
+                "frac_nominal": tfl / NOMINAL_TFLOPS if tensor_bound else gbs / NOMINAL_GBS,
+                "peak_nominal": NOMINAL_TFLOPS if tensor_bound else NOMINAL_GBS,
                 "attn_ms": attn_ms, "bytes_per_launch": self.bytes_alg, "flops_per_launch": self.flops_alg}
 
 
@@ -615,7 +619,7 @@ def main():
                 if f and f[0] == f"cfg{args.config}":
                     traffic, traffic_src = int(f[1]), "not measured in this run: " + ",".join(f[3:])
         splits = int(r["ctx"].lib.echo_attn_splits(r["ctx"]._h, wl.R, wl.Hkv)) if not args.splits else args.splits
-        roofline = {k_: roof[k_] for k_ in ("bound", "achieved", "peak", "unit", "frac")}
+        roofline = {k_: roof[k_] for k_ in ("bound", "achieved", "peak", "unit", "frac", "frac_nominal", "peak_nominal")}
         roofline.update(traffic=traffic, traffic_source=traffic_src, peak_source=roof["peak_source"],
                         kernel="echo_verify_attn (k_plan + k_verify_attn_tc" + (" + k_lse_merge)" if splits > 1 else ")"),
                         bytes_per_launch=case.bytes_alg, flops_per_launch=case.flops_alg)

@@ -53,6 +53,24 @@ def test_roofline_picks_the_bounding_roof():
     assert 100 < ai[(2, False)] < 130 and 380 < ai[(2, True)] < 410          # AI ~ K_i G: SURVEY's 114-126 / 396
 
 
+def test_roofline_object_arithmetic():
+    """Case.roofline on the pinned cfg2 / static-60 work: achieved = algorithmic bytes (FLOPs) / time, fractions
+    against the measured and the nominal roof (no GPU needed: the object only holds the two counts)"""
+    c = bench.Case.__new__(bench.Case)
+    c.bytes_alg, c.flops_alg = PINS[(2, False)][:2]
+    r = c.roofline(0.25)
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["bytes_per_launch"] == 1365385216
+    assert r["achieved"] == pytest.approx(1365385216 / 0.25e-3 / 1e9)
+    assert r["frac"] == pytest.approx(r["achieved"] / bench.peaks()[0])
+    assert r["frac_nominal"] == pytest.approx(r["achieved"] / 8000.0) and r["peak_nominal"] == 8000.0
+    c.bytes_alg, c.flops_alg = PINS[(2, True)][:2]
+    r = c.roofline(0.64, sustained=True)
+    assert r["bound"] == "tensor" and r["unit"] == "TFLOP/s"
+    assert r["achieved"] == pytest.approx(619870912512 / 0.64e-3 / 1e12)
+    assert r["frac"] == pytest.approx(r["achieved"] / bench.tensor_peak(True)[0])
+    assert r["frac_nominal"] == pytest.approx(r["achieved"] / 2250.0)
+
+
 def test_clock_sampler_summary_parses_nvidia_smi_rows():
     s = bench.ClockSampler(0)
     rows = [["1965", "1965", "310.5", "Not Active", "Not Active", "Not Active", "Not Active"],
