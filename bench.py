@@ -125,10 +125,24 @@ def algorithmic_bytes(wl, sel_h):
     return int(kvb + qo), int(flops)
 
 
-def oracle_sample(wl, n_attn_nodes=6, qkv=None):
-    """The CPU oracle as it stands on a bounded sample: gating + acceptance on the whole batch,
-    attention (all Hq heads) for `n_attn_nodes` packed nodes.  Returns (tokens/s, description, cores)."""
-    from oracle import echo_oracle as orc           # cpu_baseline / reference arm only
+def host_qkv_bits(wl, n):
+    """bf16 bit patterns for the oracle legs: the CPU time depends on shapes only, so finite random patterns (|x| in
+    [2^-7, 2), random signs) stand in for the device's N(0,1) draw; K and V share one pool"""
+    rng = np.random.default_rng(1)
+
+    def bits(shape):
+        return (rng.integers(0x3C00, 0x4000, size=shape, dtype=np.uint16) |
+                (rng.integers(0, 2, size=shape, dtype=np.uint16) << 15))
+    pool = bits((1, wl.num_pages, wl.Hkv, 16, 128))
+    return bits((max(1, n), wl.Hq, 128)), pool, pool
+
+
+def oracle_sample(wl, n_attn_nodes=6, qkv=None, sel=None):
+    """The CPU oracle as it stands on a bounded sample: gating + acceptance (numpy, one core) on the whole batch,
+    attention (all Hq heads; the plain-C restatement of the definition, oracle/echo_oracle_attn.c, on every host core
+    this process may use) for `n_attn_nodes` packed nodes, all of them if the batch has no more.
+    Returns (tokens/s, description, threads used by the attention, which is > 98 % of the work)."""
+    from oracle import attn_c, echo_oracle as orc    # cpu_baseline / reference arm only
     g = wl.gate
     t0 = time.perf_counter()
     sel = orc.gate_select(wl.cand_offsets, wl.parent, wl.logq, g.depth_mask, g.log_tau, g.w_max, g.budget, g.static_k)
@@ -139,26 +153,22 @@ def oracle_sample(wl, n_attn_nodes=6, qkv=None):
     orc.accept(sel, wl.draft_token[glob], wl.prev_token, wl.target_after[glob], wl.R)
     t_acc = time.perf_counter() - t0
     rng = np.random.default_rng(1)
-    nodes = sorted(set(int(x) for x in rng.integers(0, max(1, n), size=n_attn_nodes)))
-    if qkv is None:
-        # same distribution as the GPU arm (bf16 N(0,1)), drawn on the host for the sampled requests only
-        # timing depends on shapes only: finite bf16 bit patterns (|x| in [2^-7, 2)) with random signs
-        def bits(shape):
-            return (rng.integers(0x3C00, 0x4000, size=shape, dtype=np.uint16) |
-                    (rng.integers(0, 2, size=shape, dtype=np.uint16) << 15))
-        qb = bits((max(1, n), wl.Hq, 128))
-        pool = bits((1, wl.num_pages, wl.Hkv, 16, 128))
-        kb = vb = pool
+    if n_attn_nodes >= n:
+        nodes = list(range(n))
     else:
-        qb, kb, vb = qkv
+        nodes = sorted(set(int(x) for x in rng.choice(max(1, n), size=n_attn_nodes, replace=False)))
+    qb, kb, vb = qkv if qkv is not None else host_qkv_bits(wl, n)
     rows = [(k, h) for k in nodes for h in range(wl.Hq)]
+    threads = attn_c.host_threads()
+    attn_c.build()
     t0 = time.perf_counter()
-    orc.verify_attn(sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, rows=rows)
+    attn_c.verify_attn(sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, rows=rows, threads=threads)
     t_attn = time.perf_counter() - t0
     t_total = t_attn + (t_gate + t_acc) * len(nodes) / max(1, n)
-    desc = (f"{wl.name}: attention of {len(nodes)} packed nodes x {wl.Hq} heads ({t_attn:.2f}s) + the nodes' share of "
-            f"gating ({t_gate:.2f}s) and acceptance ({t_acc:.2f}s) over all {n} nodes")
-    return len(nodes) / t_total, desc, 1
+    desc = (f"{wl.name}: attention of {len(nodes)} of {n} packed nodes x {wl.Hq} heads by the plain-C fp64 oracle on "
+            f"{threads} threads ({t_attn:.2f}s) + the nodes' share of gating ({t_gate:.2f}s) and acceptance ({t_acc:.2f}s; "
+            f"numpy, one core) over all {n} nodes")
+    return len(nodes) / t_total, desc, threads
 
 
 def run_reference(args, rank, world):
@@ -167,12 +177,13 @@ def run_reference(args, rank, world):
         return
     from paper_2604_09603_b200 import workloads as W
     wl = W.make_config(args.config)
+    qkv = host_qkv_bits(wl, wl.capacity())
     vals = []
     for _ in range(args.warmup):
-        oracle_sample(wl, n_attn_nodes=1)
+        oracle_sample(wl, n_attn_nodes=8, qkv=qkv)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        v, desc, cores = oracle_sample(wl, n_attn_nodes=args.ref_nodes)
+        v, desc, cores = oracle_sample(wl, n_attn_nodes=args.ref_nodes, qkv=qkv)
         vals.append(v)
     dt = time.perf_counter() - t0
     value = float(np.mean(vals))
@@ -573,8 +584,11 @@ def main():
     ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
     ap.add_argument("--attn-path", type=int, default=0)
     ap.add_argument("--splits", type=int, default=0)
-    ap.add_argument("--ref-nodes", type=int, default=32, help="--impl reference: packed nodes of oracle attention per step (~0.75 s)")
-    ap.add_argument("--baseline-nodes", type=int, default=512, help="cpu_baseline leg: packed nodes of oracle attention (~12 s once)")
+    ap.add_argument("--ref-nodes", type=int, default=256,
+                    help="--impl reference: packed nodes of oracle attention per step (~0.2 s on 8 cores at cfg2)")
+    ap.add_argument("--baseline-nodes", type=int, default=2048,
+                    help="cpu_baseline leg: packed nodes of oracle attention (cfg2: the whole batch, ~13 s on 8 cores; "
+                         "cfg4's long prefixes: a quarter of this)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sustained-seconds", type=float, default=2.0,
                     help="length of the second timed leg (back-to-back steps under the power cap); 0 = skip")
@@ -653,7 +667,7 @@ def main():
             line["clocks_sustained"] = sampler.summary(sampler.window("sus0", "sus1"), [r["sustained"]["sm_mhz"]])
         if not args.no_cpu_baseline:
             try:
-                v, desc, cores = oracle_sample(wl, n_attn_nodes=args.baseline_nodes)
+                v, desc, cores = oracle_sample(wl, n_attn_nodes=args.baseline_nodes // (4 if args.config == 4 else 1))
                 line["cpu_baseline"] = {"value": v, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": desc}
             except Exception as e:  # the baseline leg must never take the GPU number down with it
                 line["cpu_baseline"] = {"value": None, "unit": "tokens/s", "cores": 1, "kind": "oracle", "sample": f"failed: {e}"}

@@ -27,6 +27,10 @@ The paper prints no numeric example of this path, so parity with
 "the paper's values" is unpinned; every function below is pinned by the
 mathematics listed above.
 
+`oracle/echo_oracle_attn.c` (wrapper `oracle/attn_c.py`) restates `verify_attn` as plain C loops over POSIX
+threads, for every-row parity at full size and the multi-core CPU baseline; it is pinned against this file's
+`verify_attn` and by closed forms of its own (tests/test_oracle_attn_c_pins.py).
+
 Precision: path scores fp32 sequential root->leaf (north_star); attention fp64.
 """
 from __future__ import annotations

@@ -93,5 +93,6 @@ def test_reference_arm_prints_the_contract_line():
     assert line["higher_is_better"] is True and line["value"] > 0 and line["steps"] == 1 and line["gpu_launches"] == 0
     assert line["config"]["workload"].startswith("cfg1")
     cb = line["cpu_baseline"]
-    assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] == line["value"] and "packed nodes" in cb["sample"]
+    assert cb["kind"] == "oracle" and cb["value"] == line["value"] and "packed nodes" in cb["sample"]
+    assert cb["cores"] == len(os.sched_getaffinity(0)) and f"on {cb['cores']} threads" in cb["sample"]   # the cores it used
     assert line["e2e"] == {"value": line["value"], "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
