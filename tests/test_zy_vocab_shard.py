@@ -101,6 +101,39 @@ def test_sharded_argmax_ties_and_edges(world, V, ld):
     assert ctx.device_status() == 0
 
 
+# keys written out by hand from include/echo.h: ordered(v) = bits | 0x80000000 for v >= 0, ~bits for v < 0 (-0 counts
+# as +0), in the high word; 0x7FFFFFFF - (vocab_base + first index) in the low word
+HAND_KEYS = [  # (planted logits {column: value}, fill value, expected key) for a shard of 16 columns at vocab_base 16
+    ({5: 1.0}, -1.0, 0xBF800000_7FFFFFEA),            # 1.0 = 0x3F800000 at global index 21
+    ({}, -2.0, 0x3FFFFFFF_7FFFFFEF),                  # all -2.0 = 0xC0000000: first index, 16
+    ({}, float("-inf"), 0x007FFFFF_7FFFFFEF),         # all -inf = 0xFF800000: first index
+    ({9: -0.0}, -1.0, 0x80000000_7FFFFFE6),           # -0 reported as +0 at global index 25
+    ({3: 0.5, 12: 0.5}, 0.25, 0xBF000000_7FFFFFEC),   # duplicate maximum 0.5 = 0x3F000000: lower index, 19
+    ({15: 3.0}, 0.0, 0xC0400000_7FFFFFE0),            # last column, global index 31; 3.0 = 0x40400000
+]
+
+
+def test_argmax_shard_keys_by_hand():
+    import torch
+    ctx = get_ctx()
+    wl = W.make_config(0, gated=False)
+    sel = run_gate_select(ctx, wl)
+    assert int(sel.n_selected.item()) >= len(HAND_KEYS)
+    lg = torch.zeros(sel.capacity, 32, dtype=torch.bfloat16, device="cuda")
+    lg[:, :16] = 77.0                                              # another rank's columns: never read
+    for r, (planted, fill, _) in enumerate(HAND_KEYS):
+        lg[r, 16:] = fill
+        for c, val in planted.items():
+            lg[r, 16 + c] = val
+    keys = ctx.argmax_shard(sel, lg[:, 16:], 16).cpu().numpy().view(np.uint64)
+    for r, (_, _, want) in enumerate(HAND_KEYS):
+        assert int(keys[r]) == want, (r, hex(int(keys[r])), hex(want))
+    tok = ctx.argmax_merge(sel, torch.stack([torch.zeros_like(ctx.argmax_shard(sel, lg[:, 16:], 16)),
+                                             ctx.argmax_shard(sel, lg[:, 16:], 16)]), 2).cpu().numpy()
+    assert tok[:len(HAND_KEYS)].tolist() == [21, 16, 16, 25, 19, 31]    # key 0 (a rank without columns) never wins
+    assert ctx.device_status() == 0
+
+
 def test_sharding_helper_one_rank_equals_fused_argmax():
     """sharding.sharded_argmax with one rank (no collective) against echo_accept's own argmax"""
     import torch
