@@ -1,5 +1,5 @@
 """-m gpu parity at BASELINE.json's full sizes and on the branches only large inputs reach:
-cfg1 (R=32), cfg2 and cfg3 (BS=128) attention on every row (the latter two by the plain-C oracle on all host cores);
+cfg1 (R=32) attention on every row (cfg2 / cfg3 on every row: test_zx_attn_every_row.py);
 cfg2 / cfg2-static / cfg3 / cfg4 (R=256) attention on a STRATIFIED row sample
 (first and last row of every 128-row tile, last valid row, deepest and root nodes, for the requests with extreme K_i
 and P_i and 16 random ones, topped up with uniform rows); cfg4 acceptance from the full 4096 x 151 936 logits, greedy
@@ -97,36 +97,6 @@ def test_attn_full_size_stratified_rows(cfg, static, target):
     _check_rows(wl, want_sel, q, k, v, out, lse, rows)
     o_gpu = bf16_bits_to_f32(torch_bf16_to_bits(out))[:n]
     assert np.isfinite(o_gpu).all() and np.isfinite(lse.cpu().numpy()[:n]).all()
-
-
-@pytest.mark.parametrize("cfg,static,requests", [(2, False, None), (3, False, None), (2, True, 24), (4, False, 32)])
-def test_attn_full_size_every_row(cfg, static, requests):
-    """cfg2 and cfg3 at full size: EVERY (node, head) row -- 131 072 / 65 536 of them -- against the fp64 definition,
-    computed by the plain-C oracle on all host cores ("full parity on cfg0-3"); the static-60 run (491 520
-    rows) on every row of a seeded sample of 24 requests, cfg4 (R = 256, prefixes up to 32 768) on every row of a seeded
-    sample of 32 requests ("else on a seeded sample of 32 requests")."""
-    from oracle import attn_c
-    wl = W.make_config(cfg, static=static, gated=not static)
-    want_sel, q, k, v, out, lse = _attn_case(wl)
-    n = want_sel["n_selected"]
-    qb, kb, vb = torch_bf16_to_bits(q), torch_bf16_to_bits(k), torch_bf16_to_bits(v)
-    o_gpu = bf16_bits_to_f32(torch_bf16_to_bits(out))[:n]
-    l_gpu = lse.cpu().numpy()[:n]
-    assert np.isfinite(o_gpu).all() and np.isfinite(l_gpu).all()
-    if requests is None:
-        O, L = attn_c.verify_attn(want_sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE)
-        eo, el = np.abs(o_gpu - O).max(), np.abs(l_gpu - L).max()
-    else:
-        offs = want_sel["sel_offsets"]
-        act = np.flatnonzero(np.diff(offs) > 0)
-        reqs = np.sort(np.random.default_rng(400 + cfg).choice(act, size=min(requests, len(act)), replace=False))
-        nodes = np.concatenate([np.arange(offs[i], offs[i + 1]) for i in reqs])
-        rows = [(int(k_), h) for k_ in nodes for h in range(wl.Hq)]
-        O, L = attn_c.verify_attn(want_sel, qb, kb, vb, wl.page_table, wl.prefix_len, wl.Hq, wl.Hkv, SM_SCALE, rows=rows)
-        eo = np.abs(o_gpu[nodes].reshape(-1, 128) - O).max()
-        el = np.abs(l_gpu[nodes].reshape(-1) - L).max()
-    assert eo <= TOL_O, f"max|dO| = {eo}"
-    assert el <= TOL_LSE, f"max|dlse| = {el}"
 
 
 def test_attn_many_requests_planner_multi_pass():
